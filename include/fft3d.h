@@ -1,0 +1,127 @@
+/*
+ * fft3d.h -- C ABI of the B200-native slab-decomposed 3D real-to-complex / complex-to-real FFT.
+ *
+ * The operation is the one "Scalable Multi-node Fast Fourier Transform on GPUs"
+ * (arXiv 2202.12756) distributes over p GPUs; here the p slabs are VIRTUAL and live on one
+ * GPU, so the paper's MPI all-to-all becomes a layout permutation that is folded into the
+ * FFT passes.  Citations: P:n = PAPER.md line n (the paper's text), D:x = DESIGN.md section.
+ *
+ *   forward  F(kx,ky,kz) = sum_j f(jx,jy,jz) exp(-2 pi i [jx kx/Nx + jy ky/Ny + jz kz/Nz])
+ *            kx in [0,Nx), ky in [0,Ny), kz in [0,Nz/2]         Eq. (1), Eq. (4)
+ *            UNNORMALISED.
+ *   inverse  f(j) = 1/(Nx Ny Nz) Re sum_{k, full grid} Ft(k) exp(+2 pi i [...]),
+ *            Ft = the stored half extended by Ft(kx,ky,kz) = conj F(-kx,-ky,Nz-kz)
+ *            for kz > Nz/2                                      Eq. (2), Eq. (3)
+ *            NORMALISED by 1/(Nx Ny Nz) (the paper's separately timed "normalization",
+ *            P:184; reading R1 in D:3).  Imaginary parts that Eq. (3) makes irrelevant
+ *            (the non-Hermitian part of the planes kz=0 and kz=Nz/2) are ignored exactly as
+ *            that definition ignores them (reading R8).
+ *
+ * Pipeline (P:69-77 steps 1-5; inverse = reverse order), each line ONE kernel pass:
+ *   forward : z-axis R2C  ->  y-axis C2C + global transpose X (steps 2+3+4)  ->  x-axis C2C
+ *   inverse : x-axis C2C  ->  inverse transpose + y-axis C2C  ->  z-axis C2R * 1/(NxNyNz)
+ *
+ * LAYOUTS (all dense, row-major, no padding; complex = interleaved (re, im)):
+ *   real     f[jx][jy][jz]                    z fastest, x slowest
+ *   complex  F[q][kx][ky_l][kz]               q = ky / (Ny/p), ky_l = ky % (Ny/p), kz = 0..Nz/2
+ *            i.e. virtual rank q owns [Nx][Ny/p][Nz/2+1] with x stride (Ny/p)(Nz/2+1)
+ *            and the p ranks are concatenated.  p = 1 is FFTW's natural order.
+ *            fft3d_index() returns the element offset of (kx,ky,kz).
+ *
+ * OWNERSHIP: the caller owns every data buffer and the stream.  A plan owns only its small
+ * device twiddle tables and host metadata; it is immutable after creation and may be used
+ * from several streams concurrently as long as each call has its own workspace.
+ *
+ * DEVICE entry points (fft3d_r2c / fft3d_c2r) take DEVICE pointers, 16-byte aligned, and
+ * return after enqueueing work on `cuda_stream` (a cudaStream_t passed as void*; NULL = the
+ * legacy default stream).  They do not allocate and do not synchronise.  Inputs are
+ * preserved.  in == out, or a workspace overlapping either, is rejected (FFT3D_EINVAL).
+ *
+ * HOST entry points (fft3d_r2c_host / fft3d_c2r_host) take HOST pointers (pinned memory
+ * gives the best copy rate, pageable works), allocate device buffers inside the plan on
+ * first use (released by fft3d_destroy), copy in, transform, copy out and return when the
+ * result is in host memory.
+ *
+ * ERRORS: every function returns an int status (FFT3D_OK = 0) unless stated; none throws,
+ * prints or aborts.  No CPU fallback exists: without a CUDA device every compute call
+ * returns FFT3D_ECUDA.
+ */
+#ifndef FFT3D_H_
+#define FFT3D_H_
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct fft3d_plan_s fft3d_plan_t;      /* opaque */
+
+enum { FFT3D_F32 = 0, FFT3D_F64 = 1 };          /* dtype of reals; complex is two of them */
+
+enum {
+    FFT3D_OK = 0,
+    FFT3D_EINVAL = 1,         /* null pointer, extent < 2, p < 1, p not dividing Nx and Ny,
+                                 bad dtype, aliased / misaligned buffers                      */
+    FFT3D_EUNSUPPORTED = 2,   /* Nz odd, or an extent this build has no kernel for
+                                 (see fft3d_supported_length)                                 */
+    FFT3D_ENOMEM = 3,         /* host or device allocation failed                             */
+    FFT3D_ECUDA = 4,          /* no device, launch or runtime error (cudaGetLastError cleared) */
+    FFT3D_EWORKSPACE = 5      /* reserved: workspace too small cannot be detected from a bare
+                                 pointer; callers size it with fft3d_workspace_bytes          */
+};
+
+/* Create a plan for an Nx x Ny x Nz real grid split into `virtual_slabs` = p x-slabs
+ * (slab decomposition, p <= Nx).  Requirements (reading R6/R7 in D:3): extents >= 2,
+ * Nz even, p >= 1, p | Nx, p | Ny, Nx and Ny in the supported C2C length set and Nz/2 in it
+ * too (the z pass runs an Nz/2-point complex FFT on packed even/odd pairs).
+ * BASELINE.json: fft3d_plan(Nx,Ny,Nz,dtype,virtual_slabs).  *out is NULL on failure. */
+int fft3d_plan(fft3d_plan_t **out, long long Nx, long long Ny, long long Nz,
+               int dtype, int virtual_slabs);
+
+/* 1 if this build has a C2C kernel of length n (n = 2^a or 3*2^a, 2 <= n <= 4096), else 0. */
+int fft3d_supported_length(long long n);
+
+/* Sizes in bytes.  Workspace: the single work buffer shared by R2C and C2R (opt. 1):
+ * Nx*Ny*(Nz/2) complex.  Real: Nx*Ny*Nz reals.  Complex: Nx*Ny*(Nz/2+1) complex. */
+size_t fft3d_workspace_bytes(const fft3d_plan_t *plan);
+size_t fft3d_real_bytes(const fft3d_plan_t *plan);
+size_t fft3d_complex_bytes(const fft3d_plan_t *plan);
+
+/* Element (not byte) offset of F(kx,ky,kz) in the complex array:
+ * ((q*Nx + kx)*(Ny/p) + ky % (Ny/p))*(Nz/2+1) + kz, q = ky / (Ny/p); -1 if out of range.
+ * This is the composition of the paper's steps 2-4 (derivation in D:2). */
+long long fft3d_index(const fft3d_plan_t *plan, long long kx, long long ky, long long kz);
+
+/* Forward R2C, Eq. (1): d_real_in [Nx][Ny][Nz] -> d_cplx_out in the slab layout above.
+ * d_work: fft3d_workspace_bytes() bytes.  d_cplx_out is also used as scratch while the call
+ * runs.  3 full-array kernel passes + one plane-sized fix-up kernel. */
+int fft3d_r2c(const fft3d_plan_t *plan, const void *d_real_in, void *d_cplx_out,
+              void *d_work, void *cuda_stream);
+
+/* Inverse C2R, Eq. (2)+(3) scaled by 1/(NxNyNz): d_cplx_in (slab layout) -> d_real_out
+ * [Nx][Ny][Nz].  d_real_out is also used as scratch while the call runs. */
+int fft3d_c2r(const fft3d_plan_t *plan, const void *d_cplx_in, void *d_real_out,
+              void *d_work, void *cuda_stream);
+
+/* Host-buffer variants: H2D copy, transform, D2H copy, synchronous.  The plan lazily
+ * allocates real + complex + workspace device buffers (fft3d_real_bytes + fft3d_complex_bytes
+ * + fft3d_workspace_bytes) and keeps them until fft3d_destroy. */
+int fft3d_r2c_host(fft3d_plan_t *plan, const void *h_real_in, void *h_cplx_out);
+int fft3d_c2r_host(fft3d_plan_t *plan, const void *h_cplx_in, void *h_real_out);
+
+/* Number of kernels one fft3d_r2c (which = 0) or fft3d_c2r (which = 1) call launches. */
+int fft3d_launches(const fft3d_plan_t *plan, int which);
+
+/* Kernel configuration knob for experiments: variant 0 = default for this build.
+ * Returns FFT3D_EINVAL for an unknown variant; affects later r2c/c2r calls on this plan. */
+int fft3d_set_variant(fft3d_plan_t *plan, int variant);
+
+int fft3d_destroy(fft3d_plan_t *plan);          /* NULL is accepted */
+
+const char *fft3d_strerror(int status);         /* static string, never NULL */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* FFT3D_H_ */
