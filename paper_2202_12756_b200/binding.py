@@ -1,0 +1,195 @@
+"""ctypes binding of include/fft3d.h -- argument marshalling only.
+
+Every step of the transform runs in the kernels of ``libfft3d.so``; PyTorch supplies device
+memory and the stream.  There is no fallback: if the library is missing or no CUDA device
+is present the calls raise.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import torch
+
+F32, F64 = 0, 1
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libfft3d.so")
+
+EXPORTS = (
+    "fft3d_plan", "fft3d_supported_length", "fft3d_workspace_bytes", "fft3d_real_bytes",
+    "fft3d_complex_bytes", "fft3d_index", "fft3d_r2c", "fft3d_c2r", "fft3d_r2c_host",
+    "fft3d_c2r_host", "fft3d_launches", "fft3d_set_variant", "fft3d_destroy", "fft3d_strerror",
+)
+
+_lib = None
+
+
+class Fft3dError(RuntimeError):
+    def __init__(self, status: int, where: str):
+        self.status = status
+        super().__init__("%s: %s (status %d)" % (where, strerror(status), status))
+
+
+def load_library() -> ctypes.CDLL:
+    """Load libfft3d.so (built by ``__graft_entry__.build()`` / ``make -C csrc``)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(
+            "%s is missing: build it with `python -c 'import __graft_entry__ as g; g.build()'` "
+            "(there is no CPU or PyTorch fallback for the FFT path)" % LIB_PATH)
+    lib = ctypes.CDLL(LIB_PATH)
+    vp, ll, i, sz = ctypes.c_void_p, ctypes.c_longlong, ctypes.c_int, ctypes.c_size_t
+    lib.fft3d_plan.argtypes = [ctypes.POINTER(vp), ll, ll, ll, i, i]
+    lib.fft3d_plan.restype = i
+    lib.fft3d_supported_length.argtypes = [ll]
+    lib.fft3d_supported_length.restype = i
+    for nm in ("fft3d_workspace_bytes", "fft3d_real_bytes", "fft3d_complex_bytes"):
+        getattr(lib, nm).argtypes = [vp]
+        getattr(lib, nm).restype = sz
+    lib.fft3d_index.argtypes = [vp, ll, ll, ll]
+    lib.fft3d_index.restype = ll
+    for nm in ("fft3d_r2c", "fft3d_c2r"):
+        getattr(lib, nm).argtypes = [vp, vp, vp, vp, vp]
+        getattr(lib, nm).restype = i
+    for nm in ("fft3d_r2c_host", "fft3d_c2r_host"):
+        getattr(lib, nm).argtypes = [vp, vp, vp]
+        getattr(lib, nm).restype = i
+    lib.fft3d_launches.argtypes = [vp, i]
+    lib.fft3d_launches.restype = i
+    lib.fft3d_set_variant.argtypes = [vp, i]
+    lib.fft3d_set_variant.restype = i
+    lib.fft3d_destroy.argtypes = [vp]
+    lib.fft3d_destroy.restype = i
+    lib.fft3d_strerror.argtypes = [i]
+    lib.fft3d_strerror.restype = ctypes.c_char_p
+    _lib = lib
+    return lib
+
+
+def strerror(status: int) -> str:
+    return load_library().fft3d_strerror(int(status)).decode()
+
+
+def supported_length(n: int) -> bool:
+    return bool(load_library().fft3d_supported_length(int(n)))
+
+
+_REAL = {F32: torch.float32, F64: torch.float64}
+_CPLX = {F32: torch.complex64, F64: torch.complex128}
+
+
+class Plan:
+    """fft3d_plan(Nx, Ny, Nz, dtype, virtual_slabs) with torch tensors as buffers."""
+
+    def __init__(self, Nx: int, Ny: int, Nz: int, dtype=torch.float32, virtual_slabs: int = 1):
+        lib = load_library()
+        self.dtype_code = {torch.float32: F32, torch.float64: F64}[dtype]
+        self.shape = (int(Nx), int(Ny), int(Nz))
+        self.p = int(virtual_slabs)
+        h = ctypes.c_void_p()
+        rc = lib.fft3d_plan(ctypes.byref(h), Nx, Ny, Nz, self.dtype_code, self.p)
+        if rc != 0:
+            raise Fft3dError(rc, "fft3d_plan(%d,%d,%d,p=%d)" % (Nx, Ny, Nz, self.p))
+        self._h = h
+        self._lib = lib
+        self.real_dtype = _REAL[self.dtype_code]
+        self.complex_dtype = _CPLX[self.dtype_code]
+        self.real_bytes = lib.fft3d_real_bytes(h)
+        self.complex_bytes = lib.fft3d_complex_bytes(h)
+        self.workspace_bytes = lib.fft3d_workspace_bytes(h)
+        self.n_complex = Nx * Ny * (Nz // 2 + 1)
+
+    # ---- buffers -------------------------------------------------------------------------
+    def empty_real(self, device="cuda"):
+        return torch.empty(self.shape, dtype=self.real_dtype, device=device)
+
+    def empty_complex(self, device="cuda"):
+        """Flat complex buffer in the slab layout [p][Nx][Ny/p][Nz/2+1]."""
+        return torch.empty(self.n_complex, dtype=self.complex_dtype, device=device)
+
+    def empty_workspace(self, device="cuda"):
+        return torch.empty(self.workspace_bytes, dtype=torch.uint8, device=device)
+
+    def index(self, kx: int, ky: int, kz: int) -> int:
+        return int(self._lib.fft3d_index(self._h, kx, ky, kz))
+
+    def launches(self, which: int) -> int:
+        return int(self._lib.fft3d_launches(self._h, which))
+
+    def set_variant(self, v: int):
+        rc = self._lib.fft3d_set_variant(self._h, int(v))
+        if rc != 0:
+            raise Fft3dError(rc, "fft3d_set_variant")
+
+    # ---- device entry points -------------------------------------------------------------
+    def _check(self, t: torch.Tensor, dtype, nbytes: int, name: str):
+        if not (t.is_cuda and t.is_contiguous() and t.dtype == dtype and t.numel() * t.element_size() == nbytes):
+            raise ValueError("%s must be a contiguous CUDA tensor of dtype %s and %d bytes" % (name, dtype, nbytes))
+
+    def r2c(self, real_in, cplx_out=None, work=None, stream=None):
+        self._check(real_in, self.real_dtype, self.real_bytes, "real_in")
+        if cplx_out is None:
+            cplx_out = self.empty_complex(real_in.device)
+        if work is None:
+            work = self.empty_workspace(real_in.device)
+        self._check(cplx_out, self.complex_dtype, self.complex_bytes, "cplx_out")
+        s = stream if stream is not None else torch.cuda.current_stream(real_in.device)
+        rc = self._lib.fft3d_r2c(self._h, real_in.data_ptr(), cplx_out.data_ptr(), work.data_ptr(),
+                                 ctypes.c_void_p(s.cuda_stream))
+        if rc != 0:
+            raise Fft3dError(rc, "fft3d_r2c")
+        return cplx_out
+
+    def c2r(self, cplx_in, real_out=None, work=None, stream=None):
+        self._check(cplx_in, self.complex_dtype, self.complex_bytes, "cplx_in")
+        if real_out is None:
+            real_out = self.empty_real(cplx_in.device)
+        if work is None:
+            work = self.empty_workspace(cplx_in.device)
+        self._check(real_out, self.real_dtype, self.real_bytes, "real_out")
+        s = stream if stream is not None else torch.cuda.current_stream(cplx_in.device)
+        rc = self._lib.fft3d_c2r(self._h, cplx_in.data_ptr(), real_out.data_ptr(), work.data_ptr(),
+                                 ctypes.c_void_p(s.cuda_stream))
+        if rc != 0:
+            raise Fft3dError(rc, "fft3d_c2r")
+        return real_out
+
+    # ---- host entry points (host tensors, copies inside the call) --------------------------
+    def r2c_host(self, real_in: torch.Tensor, cplx_out: torch.Tensor):
+        assert not real_in.is_cuda and not cplx_out.is_cuda and real_in.is_contiguous() and cplx_out.is_contiguous()
+        rc = self._lib.fft3d_r2c_host(self._h, real_in.data_ptr(), cplx_out.data_ptr())
+        if rc != 0:
+            raise Fft3dError(rc, "fft3d_r2c_host")
+        return cplx_out
+
+    def c2r_host(self, cplx_in: torch.Tensor, real_out: torch.Tensor):
+        assert not cplx_in.is_cuda and not real_out.is_cuda and cplx_in.is_contiguous() and real_out.is_contiguous()
+        rc = self._lib.fft3d_c2r_host(self._h, cplx_in.data_ptr(), real_out.data_ptr())
+        if rc != 0:
+            raise Fft3dError(rc, "fft3d_c2r_host")
+        return real_out
+
+    # ---- layout helpers (index arithmetic only) --------------------------------------------
+    def to_natural(self, cplx_flat: torch.Tensor) -> torch.Tensor:
+        """View a slab-layout spectrum as [Nx][Ny][Nz/2+1] (a permuted copy)."""
+        Nx, Ny, Nz = self.shape
+        L = Ny // self.p
+        return cplx_flat.reshape(self.p, Nx, L, Nz // 2 + 1).permute(1, 0, 2, 3).reshape(Nx, Ny, Nz // 2 + 1)
+
+    def from_natural(self, cplx_nat: torch.Tensor) -> torch.Tensor:
+        Nx, Ny, Nz = self.shape
+        L = Ny // self.p
+        return cplx_nat.reshape(Nx, self.p, L, Nz // 2 + 1).permute(1, 0, 2, 3).contiguous().reshape(-1)
+
+    def close(self):
+        if getattr(self, "_h", None) is not None and self._h:
+            self._lib.fft3d_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

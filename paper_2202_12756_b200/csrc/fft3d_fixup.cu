@@ -1,0 +1,94 @@
+// fft3d_fixup.cu -- the two plane-sized kernels that go with the packed column 0 of the
+// intermediate arrays.
+//
+// After the z-axis R2C, X[0] and X[Nz/2] of every row are real, so the passes keep Nz/2 columns
+// and store (X[0], X[Nz/2]) as one complex number in column 0.  The y and x transforms are
+// linear, so at the end column 0 holds C = A + iB, where A and B are the 2D transforms of two
+// REAL planes and therefore Hermitian: A(k) = (C(k) + conj C(-k))/2, B(k) = (C(k) - conj C(-k))/(2i),
+// k = (kx, ky) mod (Nx, Ny).  unpack_nyquist separates them into the planes kz = 0 and kz = Nz/2
+// of the output (Eq. (3)/(4)).  pack_nyquist is the inverse step; it first takes
+// the Hermitian part of each plane, which is all that Eq. (2)+(3) lets through (reading R8).
+#include <cuda_runtime.h>
+
+#include "fft_radix.cuh"
+
+namespace fft3d {
+
+struct PlaneArgs {
+    const void* src;
+    void* dst;
+    int Nx, Ny, L, M;
+};
+
+__device__ __forceinline__ long long slab_row(int kx, int ky, int Nx, int L) {
+    const int q = ky / L, l = ky - q * L;
+    return ((long long)q * Nx + kx) * L + l;
+}
+
+template <typename T>
+__global__ void unpack_nyquist_kernel(const PlaneArgs a) {
+    using C = cx<T>;
+    const long long n = (long long)a.Nx * a.Ny;
+    const long long pitch = a.M + 1;
+    C* out = reinterpret_cast<C*>(a.dst);
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n;
+         i += (long long)gridDim.x * blockDim.x) {
+        const int kx = (int)(i / a.Ny), ky = (int)(i % a.Ny);
+        const int mx = kx == 0 ? 0 : a.Nx - kx, my = ky == 0 ? 0 : a.Ny - ky;
+        const long long j = (long long)mx * a.Ny + my;
+        if (j < i) continue;                      // the pair is handled by its lower index
+        const long long r1 = slab_row(kx, ky, a.Nx, a.L) * pitch;
+        const long long r2 = slab_row(mx, my, a.Nx, a.L) * pitch;
+        const C c1 = out[r1], c2 = out[r2];
+        const C A = mk<T>((T)0.5 * (c1.x + c2.x), (T)0.5 * (c1.y - c2.y));
+        const C B = mk<T>((T)0.5 * (c1.y + c2.y), (T)-0.5 * (c1.x - c2.x));
+        out[r1] = A;
+        out[r1 + a.M] = B;
+        if (j != i) {
+            out[r2] = cconj(A);
+            out[r2 + a.M] = cconj(B);
+        }
+    }
+}
+
+template <typename T>
+__global__ void pack_nyquist_kernel(const PlaneArgs a) {
+    using C = cx<T>;
+    const long long n = (long long)a.Nx * a.Ny;
+    const long long pitch = a.M + 1;
+    const C* in = reinterpret_cast<const C*>(a.src);
+    C* side = reinterpret_cast<C*>(a.dst);
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n;
+         i += (long long)gridDim.x * blockDim.x) {
+        const int kx = (int)(i / a.Ny), ky = (int)(i % a.Ny);
+        const int mx = kx == 0 ? 0 : a.Nx - kx, my = ky == 0 ? 0 : a.Ny - ky;
+        const long long s1 = slab_row(kx, ky, a.Nx, a.L), s2 = slab_row(mx, my, a.Nx, a.L);
+        const C a1 = in[s1 * pitch], a2 = in[s2 * pitch];
+        const C b1 = in[s1 * pitch + a.M], b2 = in[s2 * pitch + a.M];
+        // Hermitian parts: As = (A(k) + conj A(-k))/2, Bs likewise;  side = As + i Bs
+        const C As = mk<T>((T)0.5 * (a1.x + a2.x), (T)0.5 * (a1.y - a2.y));
+        const C Bs = mk<T>((T)0.5 * (b1.x + b2.x), (T)0.5 * (b1.y - b2.y));
+        side[s1] = mk<T>(As.x - Bs.y, As.y + Bs.x);
+    }
+}
+
+template <typename T>
+static cudaError_t run(void (*k)(const PlaneArgs), const PlaneArgs& a, cudaStream_t st) {
+    const long long n = (long long)a.Nx * a.Ny;
+    long long blocks = (n + 255) / 256;
+    if (blocks > 148 * 16) blocks = 148 * 16;
+    k<<<(unsigned)blocks, 256, 0, st>>>(a);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_unpack_nyquist(int dtype, const PlaneArgs& a, cudaStream_t st) {
+    return dtype == 0 ? run<float>(unpack_nyquist_kernel<float>, a, st)
+                      : run<double>(unpack_nyquist_kernel<double>, a, st);
+}
+
+cudaError_t launch_pack_nyquist(int dtype, const PlaneArgs& a, cudaStream_t st) {
+    return dtype == 0 ? run<float>(pack_nyquist_kernel<float>, a, st)
+                      : run<double>(pack_nyquist_kernel<double>, a, st);
+}
+
+}  // namespace fft3d

@@ -1,0 +1,61 @@
+// fft_inst.cu -- compiled once per FFT length (-DFFT3D_N=<n>): instantiates the z and strided
+// kernels for fp32 and fp64 and exports their description.
+#include "fft_kernels.cuh"
+#include "fft_configs.cuh"
+#include "fft_registry.h"
+
+#ifndef FFT3D_N
+#error "compile with -DFFT3D_N=<length>"
+#endif
+
+namespace fft3d {
+
+template <typename T>
+static KernelSet make_set(int dtype) {
+    using Cfg = typename CfgFor<T, FFT3D_N>::type;
+    using C = cx<T>;
+    constexpr int TC = tile_cols(Cfg::N, (int)sizeof(C));
+    using TP = TilePad<Cfg, TC * (int)sizeof(C)>;
+    constexpr size_t TWB = (size_t)((Cfg::TWN + 1) & ~1) * sizeof(C);
+    constexpr size_t S_SMEM = TWB + (size_t)TP::ROWS * TC * sizeof(C);
+    constexpr int S_THREADS = Cfg::S * TC;
+    constexpr int S_MINB = min_blocks(S_THREADS, Cfg::P, (int)sizeof(T), S_SMEM);
+    constexpr int RPB = rows_per_block(Cfg::S);
+    constexpr size_t Z_SMEM = TWB + (size_t)Cfg::N * sizeof(C) + (size_t)RPB * RowPad<Cfg>::PITCH * sizeof(C);
+    constexpr int Z_THREADS = Cfg::S * RPB;
+    constexpr int Z_MINB = min_blocks(Z_THREADS, Cfg::P, (int)sizeof(T), Z_SMEM);
+
+    KernelSet k{};
+    k.N = Cfg::N;
+    k.dtype = dtype;
+    k.P = Cfg::P;
+    k.nst = Cfg::NST;
+    for (int s = 0; s < 5; ++s) k.radix[s] = s < Cfg::NST ? Cfg::radix(s) : 1;
+    k.twn = Cfg::TWN;
+    k.tc = TC;
+    k.s_threads = S_THREADS;
+    k.s_smem = S_SMEM;
+    k.s_fn[0][KIND_LIN_LIN]  = (const void*)fft_strided_kernel<Cfg, TC, -1, false, false, T, S_MINB>;
+    k.s_fn[0][KIND_LIN_SLAB] = (const void*)fft_strided_kernel<Cfg, TC, -1, false, true, T, S_MINB>;
+    k.s_fn[0][KIND_SLAB_LIN] = nullptr;
+    k.s_fn[1][KIND_LIN_LIN]  = (const void*)fft_strided_kernel<Cfg, TC, +1, false, false, T, S_MINB>;
+    k.s_fn[1][KIND_LIN_SLAB] = nullptr;
+    k.s_fn[1][KIND_SLAB_LIN] = (const void*)fft_strided_kernel<Cfg, TC, +1, true, false, T, S_MINB>;
+    k.z_rpb = RPB;
+    k.z_threads = Z_THREADS;
+    k.z_smem = Z_SMEM;
+    k.z_fn[0] = (const void*)fft_z_r2c_kernel<Cfg, RPB, T, Z_MINB>;
+    k.z_fn[1] = (const void*)fft_z_c2r_kernel<Cfg, RPB, T, Z_MINB>;
+    return k;
+}
+
+#define FFT3D_CAT2(a, b) a##b
+#define FFT3D_CAT(a, b) FFT3D_CAT2(a, b)
+
+const KernelSet* FFT3D_CAT(kernelset_, FFT3D_N)(int dtype) {
+    static const KernelSet f32 = make_set<float>(0);
+    static const KernelSet f64 = make_set<double>(1);
+    return dtype == 0 ? &f32 : &f64;
+}
+
+}  // namespace fft3d

@@ -1,0 +1,160 @@
+// fft_radix.cuh -- register-level building blocks: complex helpers, compile-time twiddles and a
+// fully unrolled in-register DFT of any length R = 2^a * 3^b (R <= 32 used).
+//
+// The transform implemented is the 1D DFT of Eq. (1)/(2) of the paper:
+//   X[k] = sum_j x[j] exp(DIR * 2 pi i j k / R),  DIR = -1 forward, +1 inverse (unnormalised).
+// Everything here is hand-written for sm_100a; no cuFFT, no library code.
+#pragma once
+#include <cuda_runtime.h>
+
+namespace fft3d {
+
+template <typename T> struct cx_sel;
+template <> struct cx_sel<float>  { using type = float2; };
+template <> struct cx_sel<double> { using type = double2; };
+template <typename T> using cx = typename cx_sel<T>::type;
+
+template <typename T> __host__ __device__ __forceinline__ cx<T> mk(T a, T b) { cx<T> r; r.x = a; r.y = b; return r; }
+template <typename C> __device__ __forceinline__ C cadd(C a, C b) { C r; r.x = a.x + b.x; r.y = a.y + b.y; return r; }
+template <typename C> __device__ __forceinline__ C csub(C a, C b) { C r; r.x = a.x - b.x; r.y = a.y - b.y; return r; }
+template <typename C> __device__ __forceinline__ C cmul(C a, C b) {
+    C r; r.x = a.x * b.x - a.y * b.y; r.y = a.x * b.y + a.y * b.x; return r;
+}
+template <typename C> __device__ __forceinline__ C cconj(C a) { C r; r.x = a.x; r.y = -a.y; return r; }
+// multiply by s*i, s = +1 or -1 (compile time)
+template <int S, typename C> __device__ __forceinline__ C cmul_i(C a) {
+    C r;
+    if constexpr (S > 0) { r.x = -a.y; r.y = a.x; } else { r.x = a.y; r.y = -a.x; }
+    return r;
+}
+
+// ---------------------------------------------------------------------------------------------
+// Compile-time cos/sin of 2*pi*num/den, evaluated by the compiler in double:
+// exact octant reduction in integers, then a Taylor series on [0, pi/4].
+// ---------------------------------------------------------------------------------------------
+namespace ct {
+constexpr double PI = 3.14159265358979323846264338327950288;
+
+constexpr double sin_taylor(double x) {
+    double term = x, sum = x, x2 = x * x;
+    for (int n = 1; n < 16; ++n) { term *= -x2 / ((2 * n) * (2 * n + 1)); sum += term; }
+    return sum;
+}
+constexpr double cos_taylor(double x) {
+    double term = 1.0, sum = 1.0, x2 = x * x;
+    for (int n = 1; n < 16; ++n) { term *= -x2 / ((2 * n - 1) * (2 * n)); sum += term; }
+    return sum;
+}
+struct cs { double c, s; };
+// angle = 2*pi*num/den, any integer num, den > 0
+constexpr cs cossin(long long num, long long den) {
+    long long n = num % den;
+    if (n < 0) n += den;
+    // work in units of 1/(8 den) of a turn: a = 8n, full turn = 8 den
+    long long a = 8 * n, full = 8 * den, half = 4 * den, quarter = 2 * den, oct = den;
+    bool neg_s = false, neg_c = false, swap = false;
+    if (a > half) { a = full - a; neg_s = true; }            // cos(2pi-a)=cos a, sin = -sin
+    if (a > quarter) { a = half - a; neg_c = true; }         // cos(pi-a)=-cos a, sin = sin
+    if (a > oct) { a = quarter - a; swap = true; }           // cos(pi/2-a)=sin a
+    double x = 2.0 * PI * (double)a / (double)full;
+    double c = cos_taylor(x), s = sin_taylor(x);
+    if (a == 0) { c = 1.0; s = 0.0; }
+    if (swap) { double t = c; c = s; s = t; }
+    if (neg_c) c = -c;
+    if (neg_s) s = -s;
+    return cs{c, s};
+}
+}  // namespace ct
+
+// a * exp(DIR * 2 pi i NUM / DEN) with the trivial rotations done without multiplications.
+template <int NUM, int DEN, int DIR, typename T>
+__device__ __forceinline__ cx<T> mul_root(cx<T> a) {
+    constexpr int n = ((NUM % DEN) + DEN) % DEN;
+    if constexpr (n == 0) {
+        return a;
+    } else if constexpr (4 * n == DEN) {
+        return cmul_i<DIR>(a);
+    } else if constexpr (2 * n == DEN) {
+        return mk<T>(-a.x, -a.y);
+    } else if constexpr (4 * n == 3 * DEN) {
+        return cmul_i<-DIR>(a);
+    } else {
+        constexpr ct::cs w = ct::cossin(n, DEN);
+        constexpr T c = (T)w.c;
+        constexpr T s = (T)(DIR > 0 ? w.s : -w.s);
+        cx<T> r;
+        r.x = a.x * c - a.y * s;
+        r.y = a.x * s + a.y * c;
+        return r;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// In-register DFT of length R, natural order in and out.  Decimation in time:
+//   R = R1*R2, x[R1*a + q] -> Y_q = DFT_R2, X[k + s*R2] = sum_q W_R1^{qs} (W_R^{qk} Y_q[k]).
+// ---------------------------------------------------------------------------------------------
+template <int R, int DIR, typename T>
+__device__ __forceinline__ void dft(cx<T> (&v)[R]);
+
+// combine step unrolled over k at compile time (the twiddle exponent q*k must be a template arg)
+template <int R, int R1, int R2, int DIR, typename T, int K, int Q>
+__device__ __forceinline__ void combine_tw(cx<T> (&sub)[R1][R2], cx<T> (&t)[R1]) {
+    if constexpr (Q < R1) {
+        t[Q] = mul_root<Q * K, R, DIR, T>(sub[Q][K]);
+        combine_tw<R, R1, R2, DIR, T, K, Q + 1>(sub, t);
+    }
+}
+
+template <int R, int R1, int R2, int DIR, typename T, int K>
+__device__ __forceinline__ void combine(cx<T> (&sub)[R1][R2], cx<T> (&v)[R]) {
+    if constexpr (K < R2) {
+        cx<T> t[R1];
+        combine_tw<R, R1, R2, DIR, T, K, 0>(sub, t);
+        dft<R1, DIR, T>(t);
+#pragma unroll
+        for (int s = 0; s < R1; ++s) v[K + s * R2] = t[s];
+        combine<R, R1, R2, DIR, T, K + 1>(sub, v);
+    }
+}
+
+template <int R, int DIR, typename T>
+__device__ __forceinline__ void dft(cx<T> (&v)[R]) {
+    using C = cx<T>;
+    if constexpr (R == 1) {
+        return;
+    } else if constexpr (R == 2) {
+        C a = v[0], b = v[1];
+        v[0] = cadd(a, b);
+        v[1] = csub(a, b);
+    } else if constexpr (R == 3) {
+        constexpr T h = (T)0.86602540378443864676372317075293618;   // sqrt(3)/2
+        C s = cadd(v[1], v[2]), d = csub(v[1], v[2]);
+        C m = mk<T>(v[0].x - (T)0.5 * s.x, v[0].y - (T)0.5 * s.y);
+        C id = cmul_i<DIR>(d);                                         // DIR * i * d
+        v[0] = cadd(v[0], s);
+        v[1] = mk<T>(m.x + h * id.x, m.y + h * id.y);
+        v[2] = mk<T>(m.x - h * id.x, m.y - h * id.y);
+    } else if constexpr (R == 4) {
+        C t0 = cadd(v[0], v[2]), t1 = csub(v[0], v[2]);
+        C t2 = cadd(v[1], v[3]), d = csub(v[1], v[3]);
+        C id = cmul_i<DIR>(d);
+        v[0] = cadd(t0, t2);
+        v[2] = csub(t0, t2);
+        v[1] = cadd(t1, id);
+        v[3] = csub(t1, id);
+    } else {
+        constexpr int R1 = (R % 4 == 0) ? 4 : ((R % 2 == 0) ? 2 : 3);
+        constexpr int R2 = R / R1;
+        static_assert(R1 * R2 == R, "radix must be 2^a 3^b");
+        C sub[R1][R2];
+#pragma unroll
+        for (int q = 0; q < R1; ++q)
+#pragma unroll
+            for (int a = 0; a < R2; ++a) sub[q][a] = v[R1 * a + q];
+#pragma unroll
+        for (int q = 0; q < R1; ++q) dft<R2, DIR, T>(sub[q]);
+        combine<R, R1, R2, DIR, T, 0>(sub, v);
+    }
+}
+
+}  // namespace fft3d

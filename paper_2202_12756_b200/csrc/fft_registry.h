@@ -1,0 +1,31 @@
+// fft_registry.h -- host-side description of the kernels compiled for one FFT length and dtype.
+#pragma once
+#include <cstddef>
+
+namespace fft3d {
+
+enum { KIND_LIN_LIN = 0, KIND_LIN_SLAB = 1, KIND_SLAB_LIN = 2 };
+
+struct KernelSet {
+    int N;                 // FFT length (for the z kernels: M = Nz/2)
+    int dtype;             // FFT3D_F32 / FFT3D_F64
+    int P;                 // points per thread
+    int nst;               // stages
+    int radix[5];
+    int twn;               // stage-twiddle table entries
+    // strided C2C kernels (N rows x TC columns per tile)
+    int tc;
+    int s_threads;
+    size_t s_smem;
+    const void* s_fn[2][3];    // [0 = forward, 1 = inverse][kind]; null if not compiled
+    // z kernels (rows of N packed complex)
+    int z_rpb;
+    int z_threads;
+    size_t z_smem;
+    const void* z_fn[2];       // [0 = R2C, 1 = C2R]
+};
+
+// nullptr if this build has no kernels for (n, dtype)
+const KernelSet* find_kernels(long long n, int dtype);
+
+}  // namespace fft3d
