@@ -1,0 +1,349 @@
+#!/usr/bin/env python
+"""bench.py -- the headline measurement: one step = one 3D R2C + C2R pair (all hot-path passes)
+on the 1024^3 fp32 grid of BASELINE.json configs[2], inputs resident in HBM.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--n 1024] [--slabs 8]
+
+Prints ONE JSON line (rank 0).  `value` = GFLOP/s by BASELINE.json's convention
+(2.5 N^3 log2 N^3 per real transform, 5 per pair; the paper's convention, is 2x).
+Multi-GPU (torchrun): every rank transforms its own grid (replicas), value is
+the aggregate.  `--impl reference` times the fp64 CPU oracle on a bounded sample (rank 0 only).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import math
+import os
+import statistics
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "GFLOP/s per 3D R2C+C2R pair (5*N^3*log2(N^3) flop per pair), fp32"
+FALLBACK_HBM_GBS = 6650.0        # /opt/skills/guides/B200_PROFILING.md fallback
+
+
+def flops_pair(shape):
+    n = shape[0] * shape[1] * shape[2]
+    return 5.0 * n * math.log2(n)
+
+
+def measured_peak():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as fh:
+            return float(json.load(fh)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+
+
+def stored_traffic(kernel_name):
+    """dram bytes per launch of the dominant kernel from the committed ncu capture, if any."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "traffic.json")) as fh:
+            return json.load(fh).get(kernel_name)
+    except Exception:
+        return None
+
+
+class ClockSampler:
+    QUERY = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+             "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+             "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index):
+        self.tmp = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        self.proc = None
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(gpu_index), "--query-gpu=" + self.QUERY,
+                 "--format=csv,noheader,nounits", "-lms", "100"],
+                stdout=self.tmp, stderr=subprocess.DEVNULL)
+        except Exception:
+            self.proc = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.proc is not None:
+            self.proc.terminate()
+            try:
+                self.proc.wait(timeout=5)
+            except Exception:
+                self.proc.kill()
+        try:
+            self.tmp.flush()
+            self.tmp.seek(0)
+            sm, mx, reasons = [], [], set()
+            names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+            for line in self.tmp.read().splitlines():
+                parts = [p.strip() for p in line.split(",")]
+                if len(parts) < 7:
+                    continue
+                try:
+                    sm.append(float(parts[0]))
+                    mx.append(float(parts[1]))
+                except ValueError:
+                    continue
+                for nm, val in zip(names, parts[3:7]):
+                    if val.lower().startswith("active"):
+                        reasons.add(nm)
+            if sm:
+                out = {"sm_mhz": statistics.median(sm), "sm_max_mhz": max(mx),
+                       "reasons": sorted(reasons), "samples": len(sm)}
+        finally:
+            self.tmp.close()
+            try:
+                os.unlink(self.tmp.name)
+            except OSError:
+                pass
+        return out
+
+
+# ------------------------------------------------------------------------------------------
+# reference arm: the oracle, as it stands, on the host cores
+# ------------------------------------------------------------------------------------------
+def oracle_sample_cube(budget_s, cores):
+    """Largest power-of-two cube whose oracle pair is expected to fit the per-step budget,
+    calibrated by one 64^3 pair (the oracle is O(n log n) per line)."""
+    import numpy as np
+    import oracle
+    f = np.random.Generator(np.random.PCG64(0)).uniform(-1, 1, (64, 64, 64))
+    t0 = time.perf_counter()
+    oracle.c2r(oracle.r2c(f, nthreads=cores), 64, nthreads=cores)
+    t64 = max(time.perf_counter() - t0, 1e-4)
+    best = 64
+    for n in (128, 256, 512):
+        est = t64 * flops_pair((n, n, n)) / flops_pair((64, 64, 64)) * 1.5
+        if est <= budget_s:
+            best = n
+    return best
+
+
+def time_oracle(sample_n, field, steps, warmup, cores):
+    """Oracle R2C + C2R on the [0:sample_n]^3 corner of `field` (fp32 values promoted to fp64)."""
+    import numpy as np
+    import oracle
+    sub = np.ascontiguousarray(field[:sample_n, :sample_n, :sample_n]).astype(np.float64)
+    times = []
+    for it in range(warmup + steps):
+        t0 = time.perf_counter()
+        F = oracle.r2c(sub, nthreads=cores)
+        oracle.c2r(F, sample_n, nthreads=cores)
+        dt = time.perf_counter() - t0
+        if it >= warmup:
+            times.append(dt)
+    t = sum(times) / len(times)
+    return flops_pair((sample_n,) * 3) / t / 1e9, t
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import numpy as np
+    import oracle
+    from paper_2202_12756_b200 import inputs
+    import torch
+    oracle.build_oracle()
+    cores = oracle.max_threads()
+    n = args.n
+    total = max(1, args.steps + args.warmup)
+    sample_n = min(n, oracle_sample_cube(150.0 / total, cores))
+    # the same kind of field as the CUDA arm, generated at the sample size on the host
+    field, _ = inputs.turbulence_grid((sample_n,) * 3, torch.float32, seed=0, device="cpu")
+    gf, t = time_oracle(sample_n, field.numpy(), args.steps, args.warmup, cores)
+    sample = ("oracle R2C+C2R on a %d^3 grid of the same field family (fp64), rate by the same flop formula; "
+              "the full %d^3 pair would take ~%.0f s at this rate" % (sample_n, n, flops_pair((n,) * 3) / (gf * 1e9)))
+    line = {
+        "impl": "reference", "metric": METRIC, "value": gf, "unit": "GFLOP/s",
+        "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": t * 1e3,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic",
+        "config": {"workload": "%d^3 fp32 turbulence-like grid, R2C+C2R pair, virtual_slabs=%d" % (n, args.slabs),
+                   "sample": sample},
+        "cpu_baseline": {"value": gf, "unit": "GFLOP/s", "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": gf, "unit": "GFLOP/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }
+    print(json.dumps(line), flush=True)
+
+
+# ------------------------------------------------------------------------------------------
+# CUDA arm
+# ------------------------------------------------------------------------------------------
+def run_cuda(args):
+    import torch
+    import paper_2202_12756_b200 as pkg
+    from paper_2202_12756_b200 import inputs
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the FFT path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    n, p = args.n, args.slabs
+    shape = (n, n, n)
+    plan = pkg.Plan(*shape, dtype=torch.float32, virtual_slabs=p)
+    field, _modes = inputs.turbulence_grid(shape, torch.float32, seed=rank, device=dev)
+    spec = plan.empty_complex(dev)
+    back = plan.empty_real(dev)
+    work = plan.empty_workspace(dev)
+    stream = torch.cuda.current_stream(dev)
+
+    def step():
+        plan.r2c(field, spec, work, stream)
+        plan.c2r(spec, back, work, stream)
+
+    for _ in range(args.warmup):
+        step()
+    barrier()
+    plan.timing_enable(args.steps)
+    sampler = ClockSampler(local_rank) if rank == 0 else None
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record(stream)
+    for _ in range(args.steps):
+        step()
+    e1.record(stream)
+    barrier()
+    ms_total = e0.elapsed_time(e1)
+    clocks = sampler.stop() if sampler is not None else None
+    t_fwd, c_fwd = plan.timing_read(0)
+    t_inv, c_inv = plan.timing_read(1)
+    plan.timing_enable(0)
+    if dist is not None:
+        t = torch.tensor([ms_total], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_total = float(t.item())
+    ms_step = ms_total / args.steps
+    value = world * flops_pair(shape) / (ms_step * 1e-3) / 1e9
+
+    # sanity: the timed result is a real transform pair (round trip recovers the field)
+    rt_err = (back - field).abs().max().item() / field.abs().max().item()
+    tol = 2e-6 * math.log2(n ** 3)
+
+    # ---- roofline of the dominant kernel (per-launch CUDA events inside the timed loop) ------
+    per_kernel = {}
+    for d, calls in ((t_fwd, c_fwd), (t_inv, c_inv)):
+        for k, v in d.items():
+            per_kernel[k] = v / max(1, calls)
+    real_b, cplx_b, work_b = plan.real_bytes, plan.complex_bytes, plan.workspace_bytes
+    alg_bytes = {                         # algorithmic bytes per launch: one read + one write of the array
+        "z_r2c": real_b + work_b, "y_c2c_fwd": 2 * work_b, "x_c2c_fwd": 2 * work_b,
+        "x_c2c_inv": 2 * work_b, "y_c2c_inv": 2 * work_b, "z_c2r": work_b + real_b,
+    }
+    big = {k: per_kernel[k] for k in alg_bytes}
+    dom = max(big, key=big.get)
+    peak, peak_src = measured_peak()
+    achieved = alg_bytes[dom] / (big[dom] * 1e-3) / 1e9
+    roofline = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
+                "frac": achieved / peak, "traffic": stored_traffic(dom), "peak_source": peak_src,
+                "algorithmic_bytes": alg_bytes[dom], "ms_per_launch": big[dom],
+                "all_kernels_ms": per_kernel,
+                "all_kernels_gbs": {k: alg_bytes[k] / (per_kernel[k] * 1e-3) / 1e9 for k in alg_bytes},
+                "pair_bytes_6pass": sum(alg_bytes.values()),
+                "pair_frac_of_6pass_roofline": (sum(alg_bytes.values()) / peak / 1e9) / (ms_step * 1e-3)}
+
+    # ---- end to end through the host entry points (pinned host buffers, copies timed) ---------
+    e2e = None
+    if not args.no_e2e:
+        h_in = torch.empty(shape, dtype=torch.float32).pin_memory()
+        h_spec = torch.empty(plan.n_complex, dtype=torch.complex64).pin_memory()
+        h_back = torch.empty(shape, dtype=torch.float32).pin_memory()
+        h_in.copy_(field)
+        # free the device-resident bench buffers first: the host entry points own their own
+        del spec, back, work
+        torch.cuda.empty_cache()
+        plan.r2c_host(h_in, h_spec)                     # warm-up (allocates the plan's buffers)
+        plan.c2r_host(h_spec, h_back)
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(args.e2e_steps):
+            plan.r2c_host(h_in, h_spec)
+            plan.c2r_host(h_spec, h_back)
+        torch.cuda.synchronize()
+        dt = (time.perf_counter() - t0) / args.e2e_steps
+        if dist is not None:
+            t = torch.tensor([dt], dtype=torch.float64, device=dev)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            dt = float(t.item())
+        e2e_rt = (h_back - h_in).abs().max().item() / h_in.abs().max().item()
+        e2e = {"value": world * flops_pair(shape) / dt / 1e9, "unit": "GFLOP/s", "ms_per_step": dt * 1e3,
+               "h2d_bytes_per_step": real_b + cplx_b, "d2h_bytes_per_step": cplx_b + real_b,
+               "round_trip_rel_err": e2e_rt}
+
+    # ---- the oracle timed beside it (rank 0, N=1 only) -----------------------------------------
+    cpu_baseline = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        import oracle
+        oracle.build_oracle()
+        cores = oracle.max_threads()
+        sample_n = min(n, 256 if cores < 12 else 512)
+        sub = field[:sample_n, :sample_n, :sample_n].contiguous().cpu().numpy()
+        gf, t = time_oracle(sample_n, sub, 1, 0, cores)
+        cpu_baseline = {"value": gf, "unit": "GFLOP/s", "cores": cores, "kind": "oracle",
+                        "sample": "oracle R2C+C2R (fp64) on the [0:%d]^3 corner of the %d^3 field, %.1f s; "
+                                  "rate by the same flop formula" % (sample_n, n, t)}
+
+    if rank == 0:
+        line = {
+            "metric": METRIC, "value": value, "unit": "GFLOP/s", "n_gpus": world,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_step,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+            "data": "synthetic",
+            "config": {"workload": "%d^3 fp32 turbulence-like grid (BASELINE.json configs[2]), R2C+C2R pair, "
+                                   "virtual_slabs=%d" % (n, p),
+                       "l2": "inputs (%.1f GiB per array) are far larger than the 126 MB L2; no flush needed"
+                             % (real_b / 2 ** 30),
+                       "parallelism": "replicas x%d" % world,
+                       "gflops_paper_convention": 2 * value,
+                       "round_trip_rel_err": rt_err, "round_trip_bound": tol},
+            "clocks": clocks, "e2e": e2e,
+            "gpu_launches": args.steps * (plan.launches(0) + plan.launches(1)),
+            "roofline": roofline, "cpu_baseline": cpu_baseline,
+        }
+        print(json.dumps(line), flush=True)
+        if not (rt_err <= tol):
+            raise SystemExit("round trip error %.3e exceeds %.3e: the timed path is wrong" % (rt_err, tol))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
+    ap.add_argument("--n", type=int, default=1024)
+    ap.add_argument("--slabs", type=int, default=8)
+    ap.add_argument("--e2e-steps", type=int, default=2)
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "cuda" else args.warmup
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_cuda(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -113,6 +113,18 @@ int fft3d_c2r_host(fft3d_plan_t *plan, const void *h_cplx_in, void *h_real_out);
 /* Number of kernels one fft3d_r2c (which = 0) or fft3d_c2r (which = 1) call launches. */
 int fft3d_launches(const fft3d_plan_t *plan, int which);
 
+/* Per-kernel timing for roofline reports.  After fft3d_timing_enable(plan, max_calls) every
+ * fft3d_r2c / fft3d_c2r call on this plan records CUDA events between its kernel launches on the
+ * caller's stream (until max_calls calls per direction have been recorded; later calls run
+ * untimed).  fft3d_timing_read waits for the recorded events and returns, for direction
+ * `which` (0 = r2c, 1 = c2r), the summed duration in ms of each launch slot over the recorded
+ * calls (ms_sum[i], i < fft3d_launches(plan, which), in launch order: r2c = z-R2C, y-C2C,
+ * x-C2C, Nyquist unpack; c2r = Nyquist pack, x-C2C, y-C2C, z-C2R) and the number of calls,
+ * then resets the counters.  max_calls = 0 disables timing.  Not thread-safe while enabled. */
+#define FFT3D_MAX_LAUNCHES 8
+int fft3d_timing_enable(fft3d_plan_t *plan, int max_calls);
+int fft3d_timing_read(fft3d_plan_t *plan, int which, float *ms_sum, int *calls);
+
 /* Kernel configuration knob for experiments: variant 0 = default for this build.
  * Returns FFT3D_EINVAL for an unknown variant; affects later r2c/c2r calls on this plan. */
 int fft3d_set_variant(fft3d_plan_t *plan, int variant);

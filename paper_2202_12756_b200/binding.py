@@ -19,6 +19,7 @@ EXPORTS = (
     "fft3d_plan", "fft3d_supported_length", "fft3d_workspace_bytes", "fft3d_real_bytes",
     "fft3d_complex_bytes", "fft3d_index", "fft3d_r2c", "fft3d_c2r", "fft3d_r2c_host",
     "fft3d_c2r_host", "fft3d_launches", "fft3d_set_variant", "fft3d_destroy", "fft3d_strerror",
+    "fft3d_timing_enable", "fft3d_timing_read",
 )
 
 _lib = None
@@ -60,6 +61,10 @@ def load_library() -> ctypes.CDLL:
     lib.fft3d_launches.restype = i
     lib.fft3d_set_variant.argtypes = [vp, i]
     lib.fft3d_set_variant.restype = i
+    lib.fft3d_timing_enable.argtypes = [vp, i]
+    lib.fft3d_timing_enable.restype = i
+    lib.fft3d_timing_read.argtypes = [vp, i, ctypes.POINTER(ctypes.c_float), ctypes.POINTER(i)]
+    lib.fft3d_timing_read.restype = i
     lib.fft3d_destroy.argtypes = [vp]
     lib.fft3d_destroy.restype = i
     lib.fft3d_strerror.argtypes = [i]
@@ -122,6 +127,24 @@ class Plan:
         rc = self._lib.fft3d_set_variant(self._h, int(v))
         if rc != 0:
             raise Fft3dError(rc, "fft3d_set_variant")
+
+    LAUNCH_NAMES = (("z_r2c", "y_c2c_fwd", "x_c2c_fwd", "nyquist_unpack"),
+                    ("nyquist_pack", "x_c2c_inv", "y_c2c_inv", "z_c2r"))
+
+    def timing_enable(self, max_calls: int):
+        rc = self._lib.fft3d_timing_enable(self._h, int(max_calls))
+        if rc != 0:
+            raise Fft3dError(rc, "fft3d_timing_enable")
+
+    def timing_read(self, which: int):
+        """-> (dict launch name -> summed ms, calls) for direction which (0 r2c, 1 c2r)."""
+        ms = (ctypes.c_float * 8)()
+        calls = ctypes.c_int(0)
+        rc = self._lib.fft3d_timing_read(self._h, int(which), ms, ctypes.byref(calls))
+        if rc != 0:
+            raise Fft3dError(rc, "fft3d_timing_read")
+        names = self.LAUNCH_NAMES[which]
+        return {names[k]: float(ms[k]) for k in range(self.launches(which))}, calls.value
 
     # ---- device entry points -------------------------------------------------------------
     def _check(self, t: torch.Tensor, dtype, nbytes: int, name: str):

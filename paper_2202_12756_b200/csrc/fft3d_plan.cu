@@ -49,6 +49,12 @@ cudaError_t launch_pack_nyquist(int dtype, const PlaneArgs& a, cudaStream_t st);
 
 using namespace fft3d;
 
+struct TimingState {
+    int max_calls;
+    int calls[2];
+    std::vector<cudaEvent_t> ev[2];      // (FFT3D_MAX_LAUNCHES + 1) events per recorded call
+};
+
 struct fft3d_plan_s {
     long long Nx, Ny, Nz, M, L;
     int p, dtype, esize;       // esize = bytes per real
@@ -60,6 +66,7 @@ struct fft3d_plan_s {
     // buffers of the host-pointer entry points (lazy)
     void *h_real, *h_cplx, *h_work;
     cudaStream_t h_stream;
+    TimingState* timing;       // null unless fft3d_timing_enable was called
 };
 
 namespace {
@@ -155,6 +162,19 @@ int launch(const void* fn, long long work_items, int grid_cap, int threads, size
     return FFT3D_OK;
 }
 
+// event slot `i` of the call being recorded for direction `which`, or no-op
+struct Recorder {
+    TimingState* t;
+    int which, call;
+    cudaStream_t st;
+    Recorder(const fft3d_plan_s* pl, int w, cudaStream_t s) : t(pl->timing), which(w), call(-1), st(s) {
+        if (t != nullptr && t->calls[w] < t->max_calls) call = t->calls[w]++;
+    }
+    void mark(int i) {
+        if (call >= 0) cudaEventRecord(t->ev[which][(size_t)call * (FFT3D_MAX_LAUNCHES + 1) + i], st);
+    }
+};
+
 bool overlap(const void* a, size_t na, const void* b, size_t nb) {
     uintptr_t x = (uintptr_t)a, y = (uintptr_t)b;
     return x < y + nb && y < x + na;
@@ -244,6 +264,8 @@ int fft3d_r2c(const fft3d_plan_t* pl, const void* d_in, void* d_out, void* d_wor
     cudaStream_t st = (cudaStream_t)stream;
     const long long Nx = pl->Nx, Ny = pl->Ny, M = pl->M, L = pl->L, p = pl->p;
 
+    Recorder rec(pl, 0, st);
+    rec.mark(0);
     // F1: real [Nx*Ny rows][Nz] -> packed complex [Nx][Ny][M] in d_out (scratch use)
     ZArgs z{};
     z.in = d_in; z.out = d_out; z.tw = pl->tw_z; z.twz = pl->twz; z.nrows = Nx * Ny; z.scale = 1.0;
@@ -251,6 +273,7 @@ int fft3d_r2c(const fft3d_plan_t* pl, const void* d_in, void* d_out, void* d_wor
     int rc = launch(kz->z_fn[0], (z.nrows + kz->z_rpb - 1) / kz->z_rpb, pl->grid_z[0], kz->z_threads,
                     kz->z_smem, &z, st);
     if (rc != FFT3D_OK) return rc;
+    rec.mark(1);
 
     // F2: y-axis FFT of d_out [x][y][M]; row ky goes to work[q][x][ky_l][M]  (steps 2-4 folded in)
     const KernelSet* ky = pl->ky;
@@ -262,6 +285,7 @@ int fft3d_r2c(const fft3d_plan_t* pl, const void* d_in, void* d_out, void* d_wor
     a.out_hi = L * M; a.out_lo = 0; a.out_rq = Nx * L * M; a.out_rl = M;
     rc = launch(ky->s_fn[0][KIND_LIN_SLAB], a.ntiles, pl->grid_y[0], ky->s_threads, ky->s_smem, &a, st);
     if (rc != FFT3D_OK) return rc;
+    rec.mark(2);
 
     // F3: x-axis FFT per virtual slab q and row ky_l: work (pitch M) -> d_out (pitch M+1)
     const KernelSet* kx = pl->kx;
@@ -273,11 +297,13 @@ int fft3d_r2c(const fft3d_plan_t* pl, const void* d_in, void* d_out, void* d_wor
     b.out_hi = Nx * L * (M + 1); b.out_lo = M + 1; b.out_rq = 0; b.out_rl = L * (M + 1);
     rc = launch(kx->s_fn[0][KIND_LIN_LIN], b.ntiles, pl->grid_x[0], kx->s_threads, kx->s_smem, &b, st);
     if (rc != FFT3D_OK) return rc;
+    rec.mark(3);
 
     // column 0 holds A + iB (planes kz = 0 and kz = Nz/2): separate them in place
     PlaneArgs f{};
     f.src = nullptr; f.dst = d_out; f.Nx = (int)Nx; f.Ny = (int)Ny; f.L = (int)L; f.M = (int)M;
     if (launch_unpack_nyquist(pl->dtype, f, st) != cudaSuccess) { cudaGetLastError(); return FFT3D_ECUDA; }
+    rec.mark(4);
     return FFT3D_OK;
 }
 
@@ -293,9 +319,12 @@ int fft3d_c2r(const fft3d_plan_t* pl, const void* d_in, void* d_out, void* d_wor
     // pre-pack: side[q][kx][ky_l] = sym(plane kz=0) + i sym(plane kz=Nz/2), kept at the start of
     // the workspace until I1 has consumed it (reading R8: only the Hermitian part of the two
     // self-conjugate planes enters Eq. (2)+(3)).
+    Recorder rec(pl, 1, st);
+    rec.mark(0);
     PlaneArgs f{};
     f.src = d_in; f.dst = d_work; f.Nx = (int)Nx; f.Ny = (int)Ny; f.L = (int)L; f.M = (int)M;
     if (launch_pack_nyquist(pl->dtype, f, st) != cudaSuccess) { cudaGetLastError(); return FFT3D_ECUDA; }
+    rec.mark(1);
 
     // I1: x-axis inverse FFT: d_in (pitch M+1, column 0 from the side buffer) -> d_out scratch (pitch M)
     const KernelSet* kx = pl->kx;
@@ -308,6 +337,7 @@ int fft3d_c2r(const fft3d_plan_t* pl, const void* d_in, void* d_out, void* d_wor
     b.out_hi = Nx * L * M; b.out_lo = M; b.out_rq = 0; b.out_rl = L * M;
     int rc = launch(kx->s_fn[1][KIND_LIN_LIN], b.ntiles, pl->grid_x[1], kx->s_threads, kx->s_smem, &b, st);
     if (rc != FFT3D_OK) return rc;
+    rec.mark(2);
 
     // I2: y-axis inverse FFT gathering rows from the slab layout: d_out scratch -> work [x][y][M]
     const KernelSet* ky = pl->ky;
@@ -319,14 +349,62 @@ int fft3d_c2r(const fft3d_plan_t* pl, const void* d_in, void* d_out, void* d_wor
     a.out_hi = Ny * M; a.out_lo = 0; a.out_rq = 0; a.out_rl = M;
     rc = launch(ky->s_fn[1][KIND_SLAB_LIN], a.ntiles, pl->grid_y[1], ky->s_threads, ky->s_smem, &a, st);
     if (rc != FFT3D_OK) return rc;
+    rec.mark(3);
 
     // I3: z-axis C2R with the 1/(NxNyNz) normalisation: work -> d_out
     const KernelSet* kz = pl->kz;
     ZArgs z{};
     z.in = d_work; z.out = d_out; z.tw = pl->tw_z; z.twz = pl->twz; z.nrows = Nx * Ny;
     z.scale = 1.0 / ((double)Nx * (double)Ny * (double)Nz);
-    return launch(kz->z_fn[1], (z.nrows + kz->z_rpb - 1) / kz->z_rpb, pl->grid_z[1], kz->z_threads,
-                  kz->z_smem, &z, st);
+    rc = launch(kz->z_fn[1], (z.nrows + kz->z_rpb - 1) / kz->z_rpb, pl->grid_z[1], kz->z_threads,
+                kz->z_smem, &z, st);
+    rec.mark(4);
+    return rc;
+}
+
+static void timing_free(fft3d_plan_t* pl) {
+    if (pl->timing == nullptr) return;
+    for (int w = 0; w < 2; ++w)
+        for (cudaEvent_t e : pl->timing->ev[w]) cudaEventDestroy(e);
+    delete pl->timing;
+    pl->timing = nullptr;
+}
+
+int fft3d_timing_enable(fft3d_plan_t* pl, int max_calls) {
+    if (pl == nullptr || max_calls < 0 || max_calls > 4096) return FFT3D_EINVAL;
+    timing_free(pl);
+    if (max_calls == 0) return FFT3D_OK;
+    TimingState* t = new (std::nothrow) TimingState();
+    if (t == nullptr) return FFT3D_ENOMEM;
+    t->max_calls = max_calls;
+    t->calls[0] = t->calls[1] = 0;
+    for (int w = 0; w < 2; ++w) {
+        t->ev[w].resize((size_t)max_calls * (FFT3D_MAX_LAUNCHES + 1));
+        for (auto& e : t->ev[w])
+            if (cudaEventCreate(&e) != cudaSuccess) { cudaGetLastError(); pl->timing = t; timing_free(pl); return FFT3D_ECUDA; }
+    }
+    pl->timing = t;
+    return FFT3D_OK;
+}
+
+int fft3d_timing_read(fft3d_plan_t* pl, int which, float* ms_sum, int* calls) {
+    if (pl == nullptr || pl->timing == nullptr || which < 0 || which > 1 || ms_sum == nullptr || calls == nullptr)
+        return FFT3D_EINVAL;
+    TimingState* t = pl->timing;
+    const int nl = fft3d_launches(pl, which);
+    for (int i = 0; i < FFT3D_MAX_LAUNCHES; ++i) ms_sum[i] = 0.f;
+    for (int c = 0; c < t->calls[which]; ++c) {
+        cudaEvent_t* e = &t->ev[which][(size_t)c * (FFT3D_MAX_LAUNCHES + 1)];
+        if (cudaEventSynchronize(e[nl]) != cudaSuccess) { cudaGetLastError(); return FFT3D_ECUDA; }
+        for (int i = 0; i < nl; ++i) {
+            float ms = 0.f;
+            if (cudaEventElapsedTime(&ms, e[i], e[i + 1]) != cudaSuccess) { cudaGetLastError(); return FFT3D_ECUDA; }
+            ms_sum[i] += ms;
+        }
+    }
+    *calls = t->calls[which];
+    t->calls[which] = 0;
+    return FFT3D_OK;
 }
 
 static int ensure_host_buffers(fft3d_plan_t* pl) {
@@ -389,6 +467,7 @@ int fft3d_destroy(fft3d_plan_t* pl) {
     cudaFree(pl->tw_z); cudaFree(pl->tw_y); cudaFree(pl->tw_x); cudaFree(pl->twz);
     cudaFree(pl->h_real); cudaFree(pl->h_cplx); cudaFree(pl->h_work);
     if (pl->h_stream) cudaStreamDestroy(pl->h_stream);
+    timing_free(pl);
     cudaGetLastError();
     delete pl;
     return FFT3D_OK;
