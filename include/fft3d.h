@@ -119,14 +119,17 @@ int fft3d_launches(const fft3d_plan_t *plan, int which);
  * untimed).  fft3d_timing_read waits for the recorded events and returns, for direction
  * `which` (0 = r2c, 1 = c2r), the summed duration in ms of each launch slot over the recorded
  * calls (ms_sum[i], i < fft3d_launches(plan, which), in launch order: r2c = z-R2C, y-C2C,
- * x-C2C, Nyquist unpack; c2r = Nyquist pack, x-C2C, y-C2C, z-C2R) and the number of calls,
+ * x-C2C, Nyquist unpack; c2r = Nyquist pack, x-C2C, [x-C2C of the packed column 0, only when
+ * fft3d_launches(plan, 1) == 5], y-C2C, z-C2R) and the number of calls,
  * then resets the counters.  max_calls = 0 disables timing.  Not thread-safe while enabled. */
 #define FFT3D_MAX_LAUNCHES 8
 int fft3d_timing_enable(fft3d_plan_t *plan, int max_calls);
 int fft3d_timing_read(fft3d_plan_t *plan, int which, float *ms_sum, int *calls);
 
-/* Kernel configuration knob for experiments: variant 0 = default for this build.
- * Returns FFT3D_EINVAL for an unknown variant; affects later r2c/c2r calls on this plan. */
+/* Kernel selection for the strided (y, x) passes: variant 0 (default) = TMA-pipelined
+ * persistent kernels wherever the extents and alignment allow, plain-load kernels elsewhere;
+ * variant 1 = plain-load kernels everywhere (ablation / cross-check: both give bit-identical
+ * results).  Returns FFT3D_EINVAL for an unknown variant; affects later calls on this plan. */
 int fft3d_set_variant(fft3d_plan_t *plan, int variant);
 
 int fft3d_destroy(fft3d_plan_t *plan);          /* NULL is accepted */

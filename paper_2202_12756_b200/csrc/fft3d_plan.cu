@@ -7,6 +7,7 @@
 //   F3  x-axis C2C with stride (Ny/p)(Nz/2+1)          step 5
 //   inverse: the same in reverse order with 1/(NxNyNz) fused into the last pass.
 // One workspace serves both directions (optimisation 1).
+#include <cuda.h>
 #include <cuda_runtime.h>
 
 #include <cmath>
@@ -67,6 +68,10 @@ struct fft3d_plan_s {
     void *h_real, *h_cplx, *h_work;
     cudaStream_t h_stream;
     TimingState* timing;       // null unless fft3d_timing_enable was called
+    // TMA-pipelined strided passes
+    void* encode_fn;           // cuTensorMapEncodeTiled, resolved at run time (no libcuda link dependency)
+    bool tma_y, tma_x;         // usable for this plan's extents / alignment
+    int y_rows_nat, y_rows_slab, x_rows;   // rows per TMA box
 };
 
 namespace {
@@ -162,6 +167,66 @@ int launch(const void* fn, long long work_items, int grid_cap, int threads, size
     return FFT3D_OK;
 }
 
+long long largest_divisor_le(long long n, long long cap) {
+    for (long long d = cap < n ? cap : n; d >= 1; --d)
+        if (n % d == 0) return d;
+    return 1;
+}
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+// Tensor map over 8-byte words: dims[0] is the contiguous dimension, strides in bytes for dims 1..rank-1.
+bool make_map(const fft3d_plan_s* pl, TensorMapBlob* out, const void* base, int rank, const long long* dims,
+              const long long* strides_bytes, const int* box) {
+    static_assert(sizeof(CUtensorMap) == sizeof(TensorMapBlob), "CUtensorMap is 128 bytes");
+    cuuint64_t gd[5]; cuuint64_t gs[5]; cuuint32_t bx[5]; cuuint32_t es[5];
+    for (int i = 0; i < rank; ++i) { gd[i] = (cuuint64_t)dims[i]; bx[i] = (cuuint32_t)box[i]; es[i] = 1; }
+    for (int i = 0; i + 1 < rank; ++i) gs[i] = (cuuint64_t)strides_bytes[i];
+    CUresult r = ((EncodeTiledFn)pl->encode_fn)(reinterpret_cast<CUtensorMap*>(out), CU_TENSOR_MAP_DATA_TYPE_UINT64,
+                                                (cuuint32_t)rank, const_cast<void*>(base), gd, gs, bx, es,
+                                                CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                                                CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    return r == CUDA_SUCCESS;
+}
+
+// The four array views of the strided passes (sz = bytes per complex, W = sz/8 words).
+bool map_natural(const fft3d_plan_s* pl, TensorMapBlob* m, const void* base, int tc, int rows) {   // [Nx][Ny][M]
+    const long long sz = 2 * pl->esize, W = sz / 8;
+    long long d[3] = {pl->M * W, pl->Ny, pl->Nx}, st[2] = {pl->M * sz, pl->Ny * pl->M * sz};
+    int b[3] = {(int)(tc * W), rows, 1};
+    return make_map(pl, m, base, 3, d, st, b);
+}
+bool map_slab_y(const fft3d_plan_s* pl, TensorMapBlob* m, const void* base, int tc, int rows) {    // [p][Nx][L][M], rows along (q,l)
+    const long long sz = 2 * pl->esize, W = sz / 8, L = pl->L;
+    long long d[4] = {pl->M * W, L, pl->Nx, pl->p}, st[3] = {pl->M * sz, L * pl->M * sz, pl->Nx * L * pl->M * sz};
+    int b[4] = {(int)(tc * W), (int)(rows < L ? rows : L), 1, (int)(rows < L ? 1 : rows / L)};
+    return make_map(pl, m, base, 4, d, st, b);
+}
+bool map_slab_x(const fft3d_plan_s* pl, TensorMapBlob* m, const void* base, int tc, int rows) {    // [p][Nx][L][M], rows along x; tc = box columns
+    const long long sz = 2 * pl->esize, W = sz / 8, L = pl->L;
+    long long d[4] = {pl->M * W, L, pl->Nx, pl->p}, st[3] = {pl->M * sz, L * pl->M * sz, pl->Nx * L * pl->M * sz};
+    int b[4] = {(int)(tc * W), 1, rows, 1};
+    return make_map(pl, m, base, 4, d, st, b);
+}
+bool map_user_x(const fft3d_plan_s* pl, TensorMapBlob* m, const void* base, int tc, int rows) {    // [p][Nx][L*(M+1)], rows along x
+    const long long sz = 2 * pl->esize, W = sz / 8, L = pl->L, Mp1 = pl->M + 1;
+    long long d[3] = {L * Mp1 * W, pl->Nx, pl->p}, st[2] = {L * Mp1 * sz, pl->Nx * L * Mp1 * sz};
+    int b[3] = {(int)(tc * W), rows, 1};
+    return make_map(pl, m, base, 3, d, st, b);
+}
+
+int launch_tma(const void* fn, const KernelSet* k, size_t smem, int num_sms, const TensorMapBlob& in_map,
+               const TensorMapBlob& in_map2, const TensorMapBlob& out_map, TmaArgs& a, cudaStream_t st) {
+    long long g = a.ntiles < num_sms ? a.ntiles : num_sms;
+    if (g <= 0) return FFT3D_OK;
+    void* argv[4] = {(void*)&in_map, (void*)&in_map2, (void*)&out_map, (void*)&a};
+    cudaError_t e = cudaLaunchKernel(fn, dim3((unsigned)g), dim3((unsigned)k->tma_threads), argv, smem, st);
+    if (e != cudaSuccess) { cudaGetLastError(); return FFT3D_ECUDA; }
+    return FFT3D_OK;
+}
+
 // event slot `i` of the call being recorded for direction `which`, or no-op
 struct Recorder {
     TimingState* t;
@@ -223,6 +288,37 @@ int fft3d_plan(fft3d_plan_t** out, long long Nx, long long Ny, long long Nz, int
         if (rc == FFT3D_OK) rc = prepare_kernel(ky->s_fn[d][ykind], ky->s_threads, ky->s_smem, sms, &pl->grid_y[d]);
         if (rc == FFT3D_OK) rc = prepare_kernel(kx->s_fn[d][KIND_LIN_LIN], kx->s_threads, kx->s_smem, sms, &pl->grid_x[d]);
     }
+    // TMA path: needs the driver's tensor-map encoder, 16-byte strides and whole tiles
+    if (rc == FFT3D_OK) {
+        cudaDriverEntryPointQueryResult qres;
+        void* fn = nullptr;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess ||
+            qres != cudaDriverEntryPointSuccess) { cudaGetLastError(); fn = nullptr; }
+        pl->encode_fn = fn;
+        const long long sz = 2 * pl->esize, M = pl->M, L = pl->L;
+        const bool strides_ok = (M * sz) % 16 == 0;
+        pl->tma_y = pl->tma_x = false;
+        if (fn != nullptr && strides_ok && ky->tma_fn[0] != nullptr && M % ky->tma_tc == 0) {
+            pl->y_rows_nat = (int)largest_divisor_le(Ny, 256);
+            // slab side: a box covers whole slabs (rows % L == 0) or part of one (L % rows == 0)
+            long long rows = L <= 256 ? L * largest_divisor_le(pl->p, 256 / L) : largest_divisor_le(L, 256);
+            pl->y_rows_slab = (int)rows;
+            pl->tma_y = true;
+            for (int d = 0; d < 2 && rc == FFT3D_OK; ++d) {
+                int g = 0;
+                rc = prepare_kernel(ky->tma_fn[d == 0 ? TMA_Y_FWD : TMA_Y_INV], ky->tma_threads, ky->tma_smem_y, sms, &g);
+            }
+        }
+        if (rc == FFT3D_OK && fn != nullptr && strides_ok && kx->tma_fn[TMA_X_FWD] != nullptr && M % kx->tma_tc == 0 &&
+            (L * (M + 1) * sz) % 16 == 0 && (!kx->tma_oddfix || L % 2 == 0)) {
+            pl->x_rows = (int)largest_divisor_le(Nx, 256);
+            pl->tma_x = true;
+            for (int d = 0; d < 2 && rc == FFT3D_OK; ++d) {
+                int g = 0;
+                rc = prepare_kernel(kx->tma_fn[d == 0 ? TMA_X_FWD : TMA_X_INV], kx->tma_threads, kx->tma_smem_x, sms, &g);
+            }
+        }
+    }
     if (rc != FFT3D_OK) { fft3d_destroy(pl); return rc; }
     *out = pl;
     return FFT3D_OK;
@@ -245,12 +341,13 @@ long long fft3d_index(const fft3d_plan_t* pl, long long kx, long long ky, long l
 }
 
 int fft3d_launches(const fft3d_plan_t* pl, int which) {
-    (void)which;
-    return pl ? 4 : 0;
+    if (pl == nullptr) return 0;
+    // c2r on the TMA path runs the packed column 0 of the x pass as a separate small kernel
+    return (which == 1 && pl->variant == 0 && pl->tma_x) ? 5 : 4;
 }
 
 int fft3d_set_variant(fft3d_plan_t* pl, int variant) {
-    if (pl == nullptr || variant != 0) return FFT3D_EINVAL;
+    if (pl == nullptr || variant < 0 || variant > 1) return FFT3D_EINVAL;   // 0 = TMA-pipelined where possible, 1 = plain-load kernels only
     pl->variant = variant;
     return FFT3D_OK;
 }
@@ -283,7 +380,18 @@ int fft3d_r2c(const fft3d_plan_t* pl, const void* d_in, void* d_out, void* d_wor
     a.ntiles = Nx * a.ntz;
     a.in_hi = Ny * M; a.in_lo = 0; a.in_rq = 0; a.in_rl = M;
     a.out_hi = L * M; a.out_lo = 0; a.out_rq = Nx * L * M; a.out_rl = M;
-    rc = launch(ky->s_fn[0][KIND_LIN_SLAB], a.ntiles, pl->grid_y[0], ky->s_threads, ky->s_smem, &a, st);
+    const bool use_tma = pl->variant == 0;
+    if (use_tma && pl->tma_y) {
+        TensorMapBlob mi, mo;
+        if (!map_natural(pl, &mi, d_out, ky->tma_tc, pl->y_rows_nat) ||
+            !map_slab_y(pl, &mo, d_work, ky->tma_tc, pl->y_rows_slab)) return FFT3D_ECUDA;
+        TmaArgs ta{};
+        ta.tw = pl->tw_y; ta.ntz = (int)(M / ky->tma_tc); ta.ntiles = Nx * ta.ntz;
+        ta.L = (int)L; ta.Nx = (int)Nx; ta.Mp1 = (int)(M + 1); ta.in_rows = pl->y_rows_nat; ta.out_rows = pl->y_rows_slab;
+        rc = launch_tma(ky->tma_fn[TMA_Y_FWD], ky, ky->tma_smem_y, pl->num_sms, mi, mi, mo, ta, st);
+    } else {
+        rc = launch(ky->s_fn[0][KIND_LIN_SLAB], a.ntiles, pl->grid_y[0], ky->s_threads, ky->s_smem, &a, st);
+    }
     if (rc != FFT3D_OK) return rc;
     rec.mark(2);
 
@@ -295,7 +403,21 @@ int fft3d_r2c(const fft3d_plan_t* pl, const void* d_in, void* d_out, void* d_wor
     b.ntiles = (long long)p * L * b.ntz;
     b.in_hi = Nx * L * M; b.in_lo = M; b.in_rq = 0; b.in_rl = L * M;
     b.out_hi = Nx * L * (M + 1); b.out_lo = M + 1; b.out_rq = 0; b.out_rl = L * (M + 1);
-    rc = launch(kx->s_fn[0][KIND_LIN_LIN], b.ntiles, pl->grid_x[0], kx->s_threads, kx->s_smem, &b, st);
+    if (use_tma && pl->tma_x) {
+        TensorMapBlob mi, mo;
+        TensorMapBlob mi2;
+        const int tc = kx->tma_tc, of = kx->tma_oddfix;
+        if (!map_slab_x(pl, &mi, d_work, tc, pl->x_rows) || !map_slab_x(pl, &mi2, d_work, tc + 2, pl->x_rows) ||
+            !map_user_x(pl, &mo, d_out, tc, pl->x_rows)) return FFT3D_ECUDA;
+        TmaArgs ta{};
+        ta.user_out = d_out;
+        ta.tw = pl->tw_x; ta.ntz = (int)(M / tc);
+        ta.ntiles = of ? (long long)p * (L / 2) * (2 * ta.ntz + 1) : (long long)p * L * ta.ntz;
+        ta.L = (int)L; ta.Nx = (int)Nx; ta.Mp1 = (int)(M + 1); ta.in_rows = pl->x_rows; ta.out_rows = pl->x_rows;
+        rc = launch_tma(kx->tma_fn[TMA_X_FWD], kx, kx->tma_smem_x, pl->num_sms, mi, mi2, mo, ta, st);
+    } else {
+        rc = launch(kx->s_fn[0][KIND_LIN_LIN], b.ntiles, pl->grid_x[0], kx->s_threads, kx->s_smem, &b, st);
+    }
     if (rc != FFT3D_OK) return rc;
     rec.mark(3);
 
@@ -320,11 +442,12 @@ int fft3d_c2r(const fft3d_plan_t* pl, const void* d_in, void* d_out, void* d_wor
     // the workspace until I1 has consumed it (reading R8: only the Hermitian part of the two
     // self-conjugate planes enters Eq. (2)+(3)).
     Recorder rec(pl, 1, st);
-    rec.mark(0);
+    int slot = 0;
+    rec.mark(slot++);
     PlaneArgs f{};
     f.src = d_in; f.dst = d_work; f.Nx = (int)Nx; f.Ny = (int)Ny; f.L = (int)L; f.M = (int)M;
     if (launch_pack_nyquist(pl->dtype, f, st) != cudaSuccess) { cudaGetLastError(); return FFT3D_ECUDA; }
-    rec.mark(1);
+    rec.mark(slot++);
 
     // I1: x-axis inverse FFT: d_in (pitch M+1, column 0 from the side buffer) -> d_out scratch (pitch M)
     const KernelSet* kx = pl->kx;
@@ -335,9 +458,36 @@ int fft3d_c2r(const fft3d_plan_t* pl, const void* d_in, void* d_out, void* d_wor
     b.in_hi = Nx * L * (M + 1); b.in_lo = M + 1; b.in_rq = 0; b.in_rl = L * (M + 1);
     b.c0_hi = Nx * L; b.c0_lo = 1; b.c0_rl = L;
     b.out_hi = Nx * L * M; b.out_lo = M; b.out_rq = 0; b.out_rl = L * M;
-    int rc = launch(kx->s_fn[1][KIND_LIN_LIN], b.ntiles, pl->grid_x[1], kx->s_threads, kx->s_smem, &b, st);
+    const bool use_tma = pl->variant == 0;
+    int rc;
+    if (use_tma && pl->tma_x) {
+        TensorMapBlob mi, mo;
+        TensorMapBlob mi2;
+        const int tc = kx->tma_tc, of = kx->tma_oddfix;
+        if (!map_user_x(pl, &mi, d_in, tc, pl->x_rows) || !map_user_x(pl, &mi2, d_in, tc + 2, pl->x_rows) ||
+            !map_slab_x(pl, &mo, d_out, tc, pl->x_rows)) return FFT3D_ECUDA;
+        TmaArgs ta{};
+        ta.tw = pl->tw_x; ta.ntz = (int)(M / tc);
+        ta.ntiles = of ? (long long)p * (L / 2) * (2 * ta.ntz) : (long long)p * L * ta.ntz;
+        ta.L = (int)L; ta.Nx = (int)Nx; ta.Mp1 = (int)(M + 1); ta.in_rows = pl->x_rows; ta.out_rows = pl->x_rows;
+        rc = launch_tma(kx->tma_fn[TMA_X_INV], kx, kx->tma_smem_x, pl->num_sms, mi, mi2, mo, ta, st);
+        rec.mark(slot++);
+        // packed column 0 of the result: x-transform of the side buffer, written over the (meaningless)
+        // column the tiles produced from the user's raw kz = 0 plane
+        if (rc == FFT3D_OK) {
+            StridedArgs c0{};
+            c0.in = d_work; c0.out = d_out; c0.col0 = nullptr; c0.tw = pl->tw_x;
+            c0.ntz = (int)((L + kx->tc - 1) / kx->tc); c0.ncols = (int)L; c0.a_lo = 1; c0.L = (int)Nx;
+            c0.ntiles = (long long)p * c0.ntz;
+            c0.in_hi = Nx * L; c0.in_lo = 0; c0.in_rq = 0; c0.in_rl = L;
+            c0.out_hi = Nx * L * M; c0.out_lo = 0; c0.out_rq = 0; c0.out_rl = L * M; c0.out_cs = M;
+            rc = launch(kx->s_fn[1][KIND_LIN_LIN], c0.ntiles, pl->grid_x[1], kx->s_threads, kx->s_smem, &c0, st);
+        }
+    } else {
+        rc = launch(kx->s_fn[1][KIND_LIN_LIN], b.ntiles, pl->grid_x[1], kx->s_threads, kx->s_smem, &b, st);
+    }
     if (rc != FFT3D_OK) return rc;
-    rec.mark(2);
+    rec.mark(slot++);
 
     // I2: y-axis inverse FFT gathering rows from the slab layout: d_out scratch -> work [x][y][M]
     const KernelSet* ky = pl->ky;
@@ -347,9 +497,19 @@ int fft3d_c2r(const fft3d_plan_t* pl, const void* d_in, void* d_out, void* d_wor
     a.ntiles = Nx * a.ntz;
     a.in_hi = L * M; a.in_lo = 0; a.in_rq = Nx * L * M; a.in_rl = M;
     a.out_hi = Ny * M; a.out_lo = 0; a.out_rq = 0; a.out_rl = M;
-    rc = launch(ky->s_fn[1][KIND_SLAB_LIN], a.ntiles, pl->grid_y[1], ky->s_threads, ky->s_smem, &a, st);
+    if (use_tma && pl->tma_y) {
+        TensorMapBlob mi, mo;
+        if (!map_slab_y(pl, &mi, d_out, ky->tma_tc, pl->y_rows_slab) ||
+            !map_natural(pl, &mo, d_work, ky->tma_tc, pl->y_rows_nat)) return FFT3D_ECUDA;
+        TmaArgs ta{};
+        ta.tw = pl->tw_y; ta.ntz = (int)(M / ky->tma_tc); ta.ntiles = Nx * ta.ntz;
+        ta.L = (int)L; ta.Nx = (int)Nx; ta.Mp1 = (int)(M + 1); ta.in_rows = pl->y_rows_slab; ta.out_rows = pl->y_rows_nat;
+        rc = launch_tma(ky->tma_fn[TMA_Y_INV], ky, ky->tma_smem_y, pl->num_sms, mi, mi, mo, ta, st);
+    } else {
+        rc = launch(ky->s_fn[1][KIND_SLAB_LIN], a.ntiles, pl->grid_y[1], ky->s_threads, ky->s_smem, &a, st);
+    }
     if (rc != FFT3D_OK) return rc;
-    rec.mark(3);
+    rec.mark(slot++);
 
     // I3: z-axis C2R with the 1/(NxNyNz) normalisation: work -> d_out
     const KernelSet* kz = pl->kz;
@@ -358,7 +518,7 @@ int fft3d_c2r(const fft3d_plan_t* pl, const void* d_in, void* d_out, void* d_wor
     z.scale = 1.0 / ((double)Nx * (double)Ny * (double)Nz);
     rc = launch(kz->z_fn[1], (z.nrows + kz->z_rpb - 1) / kz->z_rpb, pl->grid_z[1], kz->z_threads,
                 kz->z_smem, &z, st);
-    rec.mark(4);
+    rec.mark(slot++);
     return rc;
 }
 

@@ -70,6 +70,16 @@ __host__ __device__ constexpr int tile_cols(int N, int csize) {
     return row_bytes / csize;
 }
 
+// Tile width of the TMA-pipelined strided passes (0 = not built for this length): the consumer
+// count S*TC must be a multiple of 32 and leave room for the producer warp.
+__host__ __device__ constexpr int tma_tile_cols(int N, int S, int csize) {
+    int tc = tile_cols(N, csize);
+    while (tc > 1 && S * tc + 32 > 1024) tc /= 2;
+    if (tc * csize < 32) return 0;                 // rows narrower than a sector: not worth it
+    if ((S * tc) % 32 != 0 || N < 64) return 0;
+    return tc;
+}
+
 // Rows per CTA iteration of the z passes: aim for ~256 threads.
 __host__ __device__ constexpr int rows_per_block(int S) {
     int r = 256 / S;
@@ -78,7 +88,7 @@ __host__ __device__ constexpr int rows_per_block(int S) {
 
 // Resident CTAs per SM the kernels are compiled for (register cap via __launch_bounds__).
 __host__ __device__ constexpr int min_blocks(int threads, int P, int tsize, size_t smem) {
-    int need = (P * 2 * (tsize / 4)) * 2 + 24;            // rough register need per thread
+    int need = P * 2 * (tsize / 4) + 32;                  // data registers + working set
     if (need > 255) need = 255;
     int by_regs = 65536 / (threads * need);
     int by_thr = 2048 / threads;

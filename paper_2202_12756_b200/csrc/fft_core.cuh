@@ -8,6 +8,10 @@
 // j + i*N/r with j = t + u*S, multiplies by exp(DIR 2 pi i * i*k/(Ns r)), k = j mod Ns, applies
 // DFT_r and scatters to elements (j/Ns)*Ns*r + k + i*Ns.  For the last stage that scatter lands
 // on the thread's own elements again, so the result stays in registers.
+//
+// Shared-memory addressing is kept LINEAR in (thread part) + (compile-time part): every LDS/STS
+// of the unrolled stages is `per-thread base register + immediate`, so the exchanges cost no
+// integer instructions beyond a handful of bases per stage.
 #pragma once
 #include "fft_radix.cuh"
 
@@ -37,50 +41,138 @@ struct FftCfg {
                   "every radix must divide P");
 };
 
-// One stage (and, recursively, the following ones).  `Idx` maps an element index of this FFT
-// to a shared-memory slot (tile column / row padding folded in).  `sync` is a CTA barrier.
-template <class Cfg, int SI, int DIR, typename T, class Idx>
+// Shared-memory slot of element e of one FFT: (e + e/PADR) * TC + c.
+//   TC   = elements between consecutive e (the tile width of a strided pass; 1 for a row pass)
+//   PADR = one element (row) of padding after every PADR elements, 0 = none: breaks the
+//          power-of-two stride of the first exchange (bank conflicts)
+//   c    = per-thread constant (tile column, or the start of the thread's row)
+template <int TC_, int PADR_>
+struct SmLayout {
+    static constexpr int TC = TC_, PADR = PADR_;
+    int c;
+    __device__ __forceinline__ int at(int e) const {
+        if constexpr (PADR_ > 0) return (e + e / PADR_) * TC_ + c;
+        else return e * TC_ + c;
+    }
+    // slot offset contributed by a compile-time element offset (valid when the split is additive)
+    __host__ __device__ static constexpr int off(int econst) {
+        return (PADR_ > 0 ? econst + econst / PADR_ : econst) * TC_;
+    }
+};
+
+struct CtaSync {
+    __device__ __forceinline__ void operator()() const { __syncthreads(); }
+};
+// named barrier over the first `NT` threads of the CTA (warp-specialised kernels)
+template <int ID, int NT>
+struct NamedSync {
+    __device__ __forceinline__ void operator()() const {
+        asm volatile("bar.sync %0, %1;" ::"n"(ID), "n"(NT) : "memory");
+    }
+};
+
+template <class Cfg, class Lay>
+struct StageAddr {
+    static constexpr int S = Cfg::S;
+    // the (thread part) + (compile-time part) split of slot addresses is exact when no carry can
+    // cross a padding boundary
+    static constexpr bool LINEAR = (Lay::PADR == 0) || (S % Lay::PADR == 0 && Lay::PADR == Cfg::radix(0));
+};
+
+// Read the thread's P elements (t + m*S) from shared memory.
+template <class Cfg, typename T, class Lay>
+__device__ __forceinline__ void read_own(cx<T> (&v)[Cfg::P], const cx<T>* __restrict__ sm, int t, const Lay& lay) {
+    constexpr int P = Cfg::P, S = Cfg::S;
+    if constexpr (StageAddr<Cfg, Lay>::LINEAR) {
+        const cx<T>* b = sm + lay.at(t);
+#pragma unroll
+        for (int m = 0; m < P; ++m) v[m] = b[Lay::off(m * S)];
+    } else {
+#pragma unroll
+        for (int m = 0; m < P; ++m) v[m] = sm[lay.at(t + m * S)];
+    }
+}
+
+template <class Cfg, typename T, class Lay>
+__device__ __forceinline__ void write_own(const cx<T> (&v)[Cfg::P], cx<T>* __restrict__ sm, int t, const Lay& lay) {
+    constexpr int P = Cfg::P, S = Cfg::S;
+    if constexpr (StageAddr<Cfg, Lay>::LINEAR) {
+        cx<T>* b = sm + lay.at(t);
+#pragma unroll
+        for (int m = 0; m < P; ++m) b[Lay::off(m * S)] = v[m];
+    } else {
+#pragma unroll
+        for (int m = 0; m < P; ++m) sm[lay.at(t + m * S)] = v[m];
+    }
+}
+
+// One stage (and, recursively, the following ones).
+template <class Cfg, int SI, int DIR, typename T, class Lay, class Sync>
 __device__ __forceinline__ void fft_stages(cx<T> (&v)[Cfg::P], cx<T>* __restrict__ sm,
-                                           const cx<T>* __restrict__ tw, int t, const Idx& idx) {
+                                           const cx<T>* __restrict__ tw, int t, const Lay& lay,
+                                           const Sync& sync) {
     using C = cx<T>;
     constexpr int r = Cfg::radix(SI), Ns = Cfg::ns(SI), P = Cfg::P, S = Cfg::S, B = P / r;
     constexpr bool last = (SI == Cfg::NST - 1);
-    if constexpr (!last && SI > 0) __syncthreads();      // everyone has read the previous exchange
+    constexpr bool LIN = StageAddr<Cfg, Lay>::LINEAR;
+    // how j = t + u*S splits into (j / Ns, j % Ns)
+    constexpr bool CASE_A = (S % Ns == 0);                 // j%Ns = t%Ns, j/Ns = t/Ns + u*S/Ns
+    constexpr bool CASE_B = !CASE_A && (Ns % S == 0);      // j%Ns = t + (u%(Ns/S))*S, j/Ns = u/(Ns/S)
+    if constexpr (!last && SI > 0) sync();                 // everyone has read the previous exchange
+
+    int jr_run = 0, erun = 0;                              // thread parts of j%Ns and of the scatter base
+    if constexpr (CASE_A) { jr_run = t % Ns; erun = (t / Ns) * (Ns * r) + jr_run; }
+    else if constexpr (CASE_B) { jr_run = t; erun = t; }
+    const C* twb = tw + Cfg::twoff(SI) + jr_run;
+    C* wb = sm + ((LIN && (CASE_A || CASE_B)) ? lay.at(erun) : 0);
+
 #pragma unroll
     for (int u = 0; u < B; ++u) {
         C a[r];
 #pragma unroll
         for (int i = 0; i < r; ++i) a[i] = v[u + i * B];
-        const int j = t + u * S;
+        // compile-time parts
+        int jr_c = 0, e_c = 0;
+        if constexpr (CASE_A) { jr_c = 0; e_c = u * (S / Ns) * (Ns * r); }
+        else if constexpr (CASE_B) { jr_c = (u % (Ns / S)) * S; e_c = (u / (Ns / S)) * (Ns * r) + jr_c; }
         if constexpr (Ns > 1) {
-            const int k = j % Ns;
-            const C* twk = tw + Cfg::twoff(SI) + k;
+            if constexpr (CASE_A || CASE_B) {
 #pragma unroll
-            for (int i = 1; i < r; ++i) a[i] = cmul(a[i], twk[(i - 1) * Ns]);
+                for (int i = 1; i < r; ++i) a[i] = cmul(a[i], twb[jr_c + (i - 1) * Ns]);
+            } else {
+                const int k = (t + u * S) % Ns;
+                const C* twk = tw + Cfg::twoff(SI) + k;
+#pragma unroll
+                for (int i = 1; i < r; ++i) a[i] = cmul(a[i], twk[(i - 1) * Ns]);
+            }
         }
         dft<r, DIR, T>(a);
         if constexpr (last) {
 #pragma unroll
             for (int i = 0; i < r; ++i) v[u + i * B] = a[i];
+        } else if constexpr (LIN && (CASE_A || CASE_B)) {
+#pragma unroll
+            for (int i = 0; i < r; ++i) wb[Lay::off(e_c + i * Ns)] = a[i];
         } else {
+            const int j = t + u * S;
             const int j0 = (j / Ns) * (Ns * r) + (j % Ns);
 #pragma unroll
-            for (int i = 0; i < r; ++i) sm[idx(j0 + i * Ns)] = a[i];
+            for (int i = 0; i < r; ++i) sm[lay.at(j0 + i * Ns)] = a[i];
         }
     }
     if constexpr (!last) {
-        __syncthreads();
-#pragma unroll
-        for (int m = 0; m < P; ++m) v[m] = sm[idx(t + m * S)];
-        fft_stages<Cfg, SI + 1, DIR, T, Idx>(v, sm, tw, t, idx);
+        sync();
+        read_own<Cfg, T, Lay>(v, sm, t, lay);
+        fft_stages<Cfg, SI + 1, DIR, T, Lay, Sync>(v, sm, tw, t, lay, sync);
     }
 }
 
 // Copy the plan's forward twiddle table (exp(-2 pi i ...)) into shared memory, conjugated for
 // the inverse direction.
 template <int DIR, typename T>
-__device__ __forceinline__ void load_twiddles(cx<T>* dst, const cx<T>* __restrict__ src, int n) {
-    for (int i = threadIdx.x; i < n; i += blockDim.x) {
+__device__ __forceinline__ void load_twiddles(cx<T>* dst, const cx<T>* __restrict__ src, int n,
+                                              int tid, int nthreads) {
+    for (int i = tid; i < n; i += nthreads) {
         cx<T> w = src[i];
         if constexpr (DIR > 0) w.y = -w.y;
         dst[i] = w;

@@ -4,6 +4,9 @@
 #include "fft_configs.cuh"
 #include "fft_registry.h"
 
+#ifndef FFT3D_PREFETCH
+#define FFT3D_PREFETCH true
+#endif
 #ifndef FFT3D_N
 #error "compile with -DFFT3D_N=<length>"
 #endif
@@ -19,7 +22,8 @@ static KernelSet make_set(int dtype) {
     constexpr size_t TWB = (size_t)((Cfg::TWN + 1) & ~1) * sizeof(C);
     constexpr size_t S_SMEM = TWB + (size_t)TP::ROWS * TC * sizeof(C);
     constexpr int S_THREADS = Cfg::S * TC;
-    constexpr int S_MINB = min_blocks(S_THREADS, Cfg::P, (int)sizeof(T), S_SMEM);
+    constexpr bool S_PF = FFT3D_PREFETCH;
+    constexpr int S_MINB = S_PF ? 1 : min_blocks(S_THREADS, Cfg::P, (int)sizeof(T), S_SMEM);
     constexpr int RPB = rows_per_block(Cfg::S);
     constexpr size_t Z_SMEM = TWB + (size_t)Cfg::N * sizeof(C) + (size_t)RPB * RowPad<Cfg>::PITCH * sizeof(C);
     constexpr int Z_THREADS = Cfg::S * RPB;
@@ -35,17 +39,37 @@ static KernelSet make_set(int dtype) {
     k.tc = TC;
     k.s_threads = S_THREADS;
     k.s_smem = S_SMEM;
-    k.s_fn[0][KIND_LIN_LIN]  = (const void*)fft_strided_kernel<Cfg, TC, -1, false, false, T, S_MINB>;
-    k.s_fn[0][KIND_LIN_SLAB] = (const void*)fft_strided_kernel<Cfg, TC, -1, false, true, T, S_MINB>;
+    k.s_fn[0][KIND_LIN_LIN]  = (const void*)fft_strided_kernel<Cfg, TC, -1, false, false, T, S_MINB, S_PF>;
+    k.s_fn[0][KIND_LIN_SLAB] = (const void*)fft_strided_kernel<Cfg, TC, -1, false, true, T, S_MINB, S_PF>;
     k.s_fn[0][KIND_SLAB_LIN] = nullptr;
-    k.s_fn[1][KIND_LIN_LIN]  = (const void*)fft_strided_kernel<Cfg, TC, +1, false, false, T, S_MINB>;
+    k.s_fn[1][KIND_LIN_LIN]  = (const void*)fft_strided_kernel<Cfg, TC, +1, false, false, T, S_MINB, S_PF>;
     k.s_fn[1][KIND_LIN_SLAB] = nullptr;
-    k.s_fn[1][KIND_SLAB_LIN] = (const void*)fft_strided_kernel<Cfg, TC, +1, true, false, T, S_MINB>;
+    k.s_fn[1][KIND_SLAB_LIN] = (const void*)fft_strided_kernel<Cfg, TC, +1, true, false, T, S_MINB, S_PF>;
     k.z_rpb = RPB;
     k.z_threads = Z_THREADS;
     k.z_smem = Z_SMEM;
     k.z_fn[0] = (const void*)fft_z_r2c_kernel<Cfg, RPB, T, Z_MINB>;
     k.z_fn[1] = (const void*)fft_z_c2r_kernel<Cfg, RPB, T, Z_MINB>;
+    constexpr int TTC = tma_tile_cols(Cfg::N, Cfg::S, (int)sizeof(C));
+    if constexpr (TTC > 0) {
+        // complex fp32 rows of the user's spectrum (M+1 entries) start on 8-byte boundaries for odd l:
+        // the X passes shift those tiles' windows (ODDFIX, see fft_kernels.cuh)
+        constexpr bool OF = sizeof(C) % 16 != 0;
+        using TY = TmaTile<Cfg, TTC, T, false>;
+        using TX = TmaTile<Cfg, TTC, T, OF>;
+        constexpr int NSY = TY::max_stages(), NSX = TX::max_stages();
+        if constexpr (NSY >= 2 && NSX >= 2) {
+            k.tma_fn[TMA_Y_FWD] = (const void*)fft_strided_tma_kernel<Cfg, TTC, TMA_Y_FWD, T, NSY, false>;
+            k.tma_fn[TMA_Y_INV] = (const void*)fft_strided_tma_kernel<Cfg, TTC, TMA_Y_INV, T, NSY, false>;
+            k.tma_fn[TMA_X_FWD] = (const void*)fft_strided_tma_kernel<Cfg, TTC, TMA_X_FWD, T, NSX, OF>;
+            k.tma_fn[TMA_X_INV] = (const void*)fft_strided_tma_kernel<Cfg, TTC, TMA_X_INV, T, NSX, OF>;
+            k.tma_oddfix = OF ? 1 : 0;
+            k.tma_tc = TTC;
+            k.tma_threads = TY::NCONS + 32;
+            k.tma_smem_y = (size_t)TY::smem_bytes(NSY);
+            k.tma_smem_x = (size_t)TX::smem_bytes(NSX);
+        }
+    }
     return k;
 }
 

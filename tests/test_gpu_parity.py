@@ -32,10 +32,11 @@ def fft():
     return m
 
 
-def run_forward(fft, f_host, p):
+def run_forward(fft, f_host, p, variant=0):
     """f_host: torch CPU real tensor.  Returns (natural-order spectrum as numpy c128, plan, flat device out)."""
     shape = tuple(f_host.shape)
     plan = fft.Plan(*shape, dtype=f_host.dtype, virtual_slabs=p)
+    plan.set_variant(variant)
     d_in = f_host.cuda()
     keep = d_in.clone()
     out = plan.r2c(d_in)
@@ -56,16 +57,20 @@ SMALL = [
     ((24, 12, 192), 4),
     ((128, 256, 32), 16),
     ((4, 6, 8), 2),
+    ((256, 128, 256), 2),       # several TMA boxes per tile on x, slab boxes spanning whole slabs on y
+    ((64, 512, 64), 1),         # L = 512 > 256: slab boxes are parts of one slab
+    ((384, 192, 48), 12),       # 3*2^a lengths through the TMA path
 ]
 
 
 @pytest.mark.parametrize("shape,p", SMALL)
 @pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
-def test_r2c_and_c2r_match_oracle(fft, oracle_mod, shape, p, dtype):
+@pytest.mark.parametrize("variant", [0, 1])     # 0: TMA-pipelined strided passes where possible, 1: plain-load kernels
+def test_r2c_and_c2r_match_oracle(fft, oracle_mod, shape, p, dtype, variant):
     from paper_2202_12756_b200 import inputs
     f = inputs.uniform_grid(shape, dtype, seed=0)
     F_ref = oracle_mod.r2c(f.double().numpy())
-    F_gpu, plan, d_out = run_forward(fft, f, p)
+    F_gpu, plan, d_out = run_forward(fft, f, p, variant)
     assert rel_l2(F_gpu, F_ref) <= tol(shape, dtype)
     # the slab layout agrees with fft3d_index on a sample of entries
     rng = np.random.Generator(np.random.PCG64(1))
@@ -119,13 +124,14 @@ def test_results_do_not_depend_on_virtual_slabs(fft, dtype):
     shape = (32, 64, 32)
     f = inputs.normal_grid(shape, dtype, seed=5)
     ref = None
-    for p in (1, 2, 8, 32):
-        F, plan, d_out = run_forward(fft, f, p)
-        back = plan.c2r(d_out).cpu()
-        if ref is None:
-            ref = (F, back)
-        else:
-            assert np.array_equal(F, ref[0]) and torch.equal(back, ref[1])
+    for variant in (0, 1):
+        for p in (1, 2, 8, 32):
+            F, plan, d_out = run_forward(fft, f, p, variant)
+            back = plan.c2r(d_out).cpu()
+            if ref is None:
+                ref = (F, back)
+            else:
+                assert np.array_equal(F, ref[0]) and torch.equal(back, ref[1])
     # and run to run
     F2, _, _ = run_forward(fft, f, 1)
     assert np.array_equal(F2, ref[0])
