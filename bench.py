@@ -2,7 +2,7 @@
 """bench.py -- the headline measurement: one step = one 3D R2C + C2R pair (all hot-path passes)
 on the 1024^3 fp32 grid of BASELINE.json configs[2], inputs resident in HBM.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--n 1024] [--slabs 8]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--size 1024] [--slabs 8]
 
 Prints ONE JSON line (rank 0).  `value` = GFLOP/s by BASELINE.json's convention
 (2.5 N^3 log2 N^3 per real transform, 5 per pair; the paper's convention, is 2x).
@@ -143,8 +143,8 @@ def time_oracle(sample_n, field, steps, warmup, cores):
 
 
 def run_reference(args):
-    rank = int(os.environ.get("RANK", "0"))
-    if rank != 0:
+    _world, rank, _local = dist_env()
+    if rank != 0:                                   # rank 0 alone runs and prints the reference arm
         return
     import numpy as np
     import oracle
@@ -174,6 +174,41 @@ def run_reference(args):
 
 
 # ------------------------------------------------------------------------------------------
+# multi-process plumbing (one process per GPU; replicas, no data-path collective -- DESIGN.md 8)
+# ------------------------------------------------------------------------------------------
+def dist_env():
+    return (int(os.environ.get("WORLD_SIZE", "1")), int(os.environ.get("RANK", "0")),
+            int(os.environ.get("LOCAL_RANK", "0")))
+
+
+def dist_init(world, backend, device=None):
+    """torch.distributed process group for world > 1 (rendezvous from MASTER_ADDR/PORT), else None."""
+    if world <= 1:
+        return None
+    import torch.distributed as dist
+    if device is not None:
+        dist.init_process_group(backend, device_id=device)
+    else:
+        dist.init_process_group(backend)
+    return dist
+
+
+def max_over_ranks(x, dist, device="cpu"):
+    """The slowest rank's time: a job of replicas is as slow as its slowest member."""
+    if dist is None:
+        return float(x)
+    import torch
+    t = torch.tensor([float(x)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def job_gflops(world, shape, seconds_per_step):
+    """Whole-job rate: every rank transforms its own grid in the same (max-over-ranks) time."""
+    return world * flops_pair(shape) / seconds_per_step / 1e9
+
+
+# ------------------------------------------------------------------------------------------
 # CUDA arm
 # ------------------------------------------------------------------------------------------
 def run_cuda(args):
@@ -181,17 +216,12 @@ def run_cuda(args):
     import paper_2202_12756_b200 as pkg
     from paper_2202_12756_b200 import inputs
 
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
-    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world, rank, local_rank = dist_env()
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: the FFT path has no CPU fallback")
     torch.cuda.set_device(local_rank)
     dev = torch.device("cuda", local_rank)
-    dist = None
-    if world > 1:
-        import torch.distributed as dist
-        dist.init_process_group("nccl", device_id=dev)
+    dist = dist_init(world, "nccl", dev)
 
     def barrier():
         if dist is not None:
@@ -228,12 +258,9 @@ def run_cuda(args):
     t_fwd, c_fwd = plan.timing_read(0)
     t_inv, c_inv = plan.timing_read(1)
     plan.timing_enable(0)
-    if dist is not None:
-        t = torch.tensor([ms_total], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total = float(t.item())
+    ms_total = max_over_ranks(ms_total, dist, dev)
     ms_step = ms_total / args.steps
-    value = world * flops_pair(shape) / (ms_step * 1e-3) / 1e9
+    value = job_gflops(world, shape, ms_step * 1e-3)
 
     # sanity: the timed result is a real transform pair (round trip recovers the field)
     rt_err = (back - field).abs().max().item() / field.abs().max().item()
@@ -280,12 +307,9 @@ def run_cuda(args):
             plan.c2r_host(h_spec, h_back)
         torch.cuda.synchronize()
         dt = (time.perf_counter() - t0) / args.e2e_steps
-        if dist is not None:
-            t = torch.tensor([dt], dtype=torch.float64, device=dev)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            dt = float(t.item())
+        dt = max_over_ranks(dt, dist, dev)
         e2e_rt = (h_back - h_in).abs().max().item() / h_in.abs().max().item()
-        e2e = {"value": world * flops_pair(shape) / dt / 1e9, "unit": "GFLOP/s", "ms_per_step": dt * 1e3,
+        e2e = {"value": job_gflops(world, shape, dt), "unit": "GFLOP/s", "ms_per_step": dt * 1e3,
                "h2d_bytes_per_step": real_b + cplx_b, "d2h_bytes_per_step": cplx_b + real_b,
                "round_trip_rel_err": e2e_rt}
 
@@ -332,7 +356,7 @@ def main():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
-    ap.add_argument("--n", type=int, default=1024)
+    ap.add_argument("--size", "--n", dest="n", type=int, default=1024)
     ap.add_argument("--slabs", type=int, default=8)
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--no-e2e", action="store_true")
