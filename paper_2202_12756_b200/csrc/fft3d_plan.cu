@@ -20,6 +20,7 @@
 #include "../../include/fft3d.h"
 #include "fft_configs.cuh"
 #include "fft_kernels.cuh"
+#include "fft_zpass.cuh"
 #include "fft_registry.h"
 
 namespace fft3d {
@@ -62,6 +63,7 @@ struct fft3d_plan_s {
     int variant;
     const KernelSet *kz, *ky, *kx;
     void *tw_z, *tw_y, *tw_x, *twz;     // device tables
+    void* tw_zb;                        // stage twiddles of the bulk-pipelined z kernels
     int num_sms;
     int grid_z[2], grid_y[2], grid_x[2];   // persistent grid sizes [fwd, inv]
     // buffers of the host-pointer entry points (lazy)
@@ -71,6 +73,7 @@ struct fft3d_plan_s {
     // TMA-pipelined strided passes
     void* encode_fn;           // cuTensorMapEncodeTiled, resolved at run time (no libcuda link dependency)
     bool tma_y, tma_x;         // usable for this plan's extents / alignment
+    bool bulk_z;               // bulk-pipelined z kernels usable (row count a multiple of the tile)
     int y_rows_nat, y_rows_slab, x_rows;   // rows per TMA box
 };
 
@@ -98,14 +101,14 @@ void store(std::vector<unsigned char>& buf, size_t i, long double c, long double
 }
 
 // Stage tables of fft_core.cuh: stage s >= 1, entry (i-1)*Ns + k = exp(-2 pi i * i*k/(Ns*r)).
-int upload_stage_twiddles(const KernelSet* k, int esize, void** dptr) {
+int upload_stage_twiddles(int nst, const int* radix, int twn, int esize, void** dptr) {
     *dptr = nullptr;
-    size_t n = (size_t)(k->twn > 0 ? k->twn : 1);
+    size_t n = (size_t)(twn > 0 ? twn : 1);
     std::vector<unsigned char> buf(n * 2 * esize, 0);
     size_t off = 0;
-    long long Ns = k->radix[0];
-    for (int s = 1; s < k->nst; ++s) {
-        int r = k->radix[s];
+    long long Ns = radix[0];
+    for (int s = 1; s < nst; ++s) {
+        int r = radix[s];
         for (int i = 1; i < r; ++i)
             for (long long kk = 0; kk < Ns; ++kk) {
                 long double c, sn;
@@ -227,6 +230,18 @@ int launch_tma(const void* fn, const KernelSet* k, size_t smem, int num_sms, con
     return FFT3D_OK;
 }
 
+int launch_zbulk(const fft3d_plan_s* pl, int d, const void* in, void* out, double scale, cudaStream_t st) {
+    const KernelSet* kz = pl->kz;
+    ZBulkArgs z{};
+    z.in = in; z.out = out; z.tw = pl->tw_zb; z.twz = pl->twz;
+    z.ntiles = pl->Nx * pl->Ny / kz->zb_rpt; z.scale = scale;
+    long long g = z.ntiles < pl->num_sms ? z.ntiles : pl->num_sms;
+    void* argv[1] = {&z};
+    cudaError_t e = cudaLaunchKernel(kz->zb_fn[d], dim3((unsigned)g), dim3((unsigned)kz->zb_threads), argv, kz->zb_smem, st);
+    if (e != cudaSuccess) { cudaGetLastError(); return FFT3D_ECUDA; }
+    return FFT3D_OK;
+}
+
 // event slot `i` of the call being recorded for direction `which`, or no-op
 struct Recorder {
     TimingState* t;
@@ -278,9 +293,11 @@ int fft3d_plan(fft3d_plan_t** out, long long Nx, long long Ny, long long Nz, int
     pl->dtype = dtype; pl->esize = dtype == FFT3D_F32 ? 4 : 8;
     pl->kz = kz; pl->ky = ky; pl->kx = kx; pl->num_sms = sms;
 
-    int rc = upload_stage_twiddles(kz, pl->esize, &pl->tw_z);
-    if (rc == FFT3D_OK) rc = upload_stage_twiddles(ky, pl->esize, &pl->tw_y);
-    if (rc == FFT3D_OK) rc = upload_stage_twiddles(kx, pl->esize, &pl->tw_x);
+    int rc = upload_stage_twiddles(kz->nst, kz->radix, kz->twn, pl->esize, &pl->tw_z);
+    if (rc == FFT3D_OK) rc = upload_stage_twiddles(ky->nst, ky->radix, ky->twn, pl->esize, &pl->tw_y);
+    if (rc == FFT3D_OK) rc = upload_stage_twiddles(kx->nst, kx->radix, kx->twn, pl->esize, &pl->tw_x);
+    if (rc == FFT3D_OK && kz->zb_fn[0] != nullptr)
+        rc = upload_stage_twiddles(kz->zb_nst, kz->zb_radix, kz->zb_twn, pl->esize, &pl->tw_zb);
     if (rc == FFT3D_OK) rc = upload_z_twiddles(Nz, pl->M, pl->esize, &pl->twz);
     for (int d = 0; d < 2 && rc == FFT3D_OK; ++d) {
         rc = prepare_kernel(kz->z_fn[d], kz->z_threads, kz->z_smem, sms, &pl->grid_z[d]);
@@ -317,6 +334,13 @@ int fft3d_plan(fft3d_plan_t** out, long long Nx, long long Ny, long long Nz, int
                 int g = 0;
                 rc = prepare_kernel(kx->tma_fn[d == 0 ? TMA_X_FWD : TMA_X_INV], kx->tma_threads, kx->tma_smem_x, sms, &g);
             }
+        }
+    }
+    if (rc == FFT3D_OK && kz->zb_fn[0] != nullptr && (Nx * Ny) % kz->zb_rpt == 0) {
+        pl->bulk_z = true;
+        for (int d = 0; d < 2 && rc == FFT3D_OK; ++d) {
+            int g = 0;
+            rc = prepare_kernel(kz->zb_fn[d], kz->zb_threads, kz->zb_smem, sms, &g);
         }
     }
     if (rc != FFT3D_OK) { fft3d_destroy(pl); return rc; }
@@ -367,8 +391,9 @@ int fft3d_r2c(const fft3d_plan_t* pl, const void* d_in, void* d_out, void* d_wor
     ZArgs z{};
     z.in = d_in; z.out = d_out; z.tw = pl->tw_z; z.twz = pl->twz; z.nrows = Nx * Ny; z.scale = 1.0;
     const KernelSet* kz = pl->kz;
-    int rc = launch(kz->z_fn[0], (z.nrows + kz->z_rpb - 1) / kz->z_rpb, pl->grid_z[0], kz->z_threads,
-                    kz->z_smem, &z, st);
+    int rc;
+    if (pl->variant == 0 && pl->bulk_z) rc = launch_zbulk(pl, 0, d_in, d_out, 1.0, st);
+    else rc = launch(kz->z_fn[0], (z.nrows + kz->z_rpb - 1) / kz->z_rpb, pl->grid_z[0], kz->z_threads, kz->z_smem, &z, st);
     if (rc != FFT3D_OK) return rc;
     rec.mark(1);
 
@@ -516,8 +541,8 @@ int fft3d_c2r(const fft3d_plan_t* pl, const void* d_in, void* d_out, void* d_wor
     ZArgs z{};
     z.in = d_work; z.out = d_out; z.tw = pl->tw_z; z.twz = pl->twz; z.nrows = Nx * Ny;
     z.scale = 1.0 / ((double)Nx * (double)Ny * (double)Nz);
-    rc = launch(kz->z_fn[1], (z.nrows + kz->z_rpb - 1) / kz->z_rpb, pl->grid_z[1], kz->z_threads,
-                kz->z_smem, &z, st);
+    if (use_tma && pl->bulk_z) rc = launch_zbulk(pl, 1, d_work, d_out, z.scale, st);
+    else rc = launch(kz->z_fn[1], (z.nrows + kz->z_rpb - 1) / kz->z_rpb, pl->grid_z[1], kz->z_threads, kz->z_smem, &z, st);
     rec.mark(slot++);
     return rc;
 }
@@ -624,7 +649,7 @@ int fft3d_c2r_host(fft3d_plan_t* pl, const void* h_in, void* h_out) {
 
 int fft3d_destroy(fft3d_plan_t* pl) {
     if (pl == nullptr) return FFT3D_OK;
-    cudaFree(pl->tw_z); cudaFree(pl->tw_y); cudaFree(pl->tw_x); cudaFree(pl->twz);
+    cudaFree(pl->tw_zb); cudaFree(pl->tw_z); cudaFree(pl->tw_y); cudaFree(pl->tw_x); cudaFree(pl->twz);
     cudaFree(pl->h_real); cudaFree(pl->h_cplx); cudaFree(pl->h_work);
     if (pl->h_stream) cudaStreamDestroy(pl->h_stream);
     timing_free(pl);

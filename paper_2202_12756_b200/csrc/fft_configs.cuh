@@ -26,7 +26,7 @@ FFT3D_CFG(float, 64, 8, 8, 8)
 FFT3D_CFG(float, 128, 16, 16, 8)
 FFT3D_CFG(float, 256, 16, 16, 16)
 FFT3D_CFG(float, 512, 16, 16, 16, 2)
-FFT3D_CFG(float, 1024, 16, 16, 16, 4)
+FFT3D_CFG(float, 1024, 32, 32, 32)
 FFT3D_CFG(float, 2048, 16, 16, 16, 8)
 FFT3D_CFG(float, 4096, 16, 16, 16, 16)
 FFT3D_CFG(float, 6, 6, 6)
@@ -62,6 +62,12 @@ FFT3D_CFG(double, 384, 12, 12, 4, 4, 2)
 FFT3D_CFG(double, 768, 12, 12, 4, 4, 4)
 FFT3D_CFG(double, 1536, 12, 12, 4, 4, 4, 2)
 FFT3D_CFG(double, 3072, 12, 12, 4, 4, 4, 4)
+
+// Factorisation used by the bulk-pipelined z kernels (fft_zpass.cuh): the strided-pass one unless
+// a shape with fewer exchanges fits a row's threads inside one warp.
+template <typename T, int N> struct ZCfgFor { using type = typename CfgFor<T, N>::type; };
+template <> struct ZCfgFor<float, 512> { using type = FftCfg<512, 32, 32, 16>; };
+template <> struct ZCfgFor<float, 256> { using type = FftCfg<256, 16, 16, 16>; };
 
 // Tile width (columns) of the strided passes: 128-byte rows while the tile stays small,
 // 64-byte rows up to N = 2048, 32-byte rows beyond.

@@ -76,7 +76,10 @@ struct StageAddr {
     static constexpr int S = Cfg::S;
     // the (thread part) + (compile-time part) split of slot addresses is exact when no carry can
     // cross a padding boundary
-    static constexpr bool LINEAR = (Lay::PADR == 0) || (S % Lay::PADR == 0 && Lay::PADR == Cfg::radix(0));
+    // (S a multiple of the padding period; or, for two-stage transforms -- whose only scatter is
+    // stage 0 -- S a divisor of it: then (t + m*S)/PADR = (m*S)/PADR for every t < S)
+    static constexpr bool LINEAR = (Lay::PADR == 0) ||
+        (Lay::PADR == Cfg::radix(0) && (S % Lay::PADR == 0 || (Lay::PADR % S == 0 && Cfg::NST == 2)));
 };
 
 // Read the thread's P elements (t + m*S) from shared memory.

@@ -1,6 +1,7 @@
 // fft_inst.cu -- compiled once per FFT length (-DFFT3D_N=<n>): instantiates the z and strided
 // kernels for fp32 and fp64 and exports their description.
 #include "fft_kernels.cuh"
+#include "fft_zpass.cuh"
 #include "fft_configs.cuh"
 #include "fft_registry.h"
 
@@ -68,6 +69,25 @@ static KernelSet make_set(int dtype) {
             k.tma_threads = TY::NCONS + 32;
             k.tma_smem_y = (size_t)TY::smem_bytes(NSY);
             k.tma_smem_x = (size_t)TX::smem_bytes(NSX);
+        }
+    }
+    // bulk-pipelined z kernels: a row's S threads inside one warp, ~256 threads per 64 KiB tile
+    using ZCfg = typename ZCfgFor<T, FFT3D_N>::type;
+    if constexpr (ZCfg::S >= 8 && ZCfg::S <= 32 && (ZCfg::S & (ZCfg::S - 1)) == 0 && ZCfg::P % 2 == 0 &&
+                  ZCfg::N * sizeof(C) >= 1024) {
+        constexpr int RPT = 256 / ZCfg::S;
+        using ZT = ZTile<ZCfg, RPT, T>;
+        constexpr int NG = ZT::max_stages(2) >= 3 ? 2 : 1;
+        constexpr int NS = ZT::max_stages(NG) > 4 ? 4 : ZT::max_stages(NG);
+        if constexpr (NS >= 2) {
+            k.zb_fn[0] = (const void*)fft_z_bulk_kernel<ZCfg, RPT, -1, T, NS, NG>;
+            k.zb_fn[1] = (const void*)fft_z_bulk_kernel<ZCfg, RPT, +1, T, NS, NG>;
+            k.zb_rpt = RPT;
+            k.zb_nst = ZCfg::NST;
+            for (int s = 0; s < 5; ++s) k.zb_radix[s] = s < ZCfg::NST ? ZCfg::radix(s) : 1;
+            k.zb_twn = ZCfg::TWN;
+            k.zb_threads = ZT::GROUP * NG + 32;
+            k.zb_smem = (size_t)ZT::smem_bytes(NS, NG);
         }
     }
     return k;

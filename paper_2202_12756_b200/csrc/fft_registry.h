@@ -29,6 +29,12 @@ struct KernelSet {
     int tma_threads;           // consumers + one producer warp
     int tma_oddfix;            // 1: the X passes shift the windows of odd-l rows (fp32, see fft_kernels.cuh)
     size_t tma_smem_y, tma_smem_x;
+    // bulk-copy pipelined z kernels (null if not compiled for this length)
+    const void* zb_fn[2];      // [0 = R2C, 1 = C2R]
+    int zb_rpt;                // rows per tile: the row count must be a multiple
+    int zb_nst, zb_radix[5], zb_twn;   // their factorisation (it may differ from the strided kernels')
+    int zb_threads;            // consumer groups + one producer warp
+    size_t zb_smem;
 };
 
 // nullptr if this build has no kernels for (n, dtype)
