@@ -68,6 +68,7 @@ FFT3D_CFG(double, 3072, 12, 12, 4, 4, 4, 4)
 template <typename T, int N> struct ZCfgFor { using type = typename CfgFor<T, N>::type; };
 template <> struct ZCfgFor<float, 512> { using type = FftCfg<512, 32, 32, 16>; };
 template <> struct ZCfgFor<float, 256> { using type = FftCfg<256, 16, 16, 16>; };
+template <> struct ZCfgFor<double, 512> { using type = FftCfg<512, 16, 16, 16, 2>; };
 
 // Tile width (columns) of the strided passes: 128-byte rows while the tile stays small,
 // 64-byte rows up to N = 2048, 32-byte rows beyond.

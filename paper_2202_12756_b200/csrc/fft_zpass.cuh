@@ -223,6 +223,11 @@ __global__ void __launch_bounds__(Cfg::S * RPT * NG + 32, 1) fft_z_bulk_kernel(c
         const int s = (int)(i % NSTAGE);
         C* buf = reinterpret_cast<C*>(stages + s * ZT::STAGE_BYTES);
         tma::mbar_wait(&full[s], (unsigned)((i / NSTAGE) & 1));
+#ifdef FFT3D_COPY_ONLY_Z   // experiment: data movement without the transform (wrong results by design)
+        tma::fence_proxy_async(); __syncwarp();
+        if ((tid & 31) == 0) tma::mbar_arrive(&done[s]);
+        continue;
+#endif
         C v[P];
         read_own<Cfg, T>(v, buf, t, dense);
         if constexpr (DIR > 0) {
