@@ -220,12 +220,12 @@ bool map_user_x(const fft3d_plan_s* pl, TensorMapBlob* m, const void* base, int 
     return make_map(pl, m, base, 3, d, st, b);
 }
 
-int launch_tma(const void* fn, const KernelSet* k, size_t smem, int num_sms, const TensorMapBlob& in_map,
+int launch_tma(const void* fn, int threads, size_t smem, int num_sms, const TensorMapBlob& in_map,
                const TensorMapBlob& in_map2, const TensorMapBlob& out_map, TmaArgs& a, cudaStream_t st) {
     long long g = a.ntiles < num_sms ? a.ntiles : num_sms;
     if (g <= 0) return FFT3D_OK;
     void* argv[4] = {(void*)&in_map, (void*)&in_map2, (void*)&out_map, (void*)&a};
-    cudaError_t e = cudaLaunchKernel(fn, dim3((unsigned)g), dim3((unsigned)k->tma_threads), argv, smem, st);
+    cudaError_t e = cudaLaunchKernel(fn, dim3((unsigned)g), dim3((unsigned)threads), argv, smem, st);
     if (e != cudaSuccess) { cudaGetLastError(); return FFT3D_ECUDA; }
     return FFT3D_OK;
 }
@@ -326,13 +326,13 @@ int fft3d_plan(fft3d_plan_t** out, long long Nx, long long Ny, long long Nz, int
                 rc = prepare_kernel(ky->tma_fn[d == 0 ? TMA_Y_FWD : TMA_Y_INV], ky->tma_threads, ky->tma_smem_y, sms, &g);
             }
         }
-        if (rc == FFT3D_OK && fn != nullptr && strides_ok && kx->tma_fn[TMA_X_FWD] != nullptr && M % kx->tma_tc == 0 &&
+        if (rc == FFT3D_OK && fn != nullptr && strides_ok && kx->tma_fn[TMA_X_FWD] != nullptr && M % kx->tma_tc_x == 0 &&
             (L * (M + 1) * sz) % 16 == 0 && (!kx->tma_oddfix || L % 2 == 0)) {
             pl->x_rows = (int)largest_divisor_le(Nx, 256);
             pl->tma_x = true;
             for (int d = 0; d < 2 && rc == FFT3D_OK; ++d) {
                 int g = 0;
-                rc = prepare_kernel(kx->tma_fn[d == 0 ? TMA_X_FWD : TMA_X_INV], kx->tma_threads, kx->tma_smem_x, sms, &g);
+                rc = prepare_kernel(kx->tma_fn[d == 0 ? TMA_X_FWD : TMA_X_INV], kx->tma_threads_x, kx->tma_smem_x, sms, &g);
             }
         }
     }
@@ -413,7 +413,7 @@ int fft3d_r2c(const fft3d_plan_t* pl, const void* d_in, void* d_out, void* d_wor
         TmaArgs ta{};
         ta.tw = pl->tw_y; ta.ntz = (int)(M / ky->tma_tc); ta.ntiles = Nx * ta.ntz;
         ta.L = (int)L; ta.Nx = (int)Nx; ta.Mp1 = (int)(M + 1); ta.in_rows = pl->y_rows_nat; ta.out_rows = pl->y_rows_slab;
-        rc = launch_tma(ky->tma_fn[TMA_Y_FWD], ky, ky->tma_smem_y, pl->num_sms, mi, mi, mo, ta, st);
+        rc = launch_tma(ky->tma_fn[TMA_Y_FWD], ky->tma_threads, ky->tma_smem_y, pl->num_sms, mi, mi, mo, ta, st);
     } else {
         rc = launch(ky->s_fn[0][KIND_LIN_SLAB], a.ntiles, pl->grid_y[0], ky->s_threads, ky->s_smem, &a, st);
     }
@@ -431,7 +431,7 @@ int fft3d_r2c(const fft3d_plan_t* pl, const void* d_in, void* d_out, void* d_wor
     if (use_tma && pl->tma_x) {
         TensorMapBlob mi, mo;
         TensorMapBlob mi2;
-        const int tc = kx->tma_tc, of = kx->tma_oddfix;
+        const int tc = kx->tma_tc_x, of = kx->tma_oddfix;
         if (!map_slab_x(pl, &mi, d_work, tc, pl->x_rows) || !map_slab_x(pl, &mi2, d_work, tc + 2, pl->x_rows) ||
             !map_user_x(pl, &mo, d_out, tc, pl->x_rows)) return FFT3D_ECUDA;
         TmaArgs ta{};
@@ -439,7 +439,7 @@ int fft3d_r2c(const fft3d_plan_t* pl, const void* d_in, void* d_out, void* d_wor
         ta.tw = pl->tw_x; ta.ntz = (int)(M / tc);
         ta.ntiles = of ? (long long)p * (L / 2) * (2 * ta.ntz + 1) : (long long)p * L * ta.ntz;
         ta.L = (int)L; ta.Nx = (int)Nx; ta.Mp1 = (int)(M + 1); ta.in_rows = pl->x_rows; ta.out_rows = pl->x_rows;
-        rc = launch_tma(kx->tma_fn[TMA_X_FWD], kx, kx->tma_smem_x, pl->num_sms, mi, mi2, mo, ta, st);
+        rc = launch_tma(kx->tma_fn[TMA_X_FWD], kx->tma_threads_x, kx->tma_smem_x, pl->num_sms, mi, mi2, mo, ta, st);
     } else {
         rc = launch(kx->s_fn[0][KIND_LIN_LIN], b.ntiles, pl->grid_x[0], kx->s_threads, kx->s_smem, &b, st);
     }
@@ -488,14 +488,14 @@ int fft3d_c2r(const fft3d_plan_t* pl, const void* d_in, void* d_out, void* d_wor
     if (use_tma && pl->tma_x) {
         TensorMapBlob mi, mo;
         TensorMapBlob mi2;
-        const int tc = kx->tma_tc, of = kx->tma_oddfix;
+        const int tc = kx->tma_tc_x, of = kx->tma_oddfix;
         if (!map_user_x(pl, &mi, d_in, tc, pl->x_rows) || !map_user_x(pl, &mi2, d_in, tc + 2, pl->x_rows) ||
             !map_slab_x(pl, &mo, d_out, tc, pl->x_rows)) return FFT3D_ECUDA;
         TmaArgs ta{};
         ta.tw = pl->tw_x; ta.ntz = (int)(M / tc);
         ta.ntiles = of ? (long long)p * (L / 2) * (2 * ta.ntz) : (long long)p * L * ta.ntz;
         ta.L = (int)L; ta.Nx = (int)Nx; ta.Mp1 = (int)(M + 1); ta.in_rows = pl->x_rows; ta.out_rows = pl->x_rows;
-        rc = launch_tma(kx->tma_fn[TMA_X_INV], kx, kx->tma_smem_x, pl->num_sms, mi, mi2, mo, ta, st);
+        rc = launch_tma(kx->tma_fn[TMA_X_INV], kx->tma_threads_x, kx->tma_smem_x, pl->num_sms, mi, mi2, mo, ta, st);
         rec.mark(slot++);
         // packed column 0 of the result: x-transform of the side buffer, written over the (meaningless)
         // column the tiles produced from the user's raw kz = 0 plane
@@ -529,7 +529,7 @@ int fft3d_c2r(const fft3d_plan_t* pl, const void* d_in, void* d_out, void* d_wor
         TmaArgs ta{};
         ta.tw = pl->tw_y; ta.ntz = (int)(M / ky->tma_tc); ta.ntiles = Nx * ta.ntz;
         ta.L = (int)L; ta.Nx = (int)Nx; ta.Mp1 = (int)(M + 1); ta.in_rows = pl->y_rows_slab; ta.out_rows = pl->y_rows_nat;
-        rc = launch_tma(ky->tma_fn[TMA_Y_INV], ky, ky->tma_smem_y, pl->num_sms, mi, mi, mo, ta, st);
+        rc = launch_tma(ky->tma_fn[TMA_Y_INV], ky->tma_threads, ky->tma_smem_y, pl->num_sms, mi, mi, mo, ta, st);
     } else {
         rc = launch(ky->s_fn[1][KIND_SLAB_LIN], a.ntiles, pl->grid_y[1], ky->s_threads, ky->s_smem, &a, st);
     }

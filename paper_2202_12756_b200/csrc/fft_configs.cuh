@@ -27,7 +27,7 @@ FFT3D_CFG(float, 128, 16, 16, 8)
 FFT3D_CFG(float, 256, 16, 16, 16)
 FFT3D_CFG(float, 512, 16, 16, 16, 2)
 FFT3D_CFG(float, 1024, 32, 32, 32)
-FFT3D_CFG(float, 2048, 16, 16, 16, 8)
+FFT3D_CFG(float, 2048, 32, 32, 32, 2)
 FFT3D_CFG(float, 4096, 16, 16, 16, 16)
 FFT3D_CFG(float, 6, 6, 6)
 FFT3D_CFG(float, 12, 12, 12)

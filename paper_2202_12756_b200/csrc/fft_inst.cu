@@ -23,7 +23,8 @@ static KernelSet make_set(int dtype) {
     constexpr size_t TWB = (size_t)((Cfg::TWN + 1) & ~1) * sizeof(C);
     constexpr size_t S_SMEM = TWB + (size_t)TP::ROWS * TC * sizeof(C);
     constexpr int S_THREADS = Cfg::S * TC;
-    constexpr bool S_PF = FFT3D_PREFETCH;
+    // the second register set of the prefetching variant must fit the register file
+    constexpr bool S_PF = FFT3D_PREFETCH && (S_THREADS * (4 * Cfg::P * (int)sizeof(T) / 4 + 48) <= 65536);
     constexpr int S_MINB = S_PF ? 1 : min_blocks(S_THREADS, Cfg::P, (int)sizeof(T), S_SMEM);
     constexpr int RPB = rows_per_block(Cfg::S);
     constexpr size_t Z_SMEM = TWB + (size_t)Cfg::N * sizeof(C) + (size_t)RPB * RowPad<Cfg>::PITCH * sizeof(C);
@@ -57,19 +58,28 @@ static KernelSet make_set(int dtype) {
         // the X passes shift those tiles' windows (ODDFIX, see fft_kernels.cuh)
         constexpr bool OF = sizeof(C) % 16 != 0;
         using TY = TmaTile<Cfg, TTC, T, false>;
-        using TX = TmaTile<Cfg, TTC, T, OF>;
+        // X passes: same tile width (48-byte rows were tried to get a second ring stage back at
+        // N = 1536 where the shifted windows land TC+2 columns: rows that are not a multiple of the
+        // 32-byte sector cost 2.5x, measured)
+        constexpr int TTCX = TTC;
+        using TX = TmaTile<Cfg, TTCX, T, OF>;
         constexpr int NSY = TY::max_stages(), NSX = TX::max_stages();
-        if constexpr (NSY >= 2 && NSX >= 2) {
+        // one ring stage still works (load, transform, store in turn; the other SMs keep HBM busy)
+        if constexpr (NSY >= 1) {
             k.tma_fn[TMA_Y_FWD] = (const void*)fft_strided_tma_kernel<Cfg, TTC, TMA_Y_FWD, T, NSY, false>;
             k.tma_fn[TMA_Y_INV] = (const void*)fft_strided_tma_kernel<Cfg, TTC, TMA_Y_INV, T, NSY, false>;
-            k.tma_fn[TMA_X_FWD] = (const void*)fft_strided_tma_kernel<Cfg, TTC, TMA_X_FWD, T, NSX, OF>;
-            k.tma_fn[TMA_X_INV] = (const void*)fft_strided_tma_kernel<Cfg, TTC, TMA_X_INV, T, NSX, OF>;
-            k.tma_oddfix = OF ? 1 : 0;
-            k.tma_tc = TTC;
-            k.tma_threads = TY::NCONS + 32;
             k.tma_smem_y = (size_t)TY::smem_bytes(NSY);
+        }
+        if constexpr (NSX >= 1) {
+            k.tma_fn[TMA_X_FWD] = (const void*)fft_strided_tma_kernel<Cfg, TTCX, TMA_X_FWD, T, NSX, OF>;
+            k.tma_fn[TMA_X_INV] = (const void*)fft_strided_tma_kernel<Cfg, TTCX, TMA_X_INV, T, NSX, OF>;
             k.tma_smem_x = (size_t)TX::smem_bytes(NSX);
         }
+        k.tma_oddfix = OF ? 1 : 0;
+        k.tma_tc = TTC;
+        k.tma_threads = TY::NCONS + 32;
+        k.tma_tc_x = TTCX;
+        k.tma_threads_x = TX::NCONS + 32;
     }
     // bulk-pipelined z kernels: a row's S threads inside one warp, ~256 threads per 64 KiB tile
     using ZCfg = typename ZCfgFor<T, FFT3D_N>::type;

@@ -25,8 +25,10 @@ struct KernelSet {
     const void* z_fn[2];       // [0 = R2C, 1 = C2R]
     // TMA-pipelined strided kernels (null if not compiled for this length)
     const void* tma_fn[4];     // [TMA_Y_FWD, TMA_Y_INV, TMA_X_FWD, TMA_X_INV]
-    int tma_tc;                // tile columns
+    int tma_tc;                // tile columns of the Y passes
     int tma_threads;           // consumers + one producer warp
+    int tma_tc_x;              // tile columns / threads of the X passes (narrower when the shifted windows need room)
+    int tma_threads_x;
     int tma_oddfix;            // 1: the X passes shift the windows of odd-l rows (fp32, see fft_kernels.cuh)
     size_t tma_smem_y, tma_smem_x;
     // bulk-copy pipelined z kernels (null if not compiled for this length)
