@@ -83,7 +83,9 @@ int fft3d_plan(fft3d_plan_t **out, long long Nx, long long Ny, long long Nz,
 int fft3d_supported_length(long long n);
 
 /* Sizes in bytes.  Workspace: the single work buffer shared by R2C and C2R (opt. 1):
- * Nx*Ny*(Nz/2) complex.  Real: Nx*Ny*Nz reals.  Complex: Nx*Ny*(Nz/2+1) complex. */
+ * Nx*Ny*(Nz/2) complex, plus -- for plans whose z and y passes run fused -- a ring of a few
+ * yz-planes that lives in L2, one Nx*Ny complex side plane and 2*Nx counters (< 1 % more; the
+ * library zeroes the counters itself).  Real: Nx*Ny*Nz reals.  Complex: Nx*Ny*(Nz/2+1) complex. */
 size_t fft3d_workspace_bytes(const fft3d_plan_t *plan);
 size_t fft3d_real_bytes(const fft3d_plan_t *plan);
 size_t fft3d_complex_bytes(const fft3d_plan_t *plan);
@@ -94,13 +96,13 @@ size_t fft3d_complex_bytes(const fft3d_plan_t *plan);
 long long fft3d_index(const fft3d_plan_t *plan, long long kx, long long ky, long long kz);
 
 /* Forward R2C, Eq. (1): d_real_in [Nx][Ny][Nz] -> d_cplx_out in the slab layout above.
- * d_work: fft3d_workspace_bytes() bytes.  d_cplx_out is also used as scratch while the call
- * runs.  3 full-array kernel passes + one plane-sized fix-up kernel. */
+ * d_work: fft3d_workspace_bytes() bytes.  d_cplx_out may also be used as scratch while the call
+ * runs.  2 (fused z+y) or 3 full-array kernel passes + one plane-sized fix-up kernel. */
 int fft3d_r2c(const fft3d_plan_t *plan, const void *d_real_in, void *d_cplx_out,
               void *d_work, void *cuda_stream);
 
 /* Inverse C2R, Eq. (2)+(3) scaled by 1/(NxNyNz): d_cplx_in (slab layout) -> d_real_out
- * [Nx][Ny][Nz].  d_real_out is also used as scratch while the call runs. */
+ * [Nx][Ny][Nz].  d_real_out may also be used as scratch while the call runs. */
 int fft3d_c2r(const fft3d_plan_t *plan, const void *d_cplx_in, void *d_real_out,
               void *d_work, void *cuda_stream);
 
@@ -110,26 +112,37 @@ int fft3d_c2r(const fft3d_plan_t *plan, const void *d_cplx_in, void *d_real_out,
 int fft3d_r2c_host(fft3d_plan_t *plan, const void *h_real_in, void *h_cplx_out);
 int fft3d_c2r_host(fft3d_plan_t *plan, const void *h_cplx_in, void *h_real_out);
 
-/* Number of kernels one fft3d_r2c (which = 0) or fft3d_c2r (which = 1) call launches. */
+/* Number of kernels one fft3d_r2c (which = 0) or fft3d_c2r (which = 1) call launches, and the
+ * name of launch i (a static string; NULL if i is out of range).  Names: "z_r2c", "y_c2c_fwd",
+ * "x_c2c_fwd", "nyquist_unpack", "nyquist_pack", "x_c2c_inv", "x_c2c_inv_col0" (the packed
+ * column 0 of the inverse x pass, TMA path only), "y_c2c_inv", "z_c2r", and -- when the z and y
+ * passes of a plane run as one kernel through an L2-resident ring --
+ * "zy_r2c_fused" (paper step 1 + steps 2-4) and "yz_c2r_fused" (their reverse). */
 int fft3d_launches(const fft3d_plan_t *plan, int which);
+const char *fft3d_launch_name(const fft3d_plan_t *plan, int which, int i);
 
 /* Per-kernel timing for roofline reports.  After fft3d_timing_enable(plan, max_calls) every
  * fft3d_r2c / fft3d_c2r call on this plan records CUDA events between its kernel launches on the
  * caller's stream (until max_calls calls per direction have been recorded; later calls run
  * untimed).  fft3d_timing_read waits for the recorded events and returns, for direction
  * `which` (0 = r2c, 1 = c2r), the summed duration in ms of each launch slot over the recorded
- * calls (ms_sum[i], i < fft3d_launches(plan, which), in launch order: r2c = z-R2C, y-C2C,
- * x-C2C, Nyquist unpack; c2r = Nyquist pack, x-C2C, [x-C2C of the packed column 0, only when
- * fft3d_launches(plan, 1) == 5], y-C2C, z-C2R) and the number of calls,
- * then resets the counters.  max_calls = 0 disables timing.  Not thread-safe while enabled. */
+ * calls (ms_sum[i], i < fft3d_launches(plan, which), in launch order, named by
+ * fft3d_launch_name) and the number of calls, then resets the counters.  max_calls = 0 disables
+ * timing.  Not thread-safe while enabled. */
 #define FFT3D_MAX_LAUNCHES 8
 int fft3d_timing_enable(fft3d_plan_t *plan, int max_calls);
 int fft3d_timing_read(fft3d_plan_t *plan, int which, float *ms_sum, int *calls);
 
-/* Kernel selection for the strided (y, x) passes: variant 0 (default) = TMA-pipelined
- * persistent kernels wherever the extents and alignment allow, plain-load kernels elsewhere;
- * variant 1 = plain-load kernels everywhere (ablation / cross-check: both give bit-identical
- * results).  Returns FFT3D_EINVAL for an unknown variant; affects later calls on this plan. */
+/* Kernel selection.  variant 0 (default) = the fastest known path for the extents: z and y
+ * passes of each x-plane fused into one persistent kernel where that wins (cubic-like fp32
+ * plans of >= 2 GiB, Ny == Nz: four array passes per R2C+C2R pair) and TMA-pipelined passes
+ * elsewhere; variant 2 = the unfused TMA-pipelined passes (six array passes per pair);
+ * variant 3 = the fused z+y passes wherever they are compiled (any cubic-like plan with
+ * N >= 128); variant 1 = plain-load kernels everywhere (ablation / cross-check).  Variants 0-2
+ * without fusion give bit-identical results; the fused kernels run the same butterflies but are
+ * compiled separately, so they may differ in the last bit (FMA contraction) -- all variants meet
+ * the same error bound.  Returns FFT3D_EINVAL for an unknown variant; affects later calls on
+ * this plan.  The workspace size does not depend on the variant. */
 int fft3d_set_variant(fft3d_plan_t *plan, int variant);
 
 int fft3d_destroy(fft3d_plan_t *plan);          /* NULL is accepted */

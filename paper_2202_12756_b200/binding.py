@@ -18,7 +18,7 @@ LIB_PATH = os.path.join(_HERE, "libfft3d.so")
 EXPORTS = (
     "fft3d_plan", "fft3d_supported_length", "fft3d_workspace_bytes", "fft3d_real_bytes",
     "fft3d_complex_bytes", "fft3d_index", "fft3d_r2c", "fft3d_c2r", "fft3d_r2c_host",
-    "fft3d_c2r_host", "fft3d_launches", "fft3d_set_variant", "fft3d_destroy", "fft3d_strerror",
+    "fft3d_c2r_host", "fft3d_launches", "fft3d_launch_name", "fft3d_set_variant", "fft3d_destroy", "fft3d_strerror",
     "fft3d_timing_enable", "fft3d_timing_read",
 )
 
@@ -59,6 +59,8 @@ def load_library() -> ctypes.CDLL:
         getattr(lib, nm).restype = i
     lib.fft3d_launches.argtypes = [vp, i]
     lib.fft3d_launches.restype = i
+    lib.fft3d_launch_name.argtypes = [vp, i, i]
+    lib.fft3d_launch_name.restype = ctypes.c_char_p
     lib.fft3d_set_variant.argtypes = [vp, i]
     lib.fft3d_set_variant.restype = i
     lib.fft3d_timing_enable.argtypes = [vp, i]
@@ -128,8 +130,8 @@ class Plan:
         if rc != 0:
             raise Fft3dError(rc, "fft3d_set_variant")
 
-    LAUNCH_NAMES = (("z_r2c", "y_c2c_fwd", "x_c2c_fwd", "nyquist_unpack"),
-                    ("nyquist_pack", "x_c2c_inv", "y_c2c_inv", "z_c2r"))
+    def launch_names(self, which: int):
+        return tuple(self._lib.fft3d_launch_name(self._h, which, k).decode() for k in range(self.launches(which)))
 
     def timing_enable(self, max_calls: int):
         rc = self._lib.fft3d_timing_enable(self._h, int(max_calls))
@@ -143,10 +145,8 @@ class Plan:
         rc = self._lib.fft3d_timing_read(self._h, int(which), ms, ctypes.byref(calls))
         if rc != 0:
             raise Fft3dError(rc, "fft3d_timing_read")
-        n = self.launches(which)
-        names = self.LAUNCH_NAMES[which]
-        if which == 1 and n == 5:
-            names = ("nyquist_pack", "x_c2c_inv", "x_c2c_inv_col0", "y_c2c_inv", "z_c2r")
+        names = self.launch_names(which)
+        n = len(names)
         return {names[k]: float(ms[k]) for k in range(n)}, calls.value
 
     # ---- device entry points -------------------------------------------------------------

@@ -21,6 +21,7 @@
 #include "fft_configs.cuh"
 #include "fft_kernels.cuh"
 #include "fft_zpass.cuh"
+#include "fft_fused.cuh"
 #include "fft_registry.h"
 
 namespace fft3d {
@@ -75,6 +76,12 @@ struct fft3d_plan_s {
     bool tma_y, tma_x;         // usable for this plan's extents / alignment
     bool bulk_z;               // bulk-pipelined z kernels usable (row count a multiple of the tile)
     int y_rows_nat, y_rows_slab, x_rows;   // rows per TMA box
+    // fused z+y passes (fft_fused.cuh): the workspace is [slab array | ring | side | flags]
+    bool fused;                // fused kernels usable for this plan (variant 3 forces them)
+    bool fused_default;        // ... and expected to win (variant 0 uses them)
+    int fz_R;                  // ring depth (planes)
+    int fz_kz[2];              // [fwd, inv] SMs [0, kz) run the z tiles, the others the y tiles (0: split by CTA pairs)
+    size_t slab_bytes, ring_bytes, side_bytes, flags_bytes;
 };
 
 namespace {
@@ -242,6 +249,36 @@ int launch_zbulk(const fft3d_plan_s* pl, int d, const void* in, void* out, doubl
     return FFT3D_OK;
 }
 
+// F1+F2 (d = 0: real `in` -> slab array) or I2+I3 (d = 1: slab array -> real `out`) as one cooperative launch
+int launch_fused(const fft3d_plan_s* pl, int d, const void* in, void* out, void* slab, void* d_work, cudaStream_t st) {
+    const KernelSet* ky = pl->ky;
+    unsigned char* w = reinterpret_cast<unsigned char*>(d_work);
+    void* ring = w + pl->slab_bytes;
+    unsigned* flags = reinterpret_cast<unsigned*>(w + pl->slab_bytes + pl->ring_bytes + pl->side_bytes);
+    if (cudaMemsetAsync(flags, 0, pl->flags_bytes, st) != cudaSuccess) { cudaGetLastError(); return FFT3D_ECUDA; }
+    TensorMapBlob ring_map, slab_map;
+    {   // the ring as [R][Ny][M]
+        const long long sz = 2 * pl->esize, W = sz / 8;
+        long long dm[3] = {pl->M * W, pl->Ny, pl->fz_R}, sb[2] = {pl->M * sz, pl->Ny * pl->M * sz};
+        int bx[3] = {(int)(ky->fz_tc * W), pl->y_rows_nat, 1};
+        if (!make_map(pl, &ring_map, ring, 3, dm, sb, bx)) return FFT3D_ECUDA;
+    }
+    if (!map_slab_y(pl, &slab_map, slab, ky->fz_tc, pl->y_rows_slab)) return FFT3D_ECUDA;
+    FusedArgs a{};
+    a.in = in; a.out = out; a.ring = ring; a.tw_z = pl->tw_zb; a.twz = pl->twz; a.tw_y = pl->tw_y; a.flags = flags;
+    a.Nx = (int)pl->Nx; a.Ny = (int)pl->Ny; a.L = (int)pl->L; a.R = pl->fz_R; a.kz = pl->fz_kz[d];
+    a.rows_ring = pl->y_rows_nat; a.rows_slab = pl->y_rows_slab;
+    a.scale = 1.0 / ((double)pl->Nx * (double)pl->Ny * (double)pl->Nz);
+#ifdef FFT3D_TUNING
+    if (const char* e = getenv("FFT3D_FZ_KZ")) a.kz = atoi(e);
+#endif
+    void* argv[3] = {(void*)&ring_map, (void*)&slab_map, (void*)&a};
+    cudaError_t e = cudaLaunchCooperativeKernel(ky->fz_fn[d], dim3((unsigned)pl->num_sms), dim3((unsigned)ky->fz_threads),
+                                                argv, ky->fz_smem, st);
+    if (e != cudaSuccess) { cudaGetLastError(); return FFT3D_ECUDA; }
+    return FFT3D_OK;
+}
+
 // event slot `i` of the call being recorded for direction `which`, or no-op
 struct Recorder {
     TimingState* t;
@@ -343,13 +380,48 @@ int fft3d_plan(fft3d_plan_t** out, long long Nx, long long Ny, long long Nz, int
             rc = prepare_kernel(kz->zb_fn[d], kz->zb_threads, kz->zb_smem, sms, &g);
         }
     }
+    // fused z+y passes: cubic-like extents, whole tiles, a ring of >= 3 planes inside ~48 MB of L2,
+    // and a device that can hold one CTA per SM co-resident (cooperative launch)
+    pl->slab_bytes = (size_t)Nx * Ny * pl->M * 2 * pl->esize;
+    if (rc == FFT3D_OK && pl->tma_y && pl->bulk_z && ky->fz_fn[0] != nullptr && Nz == Ny && ky->fz_tc == ky->tma_tc &&
+        Ny % ky->fz_rpt == 0 && pl->M % ky->fz_tc == 0) {
+        const size_t plane = (size_t)Ny * pl->M * 2 * pl->esize;
+        int R = (int)(((size_t)48 << 20) / plane);
+        if (R > 8) R = 8;
+#ifdef FFT3D_TUNING
+        if (const char* e = getenv("FFT3D_FZ_R")) R = atoi(e);
+#endif
+        int coop = 0;
+        cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
+        if (R >= 2 && Nx >= R && coop) {
+            bool ok = true;
+            for (int d = 0; d < 2 && ok; ++d) {
+                int g = 0;
+                ok = prepare_kernel(ky->fz_fn[d], ky->fz_threads, ky->fz_smem, sms, &g) == FFT3D_OK && g >= sms;
+            }
+            if (ok) {
+                pl->fused = true; pl->fz_R = R;
+                // a z tile costs ~1.2x the instructions of a y tile: 54 % (forward; inverse 51 %, measured)
+                // of the SMs, rounded to whole TPCs
+                pl->fz_kz[0] = (int)(sms * 0.54 + 1.0) & ~1;
+                pl->fz_kz[1] = (int)(sms * 0.51 + 1.0) & ~1;
+                // measured on B200: the fused pass wins once the array is far larger than L2 and the CTA has
+                // two consumer groups on a 3-slot ring (fp32 1024^3: 2.64 vs 3.13 ms); below that the
+                // counters' latency and the single group (fp64: 2 slots) cost more than the HBM pass saved
+                pl->fused_default = ky->fz_ng >= 2 && ky->fz_nstage >= 3 && pl->slab_bytes >= ((size_t)2 << 30);
+                pl->ring_bytes = plane * R;
+                pl->side_bytes = ((size_t)Nx * Ny * 2 * pl->esize + 255) & ~(size_t)255;
+                pl->flags_bytes = ((size_t)2 * Nx * sizeof(unsigned) + 255) & ~(size_t)255;
+            }
+        }
+    }
     if (rc != FFT3D_OK) { fft3d_destroy(pl); return rc; }
     *out = pl;
     return FFT3D_OK;
 }
 
 size_t fft3d_workspace_bytes(const fft3d_plan_t* pl) {
-    return pl ? (size_t)pl->Nx * pl->Ny * pl->M * 2 * pl->esize : 0;
+    return pl ? pl->slab_bytes + pl->ring_bytes + pl->side_bytes + pl->flags_bytes : 0;
 }
 size_t fft3d_real_bytes(const fft3d_plan_t* pl) {
     return pl ? (size_t)pl->Nx * pl->Ny * pl->Nz * pl->esize : 0;
@@ -364,14 +436,42 @@ long long fft3d_index(const fft3d_plan_t* pl, long long kx, long long ky, long l
     return ((q * pl->Nx + kx) * pl->L + l) * (pl->M + 1) + kz;
 }
 
+static bool use_fused(const fft3d_plan_t* pl) {
+    return (pl->variant == 0 && pl->fused_default) || (pl->variant == 3 && pl->fused);
+}
+static bool use_tma(const fft3d_plan_t* pl) { return pl->variant != 1; }
+
 int fft3d_launches(const fft3d_plan_t* pl, int which) {
-    if (pl == nullptr) return 0;
+    if (pl == nullptr || which < 0 || which > 1) return 0;
     // c2r on the TMA path runs the packed column 0 of the x pass as a separate small kernel
-    return (which == 1 && pl->variant == 0 && pl->tma_x) ? 5 : 4;
+    int n = (which == 1 && use_tma(pl) && pl->tma_x) ? 5 : 4;
+    return use_fused(pl) ? n - 1 : n;
+}
+
+const char* fft3d_launch_name(const fft3d_plan_t* pl, int which, int i) {
+    if (pl == nullptr || i < 0 || i >= fft3d_launches(pl, which)) return nullptr;
+    const bool fz = use_fused(pl);
+    if (which == 0) {
+        static const char* const u[] = {"z_r2c", "y_c2c_fwd", "x_c2c_fwd", "nyquist_unpack"};
+        static const char* const f[] = {"zy_r2c_fused", "x_c2c_fwd", "nyquist_unpack"};
+        return fz ? f[i] : u[i];
+    }
+    const bool col0 = use_tma(pl) && pl->tma_x;
+    const char* seq[5];
+    int n = 0;
+    seq[n++] = "nyquist_pack";
+    seq[n++] = "x_c2c_inv";
+    if (col0) seq[n++] = "x_c2c_inv_col0";
+    if (fz) seq[n++] = "yz_c2r_fused";
+    else { seq[n++] = "y_c2c_inv"; seq[n++] = "z_c2r"; }
+    return seq[i];
 }
 
 int fft3d_set_variant(fft3d_plan_t* pl, int variant) {
-    if (pl == nullptr || variant < 0 || variant > 1) return FFT3D_EINVAL;   // 0 = TMA-pipelined where possible, 1 = plain-load kernels only
+    // 0 = the fastest known path (fused z+y passes where they win, TMA-pipelined passes elsewhere),
+    // 1 = plain-load kernels only, 2 = unfused TMA-pipelined passes (six array passes per pair),
+    // 3 = fused z+y passes wherever they are compiled
+    if (pl == nullptr || variant < 0 || variant > 3) return FFT3D_EINVAL;
     pl->variant = variant;
     return FFT3D_OK;
 }
@@ -386,16 +486,24 @@ int fft3d_r2c(const fft3d_plan_t* pl, const void* d_in, void* d_out, void* d_wor
     const long long Nx = pl->Nx, Ny = pl->Ny, M = pl->M, L = pl->L, p = pl->p;
 
     Recorder rec(pl, 0, st);
-    rec.mark(0);
+    int slot = 0;
+    rec.mark(slot++);
+    const bool tma_on = use_tma(pl), fz = use_fused(pl);
+    int rc;
+    if (fz) {
+        // F1+F2 fused: real -> (ring in L2) -> slab array in the workspace
+        rc = launch_fused(pl, 0, d_in, nullptr, d_work, d_work, st);
+        if (rc != FFT3D_OK) return rc;
+        rec.mark(slot++);
+    } else {
     // F1: real [Nx*Ny rows][Nz] -> packed complex [Nx][Ny][M] in d_out (scratch use)
     ZArgs z{};
     z.in = d_in; z.out = d_out; z.tw = pl->tw_z; z.twz = pl->twz; z.nrows = Nx * Ny; z.scale = 1.0;
     const KernelSet* kz = pl->kz;
-    int rc;
-    if (pl->variant == 0 && pl->bulk_z) rc = launch_zbulk(pl, 0, d_in, d_out, 1.0, st);
+    if (tma_on && pl->bulk_z) rc = launch_zbulk(pl, 0, d_in, d_out, 1.0, st);
     else rc = launch(kz->z_fn[0], (z.nrows + kz->z_rpb - 1) / kz->z_rpb, pl->grid_z[0], kz->z_threads, kz->z_smem, &z, st);
     if (rc != FFT3D_OK) return rc;
-    rec.mark(1);
+    rec.mark(slot++);
 
     // F2: y-axis FFT of d_out [x][y][M]; row ky goes to work[q][x][ky_l][M]  (steps 2-4 folded in)
     const KernelSet* ky = pl->ky;
@@ -405,8 +513,7 @@ int fft3d_r2c(const fft3d_plan_t* pl, const void* d_in, void* d_out, void* d_wor
     a.ntiles = Nx * a.ntz;
     a.in_hi = Ny * M; a.in_lo = 0; a.in_rq = 0; a.in_rl = M;
     a.out_hi = L * M; a.out_lo = 0; a.out_rq = Nx * L * M; a.out_rl = M;
-    const bool use_tma = pl->variant == 0;
-    if (use_tma && pl->tma_y) {
+    if (tma_on && pl->tma_y) {
         TensorMapBlob mi, mo;
         if (!map_natural(pl, &mi, d_out, ky->tma_tc, pl->y_rows_nat) ||
             !map_slab_y(pl, &mo, d_work, ky->tma_tc, pl->y_rows_slab)) return FFT3D_ECUDA;
@@ -418,7 +525,8 @@ int fft3d_r2c(const fft3d_plan_t* pl, const void* d_in, void* d_out, void* d_wor
         rc = launch(ky->s_fn[0][KIND_LIN_SLAB], a.ntiles, pl->grid_y[0], ky->s_threads, ky->s_smem, &a, st);
     }
     if (rc != FFT3D_OK) return rc;
-    rec.mark(2);
+    rec.mark(slot++);
+    }
 
     // F3: x-axis FFT per virtual slab q and row ky_l: work (pitch M) -> d_out (pitch M+1)
     const KernelSet* kx = pl->kx;
@@ -428,7 +536,7 @@ int fft3d_r2c(const fft3d_plan_t* pl, const void* d_in, void* d_out, void* d_wor
     b.ntiles = (long long)p * L * b.ntz;
     b.in_hi = Nx * L * M; b.in_lo = M; b.in_rq = 0; b.in_rl = L * M;
     b.out_hi = Nx * L * (M + 1); b.out_lo = M + 1; b.out_rq = 0; b.out_rl = L * (M + 1);
-    if (use_tma && pl->tma_x) {
+    if (tma_on && pl->tma_x) {
         TensorMapBlob mi, mo;
         TensorMapBlob mi2;
         const int tc = kx->tma_tc_x, of = kx->tma_oddfix;
@@ -444,13 +552,13 @@ int fft3d_r2c(const fft3d_plan_t* pl, const void* d_in, void* d_out, void* d_wor
         rc = launch(kx->s_fn[0][KIND_LIN_LIN], b.ntiles, pl->grid_x[0], kx->s_threads, kx->s_smem, &b, st);
     }
     if (rc != FFT3D_OK) return rc;
-    rec.mark(3);
+    rec.mark(slot++);
 
     // column 0 holds A + iB (planes kz = 0 and kz = Nz/2): separate them in place
     PlaneArgs f{};
     f.src = nullptr; f.dst = d_out; f.Nx = (int)Nx; f.Ny = (int)Ny; f.L = (int)L; f.M = (int)M;
     if (launch_unpack_nyquist(pl->dtype, f, st) != cudaSuccess) { cudaGetLastError(); return FFT3D_ECUDA; }
-    rec.mark(4);
+    rec.mark(slot++);
     return FFT3D_OK;
 }
 
@@ -469,28 +577,32 @@ int fft3d_c2r(const fft3d_plan_t* pl, const void* d_in, void* d_out, void* d_wor
     Recorder rec(pl, 1, st);
     int slot = 0;
     rec.mark(slot++);
+    const bool tma_on = use_tma(pl), fz = use_fused(pl);
+    // fused: I1 writes the slab array in the workspace and I2+I3 go from there to d_out, so the side
+    // buffer sits behind the ring; unfused: I1 -> d_out (scratch) -> I2 -> workspace -> I3 -> d_out
+    void* side = fz ? (void*)(reinterpret_cast<unsigned char*>(d_work) + pl->slab_bytes + pl->ring_bytes) : d_work;
+    void* x_out = fz ? d_work : d_out;
     PlaneArgs f{};
-    f.src = d_in; f.dst = d_work; f.Nx = (int)Nx; f.Ny = (int)Ny; f.L = (int)L; f.M = (int)M;
+    f.src = d_in; f.dst = side; f.Nx = (int)Nx; f.Ny = (int)Ny; f.L = (int)L; f.M = (int)M;
     if (launch_pack_nyquist(pl->dtype, f, st) != cudaSuccess) { cudaGetLastError(); return FFT3D_ECUDA; }
     rec.mark(slot++);
 
     // I1: x-axis inverse FFT: d_in (pitch M+1, column 0 from the side buffer) -> d_out scratch (pitch M)
     const KernelSet* kx = pl->kx;
     StridedArgs b{};
-    b.in = d_in; b.out = d_out; b.col0 = d_work; b.tw = pl->tw_x;
+    b.in = d_in; b.out = x_out; b.col0 = side; b.tw = pl->tw_x;
     b.ntz = (int)((M + kx->tc - 1) / kx->tc); b.ncols = (int)M; b.a_lo = (int)L; b.L = (int)Nx;
     b.ntiles = (long long)p * L * b.ntz;
     b.in_hi = Nx * L * (M + 1); b.in_lo = M + 1; b.in_rq = 0; b.in_rl = L * (M + 1);
     b.c0_hi = Nx * L; b.c0_lo = 1; b.c0_rl = L;
     b.out_hi = Nx * L * M; b.out_lo = M; b.out_rq = 0; b.out_rl = L * M;
-    const bool use_tma = pl->variant == 0;
     int rc;
-    if (use_tma && pl->tma_x) {
+    if (tma_on && pl->tma_x) {
         TensorMapBlob mi, mo;
         TensorMapBlob mi2;
         const int tc = kx->tma_tc_x, of = kx->tma_oddfix;
         if (!map_user_x(pl, &mi, d_in, tc, pl->x_rows) || !map_user_x(pl, &mi2, d_in, tc + 2, pl->x_rows) ||
-            !map_slab_x(pl, &mo, d_out, tc, pl->x_rows)) return FFT3D_ECUDA;
+            !map_slab_x(pl, &mo, x_out, tc, pl->x_rows)) return FFT3D_ECUDA;
         TmaArgs ta{};
         ta.tw = pl->tw_x; ta.ntz = (int)(M / tc);
         ta.ntiles = of ? (long long)p * (L / 2) * (2 * ta.ntz) : (long long)p * L * ta.ntz;
@@ -501,7 +613,7 @@ int fft3d_c2r(const fft3d_plan_t* pl, const void* d_in, void* d_out, void* d_wor
         // column the tiles produced from the user's raw kz = 0 plane
         if (rc == FFT3D_OK) {
             StridedArgs c0{};
-            c0.in = d_work; c0.out = d_out; c0.col0 = nullptr; c0.tw = pl->tw_x;
+            c0.in = side; c0.out = x_out; c0.col0 = nullptr; c0.tw = pl->tw_x;
             c0.ntz = (int)((L + kx->tc - 1) / kx->tc); c0.ncols = (int)L; c0.a_lo = 1; c0.L = (int)Nx;
             c0.ntiles = (long long)p * c0.ntz;
             c0.in_hi = Nx * L; c0.in_lo = 0; c0.in_rq = 0; c0.in_rl = L;
@@ -514,6 +626,13 @@ int fft3d_c2r(const fft3d_plan_t* pl, const void* d_in, void* d_out, void* d_wor
     if (rc != FFT3D_OK) return rc;
     rec.mark(slot++);
 
+    if (fz) {
+        // I2+I3 fused: slab array -> (ring in L2) -> real output, normalisation included
+        rc = launch_fused(pl, 1, nullptr, d_out, d_work, d_work, st);
+        rec.mark(slot++);
+        return rc;
+    }
+
     // I2: y-axis inverse FFT gathering rows from the slab layout: d_out scratch -> work [x][y][M]
     const KernelSet* ky = pl->ky;
     StridedArgs a{};
@@ -522,7 +641,7 @@ int fft3d_c2r(const fft3d_plan_t* pl, const void* d_in, void* d_out, void* d_wor
     a.ntiles = Nx * a.ntz;
     a.in_hi = L * M; a.in_lo = 0; a.in_rq = Nx * L * M; a.in_rl = M;
     a.out_hi = Ny * M; a.out_lo = 0; a.out_rq = 0; a.out_rl = M;
-    if (use_tma && pl->tma_y) {
+    if (tma_on && pl->tma_y) {
         TensorMapBlob mi, mo;
         if (!map_slab_y(pl, &mi, d_out, ky->tma_tc, pl->y_rows_slab) ||
             !map_natural(pl, &mo, d_work, ky->tma_tc, pl->y_rows_nat)) return FFT3D_ECUDA;
@@ -541,7 +660,7 @@ int fft3d_c2r(const fft3d_plan_t* pl, const void* d_in, void* d_out, void* d_wor
     ZArgs z{};
     z.in = d_work; z.out = d_out; z.tw = pl->tw_z; z.twz = pl->twz; z.nrows = Nx * Ny;
     z.scale = 1.0 / ((double)Nx * (double)Ny * (double)Nz);
-    if (use_tma && pl->bulk_z) rc = launch_zbulk(pl, 1, d_work, d_out, z.scale, st);
+    if (tma_on && pl->bulk_z) rc = launch_zbulk(pl, 1, d_work, d_out, z.scale, st);
     else rc = launch(kz->z_fn[1], (z.nrows + kz->z_rpb - 1) / kz->z_rpb, pl->grid_z[1], kz->z_threads, kz->z_smem, &z, st);
     rec.mark(slot++);
     return rc;

@@ -1,0 +1,408 @@
+// fft_fused.cuh -- the z and y passes of one x-plane fused into ONE kernel, the plane's
+// intermediate exchanged through a small L2-resident ring instead of a full HBM round trip
+// (SURVEY.md 8(f)-2):
+//
+//   fft_zy_fused_kernel<DIR = -1>   passes F1+F2: z-axis R2C of the rows of plane x (paper step 1,
+//                                   z half) -> ring -> y-axis C2C with each row ky written to
+//                                   its slab address (step 1 y half + steps 2-4)
+//   fft_zy_fused_kernel<DIR = +1>   passes I2+I3: the mirror image, 1/(NxNyNz) fused
+//
+// A 2-D FFT of a yz-plane needs a full transpose of the plane between its two 1-D stages, and a
+// plane (4 MiB at 1024^2 fp32) does not fit one SM's -- or one cluster's -- shared memory.  It
+// does fit the 126 MB L2 many times over.  So the kernel is a persistent dataflow pipeline over
+// ALL SMs, one CTA per SM, each CTA with a fixed ROLE: "z CTAs" transform z tiles (RPT whole rows),
+// "y CTAs" transform y tiles (TC columns of a plane).  Planes are handled in order; the tiles of a
+// role are dealt round-robin to the CTAs of that role.  The "phase-1" role (forward: z, inverse: y)
+// writes its result into ring slot x % R ([R][Ny][M] complex), the "phase-2" role reads it from
+// there as soon as the plane is complete -- so the ring lives in L2 (written with an evict_last
+// policy; the streaming input and output use evict_first) and HBM sees ONE read and ONE write of
+// the array for the two passes together.
+//
+// Why roles: the two tile bodies are ~35 KB of straight-line code each and the two SMs of a TPC
+// share an instruction cache; with both bodies alive in one TPC 60 % of the issue stalls in the
+// FFT code were instruction fetches (ncu, profiles/).  Roles follow %smid so that a TPC never mixes.
+//
+// Ordering between CTAs uses two counters per plane in global memory (zeroed before the launch):
+//   p1_done[x]    += 1 when a phase-1 tile of plane x has been stored (store complete, released at once)
+//   p2_loaded[x]  += 1 when a phase-2 tile of plane x has landed in shared memory
+// A phase-2 load of plane x waits for p1_done[x] == N1; a phase-1 store of plane x waits for
+// p2_loaded[x-R] == N2 (the ring slot has been read out).  Phase-2 CTAs never wait on anything a
+// later plane produces and phase-1 CTAs only on phase-2 loads R planes back, every CTA handles its
+// tiles in plane order, so with all CTAs co-resident (cooperative launch, one CTA per SM) the
+// pipeline cannot deadlock.
+//
+// Inside a CTA: a load warp, one store warp per ring slot (one elected lane each) and NG consumer groups
+// that own alternate tiles and transform them IN PLACE in an NSTAGE-deep shared-memory ring, with
+// exactly the z-tile and y-tile code of fft_zpass.cuh / fft_kernels.cuh.
+#pragma once
+#include <cstdint>
+#include <cstdio>
+
+#include "fft_core.cuh"
+#include "fft_kernels.cuh"
+#include "fft_zpass.cuh"
+
+namespace fft3d {
+
+struct FusedArgs {
+    const void* in;          // forward: the real input; inverse: unused (slab read through its tensor map)
+    void* out;               // inverse: the real output; forward: unused (slab written through its tensor map)
+    void* ring;              // [R][Ny][M] complex
+    const void* tw_z;        // stage twiddles of the M-point FFT (forward)
+    const void* twz;         // exp(-2 pi i k / Nz), k < M
+    const void* tw_y;        // stage twiddles of the Ny-point FFT (forward)
+    unsigned* flags;         // [2][Nx]: p1_done, p2_loaded
+    int Nx, Ny, L;           // L = Ny / virtual_slabs
+    int R;                   // ring planes
+    int rows_ring, rows_slab;   // rows per TMA box on the ring side / the slab side of a y tile
+    double scale;            // inverse: 1/(Nx Ny Nz)
+    int kz;                  // SMs [0, kz) take the z tiles (0: split by CTA pairs)
+};
+
+namespace tma {
+__device__ __forceinline__ unsigned long long policy_evict_first() {
+    unsigned long long p;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+__device__ __forceinline__ unsigned long long policy_evict_last() {
+    unsigned long long p;
+    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+__device__ __forceinline__ void bulk_load_h(void* dst, const void* src, unsigned bytes, unsigned long long* bar,
+                                            unsigned long long pol) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;"
+                 ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)), "l"(pol) : "memory");
+}
+__device__ __forceinline__ void bulk_store_h(void* dst, const void* src, unsigned bytes, unsigned long long pol) {
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group.L2::cache_hint [%0], [%1], %2, %3;"
+                 ::"l"(dst), "r"(smem_u32(src)), "r"(bytes), "l"(pol) : "memory");
+}
+__device__ __forceinline__ void load3_h(void* dst, const void* map, unsigned long long* bar, int c0, int c1, int c2,
+                                        unsigned long long pol) {
+    asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1, {%3, %4, %5}], [%2], %6;"
+                 ::"r"(smem_u32(dst)), "l"(map), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2), "l"(pol) : "memory");
+}
+__device__ __forceinline__ void load4_h(void* dst, const void* map, unsigned long long* bar, int c0, int c1, int c2, int c3,
+                                        unsigned long long pol) {
+    asm volatile("cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1, {%3, %4, %5, %6}], [%2], %7;"
+                 ::"r"(smem_u32(dst)), "l"(map), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "l"(pol) : "memory");
+}
+__device__ __forceinline__ void store3_h(const void* map, const void* src, int c0, int c1, int c2, unsigned long long pol) {
+    asm volatile("cp.async.bulk.tensor.3d.global.shared::cta.bulk_group.L2::cache_hint [%0, {%2, %3, %4}], [%1], %5;"
+                 ::"l"(map), "r"(smem_u32(src)), "r"(c0), "r"(c1), "r"(c2), "l"(pol) : "memory");
+}
+__device__ __forceinline__ void store4_h(const void* map, const void* src, int c0, int c1, int c2, int c3,
+                                         unsigned long long pol) {
+    asm volatile("cp.async.bulk.tensor.4d.global.shared::cta.bulk_group.L2::cache_hint [%0, {%2, %3, %4, %5}], [%1], %6;"
+                 ::"l"(map), "r"(smem_u32(src)), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "l"(pol) : "memory");
+}
+__device__ __forceinline__ void fence_proxy_async_all() { asm volatile("fence.proxy.async;" ::: "memory"); }
+__device__ __forceinline__ unsigned ld_acquire(const unsigned* p) {
+    unsigned v;
+    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void red_release_add(unsigned* p, unsigned v) {
+    asm volatile("red.release.gpu.global.add.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+__device__ __forceinline__ void wait_count(const unsigned* p, unsigned target) {
+#ifdef FFT3D_WATCHDOG
+    long long t0 = clock64();
+    while (ld_acquire(p) < target) {
+        __nanosleep(64);
+        if (clock64() - t0 > 4000000000LL) { printf("wait_count stuck: blk %d tid %d have %u want %u\n", blockIdx.x, threadIdx.x, ld_acquire(p), target); __trap(); }
+    }
+#else
+    while (ld_acquire(p) < target) __nanosleep(64);
+#endif
+}
+// mbarrier wait with a watchdog (debug builds)
+__device__ __forceinline__ void mbar_wait_dbg(unsigned long long* bar, unsigned parity, int what) {
+#ifdef FFT3D_WATCHDOG
+    long long t0 = clock64();
+    unsigned ok = 0;
+    while (!ok) {
+        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                     : "=r"(ok) : "r"(smem_u32(bar)), "r"(parity) : "memory");
+        if (!ok && clock64() - t0 > 4000000000LL) { printf("mbar stuck: what %d blk %d tid %d parity %u\n", what, blockIdx.x, threadIdx.x, parity); __trap(); }
+    }
+#else
+    mbar_wait(bar, parity);
+#endif
+}
+}  // namespace tma
+
+template <class ZCfg, int RPT, class YCfg, int TC, typename T, int NG_ = 2>
+struct FusedTile {
+    using C = cx<T>;
+    using ZT = ZTile<ZCfg, RPT, T>;
+    using YT = TmaTile<YCfg, TC, T, false>;
+    static constexpr int GROUP = ZT::GROUP;                     // consumer threads per group
+    static constexpr bool OK = (ZT::GROUP == YT::NCONS) && (ZT::GROUP % 32 == 0);
+    static constexpr int NG = NG_;
+    static constexpr int STAGE_BYTES = ZT::STAGE_BYTES > YT::STAGE_BYTES ? ZT::STAGE_BYTES : YT::STAGE_BYTES;
+    static constexpr int TWZ_BYTES = ZT::TW_BYTES, TWY_BYTES = YT::TW_BYTES;
+    static constexpr int FIXED = TWZ_BYTES + TWY_BYTES + NG * ZT::SCRATCH_BYTES + 256;
+    // + one load warp + one store warp per ring slot (each store thread blocks on ITS tile's completion only)
+    __host__ __device__ static constexpr int threads(int nstage) { return NG * GROUP + 32 * (1 + nstage); }
+    __host__ __device__ static constexpr int smem_bytes(int nstage) { return FIXED + nstage * STAGE_BYTES; }
+    __host__ __device__ static constexpr int max_stages() {
+        int n = (227 * 1024 - FIXED) / STAGE_BYTES;
+        return n > 4 ? 4 : n;
+    }
+    static constexpr int THREADS = threads(max_stages());
+};
+
+struct FItem { int p1, x, j; };
+
+template <class ZCfg, int RPT, class YCfg, int TC, int DIR, typename T, int NSTAGE, int NG_>
+__global__ void __launch_bounds__((FusedTile<ZCfg, RPT, YCfg, TC, T, NG_>::THREADS), 1)
+fft_zy_fused_kernel(const __grid_constant__ TensorMapBlob ring_map, const __grid_constant__ TensorMapBlob slab_map,
+                    const FusedArgs a) {
+    using C = cx<T>;
+    using FT = FusedTile<ZCfg, RPT, YCfg, TC, T, NG_>;
+    using ZT = typename FT::ZT;
+    using YT = typename FT::YT;
+    constexpr int GROUP = FT::GROUP, NG = FT::NG, NCONS = NG * GROUP, W = YT::W;
+    constexpr int M = ZCfg::N, NY = YCfg::N;
+    constexpr bool FWD = DIR < 0;
+    static_assert(FT::OK, "z tile and y tile must use the same number of consumer threads");
+    static_assert(ZCfg::S <= 32 && (ZCfg::S & (ZCfg::S - 1)) == 0, "a row's threads must sit inside one warp");
+
+    extern __shared__ __align__(1024) unsigned char smem_dyn[];
+    C* twz_s = reinterpret_cast<C*>(smem_dyn);                                   // z stage twiddles
+    C* twy_s = reinterpret_cast<C*>(smem_dyn + FT::TWZ_BYTES);                   // y stage twiddles
+    unsigned char* stages = smem_dyn + FT::TWZ_BYTES + FT::TWY_BYTES;
+    C* scratch = reinterpret_cast<C*>(stages + NSTAGE * FT::STAGE_BYTES);
+    unsigned long long* full = reinterpret_cast<unsigned long long*>(reinterpret_cast<unsigned char*>(scratch) + NG * ZT::SCRATCH_BYTES);
+    unsigned long long* done = full + NSTAGE;            // consumers -> store warp: tile transformed
+    unsigned long long* empty = done + NSTAGE;           // store warp -> load warp: slot read out
+    // seen[s] = number of phases of full[s] a consumer group has observed complete.  A slot is used by
+    // the groups in turn (NSTAGE need not be a multiple of NG) and a parity wait is only meaningful
+    // within one phase of the barrier's current one, so a group polls seen[s] before it waits for ITS phase.
+    volatile int* seen = reinterpret_cast<volatile int*>(empty + NSTAGE);
+
+    const int tid = threadIdx.x;
+    if (tid == NCONS) {
+        for (int s = 0; s < NSTAGE; ++s) {
+            tma::mbar_init(&full[s], 1); tma::mbar_init(&done[s], GROUP / 32); tma::mbar_init(&empty[s], 1);
+            seen[s] = 0;
+        }
+        tma::fence_mbar_init();
+    }
+    if (tid < NCONS) {
+        load_twiddles<DIR, T>(twz_s, reinterpret_cast<const C*>(a.tw_z), ZCfg::TWN, tid, NCONS);
+        load_twiddles<DIR, T>(twy_s, reinterpret_cast<const C*>(a.tw_y), YCfg::TWN, tid, NCONS);
+    }
+    __syncthreads();
+
+    const int n_z = a.Ny / RPT, n_y = M / TC;            // z tiles / y tiles per plane
+    const int n1 = FWD ? n_z : n_y, n2 = FWD ? n_y : n_z;
+    // Role of this CTA: z tiles or y tiles, never both -- the two bodies are ~35 KB of straight-line
+    // code each, and the SMs of a TPC share an instruction cache, so both SMs of a TPC get the same role.
+    //   kz > 0 and one CTA per SM (grid == %nsmid): SMs [0, kz) take the z tiles, the rest the y tiles
+    //   otherwise: CTA pairs (4k, 4k+1) -> z, (4k+2, 4k+3) -> y
+    unsigned smid, nsmid;
+    asm("mov.u32 %0, %%smid;" : "=r"(smid));
+    asm("mov.u32 %0, %%nsmid;" : "=r"(nsmid));
+    int role_z, rank, nrole;
+    if (a.kz > 0 && nsmid == gridDim.x && a.kz < (int)gridDim.x) {
+        role_z = (int)smid < a.kz;
+        rank = role_z ? (int)smid : (int)smid - a.kz;
+        nrole = role_z ? a.kz : (int)gridDim.x - a.kz;
+    } else {
+        const int b = blockIdx.x, g4 = gridDim.x / 4 * 4;
+        if (b < g4) { role_z = !((b >> 1) & 1); rank = ((b >> 2) << 1) | (b & 1); nrole = g4 / 2; }
+        else { role_z = !(b & 1); rank = g4 / 2 + ((b - g4) >> 1); nrole = g4 / 2; }
+        nrole += role_z ? ((int)gridDim.x - g4 + 1) / 2 : ((int)gridDim.x - g4) / 2;
+    }
+    const int my_p1 = FWD ? role_z : !role_z;            // this CTA's tiles are the phase-1 tiles
+    const int nper = role_z ? n_z : n_y;                 // tiles per plane of this role
+    const int total = a.Nx * nper;
+    unsigned* p1_done = a.flags;
+    unsigned* p2_loaded = a.flags + a.Nx;
+    const long long plane_bytes = (long long)a.Ny * M * (long long)sizeof(C);
+
+    if (tid >= NCONS) {
+        if (tid == NCONS) {
+            // ------------------------- load warp -------------------------
+            const unsigned long long pol_stream = tma::policy_evict_first(), pol_keep = tma::policy_evict_last();
+            int i = 0, ready = -1;                       // planes <= ready are known to be complete in the ring
+            for (int g = rank; g < total; g += nrole) {
+                FItem it; it.p1 = my_p1; it.x = g / nper; it.j = g - it.x * nper;
+                const int s = i % NSTAGE, n = i / NSTAGE;
+                unsigned char* dst = stages + s * FT::STAGE_BYTES;
+                if (n > 0) tma::mbar_wait_dbg(&empty[s], (unsigned)((n - 1) & 1), 0);
+                if (!it.p1 && it.x > ready) {
+                    tma::wait_count(&p1_done[it.x], (unsigned)n1);
+                    tma::fence_proxy_async_all();
+                    ready = it.x;
+                }
+                const bool isz = FWD ? it.p1 : !it.p1;
+                if (isz) {
+                    // forward: rows of the real input (HBM stream); inverse: rows of the ring
+                    const unsigned char* src = FWD
+                        ? reinterpret_cast<const unsigned char*>(a.in) + (long long)it.x * plane_bytes
+                        : reinterpret_cast<const unsigned char*>(a.ring) + (long long)(it.x % a.R) * plane_bytes;
+                    src += (long long)it.j * ZT::TILE_BYTES;
+                    const unsigned long long pol = FWD ? pol_stream : pol_keep;
+                    constexpr int CHUNK = 16384;
+                    tma::mbar_expect_tx(&full[s], ZT::TILE_BYTES);
+                    for (int o = 0; o < ZT::TILE_BYTES; o += CHUNK)
+                        tma::bulk_load_h(dst + o, src + o, ZT::TILE_BYTES - o < CHUNK ? ZT::TILE_BYTES - o : CHUNK, &full[s], pol);
+                } else {
+                    tma::mbar_expect_tx(&full[s], YT::TILE_BYTES);
+                    if constexpr (FWD) {                 // columns of the ring plane
+                        const int nb = NY / a.rows_ring;
+                        for (int b = 0; b < nb; ++b)
+                            tma::load3_h(dst + (size_t)b * a.rows_ring * YT::ROW_BYTES, &ring_map, &full[s],
+                                         it.j * TC * W, b * a.rows_ring, it.x % a.R, pol_keep);
+                    } else {                             // columns of plane x gathered from the slab layout
+                        const int nb = NY / a.rows_slab;
+                        for (int b = 0; b < nb; ++b) {
+                            const int r0 = b * a.rows_slab;
+                            tma::load4_h(dst + (size_t)b * a.rows_slab * YT::ROW_BYTES, &slab_map, &full[s],
+                                         it.j * TC * W, r0 % a.L, it.x, r0 / a.L, pol_stream);
+                        }
+                    }
+                }
+                ++i;
+            }
+        } else if ((tid & 31) == 0) {
+            // ------------------------- store warp of ring slot my_s -------------------------
+            const int my_s = (tid - NCONS) / 32 - 1;
+            const unsigned long long pol_stream = tma::policy_evict_first(), pol_keep = tma::policy_evict_last();
+            int i = 0, freed = -1;
+            for (int g = rank; g < total; g += nrole) {
+                FItem it; it.p1 = my_p1; it.x = g / nper; it.j = g - it.x * nper;
+                const int s = i % NSTAGE, n = i / NSTAGE;
+                if (s != my_s) { ++i; continue; }
+                const unsigned char* src = stages + s * FT::STAGE_BYTES;
+                tma::mbar_wait_dbg(&done[s], (unsigned)(n & 1), 1);
+                if (it.p1 && it.x >= a.R && it.x - a.R > freed) {          // ring slot must have been read out
+                    tma::wait_count(&p2_loaded[it.x - a.R], (unsigned)n2);
+                    freed = it.x - a.R;
+                }
+                const bool isz = FWD ? it.p1 : !it.p1;
+                if (isz) {
+                    unsigned char* dst = FWD
+                        ? reinterpret_cast<unsigned char*>(a.ring) + (long long)(it.x % a.R) * plane_bytes
+                        : reinterpret_cast<unsigned char*>(a.out) + (long long)it.x * plane_bytes;
+                    dst += (long long)it.j * ZT::TILE_BYTES;
+                    const unsigned long long pol = FWD ? pol_keep : pol_stream;
+                    constexpr int CHUNK = 16384;
+                    for (int o = 0; o < ZT::TILE_BYTES; o += CHUNK)
+                        tma::bulk_store_h(dst + o, src + o, ZT::TILE_BYTES - o < CHUNK ? ZT::TILE_BYTES - o : CHUNK, pol);
+                } else {
+                    if constexpr (FWD) {                 // rows go to their slab addresses (steps 2-4 as addressing)
+                        const int nb = NY / a.rows_slab;
+                        for (int b = 0; b < nb; ++b) {
+                            const int r0 = b * a.rows_slab;
+                            tma::store4_h(&slab_map, src + (size_t)b * a.rows_slab * YT::ROW_BYTES,
+                                          it.j * TC * W, r0 % a.L, it.x, r0 / a.L, pol_stream);
+                        }
+                    } else {
+                        const int nb = NY / a.rows_ring;
+                        for (int b = 0; b < nb; ++b)
+                            tma::store3_h(&ring_map, src + (size_t)b * a.rows_ring * YT::ROW_BYTES,
+                                          it.j * TC * W, b * a.rows_ring, it.x % a.R, pol_keep);
+                    }
+                }
+                tma::store_commit();
+                tma::store_wait_read0();                 // slot s has been read out
+                tma::mbar_arrive(&empty[s]);
+                if (it.p1) {
+                    // publish at once: a deferred release would make this plane's readers depend on a LATER
+                    // item of this CTA, and with the ring's back-pressure that closes a cycle
+                    tma::store_wait_all();
+                    tma::fence_proxy_async_all();
+                    tma::red_release_add(&p1_done[it.x], 1u);
+                }
+                ++i;
+            }
+            tma::store_wait_all();
+        }
+        return;
+    }
+
+    // ---------------- consumers: group gq takes the CTA's items gq, gq+NG, ... ----------------
+    const int gq = tid / GROUP, gt = tid % GROUP;
+    const GroupSync sync{1 + gq, GROUP};
+    // z-tile role: thread tz of row rr
+    const int tz = gt % ZCfg::S, rr = gt / ZCfg::S;
+    const SmLayout<1, 0> z_dense{rr * M};
+    const SmLayout<1, ZT::PADR> z_padded{rr * ZT::PITCH};
+    C* scr = scratch + gq * (RPT * ZCfg::P) + rr * ZCfg::P;
+    C wt = reinterpret_cast<const C*>(a.twz)[tz];        // exp(-2 pi i t/Nz), conjugated for the inverse
+    if constexpr (DIR > 0) wt.y = -wt.y;
+    const T scale = (T)a.scale;
+    // y-tile role: thread ty of column cc
+    const int cc = gt % TC, ty = gt / TC;
+    const SmLayout<TC, 0> y_dense{cc};
+    const SmLayout<TC, YT::PADR> y_padded{cc};
+
+    int i = 0;
+    for (int g = rank; g < total; g += nrole) {
+        FItem it; it.p1 = my_p1; it.x = g / nper; it.j = g - it.x * nper;
+        const int mine = (i % NG) == gq;
+        const int s = i % NSTAGE, n = i / NSTAGE;
+        ++i;
+        if (!mine) continue;
+        C* buf = reinterpret_cast<C*>(stages + s * FT::STAGE_BYTES);
+        while (seen[s] < n) { }                          // the previous phase of this slot has been observed
+        tma::mbar_wait_dbg(&full[s], (unsigned)(n & 1), 2);
+        if (gt == 0) seen[s] = n + 1;
+        if (!it.p1 && gt == 0) tma::red_release_add(&p2_loaded[it.x], 1u);   // the ring tile has been read
+        const bool isz = FWD ? it.p1 : !it.p1;
+#ifdef FFT3D_COPY_ONLY_FUSED   // experiment: data movement without the transforms (wrong results by design)
+        tma::fence_proxy_async(); __syncwarp();
+        if ((tid & 31) == 0) tma::mbar_arrive(&done[s]);
+        continue;
+#endif
+        if (isz) {
+            constexpr int P = ZCfg::P;
+            C v[P];
+            read_own<ZCfg, T>(v, buf, tz, z_dense);
+            if constexpr (DIR > 0) {
+                if (tz == 0) {
+#pragma unroll
+                    for (int m = 0; m < P; ++m) scr[m] = v[m];
+                }
+                __syncwarp();
+                hermitian_step<ZCfg, true, T>(v, wt, tz, scr);
+                __syncwarp();
+            }
+            if constexpr (ZCfg::NST > 1) sync();
+            fft_stages<ZCfg, 0, DIR, T>(v, buf, twz_s, tz, z_padded, sync);
+            if constexpr (DIR < 0) {
+                if (tz == 0) {
+#pragma unroll
+                    for (int m = 0; m < P; ++m) scr[m] = v[m];
+                }
+                __syncwarp();
+                hermitian_step<ZCfg, false, T>(v, wt, tz, scr);
+                __syncwarp();
+            } else {
+#pragma unroll
+                for (int m = 0; m < P; ++m) v[m] = mk<T>(v[m].x * scale, v[m].y * scale);
+            }
+            if constexpr (ZCfg::NST > 1) sync();
+            write_own<ZCfg, T>(v, buf, tz, z_dense);
+        } else {
+            constexpr int P = YCfg::P;
+            C v[P];
+            read_own<YCfg, T>(v, buf, ty, y_dense);
+            if constexpr (YCfg::NST > 1) sync();
+            fft_stages<YCfg, 0, DIR, T>(v, buf, twy_s, ty, y_padded, sync);
+            if constexpr (YCfg::NST > 1) sync();
+            write_own<YCfg, T>(v, buf, ty, y_dense);
+        }
+        tma::fence_proxy_async();
+        __syncwarp();
+        if ((tid & 31) == 0) tma::mbar_arrive(&done[s]);
+    }
+}
+
+}  // namespace fft3d

@@ -2,6 +2,7 @@
 // kernels for fp32 and fp64 and exports their description.
 #include "fft_kernels.cuh"
 #include "fft_zpass.cuh"
+#include "fft_fused.cuh"
 #include "fft_configs.cuh"
 #include "fft_registry.h"
 
@@ -13,6 +14,35 @@
 #endif
 
 namespace fft3d {
+
+// fused z+y kernels for Nz == Ny == N (z FFT of N/2 points, y FFT of N points)
+template <typename T, int N>
+static void add_fused(KernelSet& k) {
+    if constexpr (N >= 128) {
+        using C = cx<T>;
+        using YCfg = typename CfgFor<T, N>::type;
+        using ZCfg = typename ZCfgFor<T, N / 2>::type;
+        constexpr int TTC = tma_tile_cols(YCfg::N, YCfg::S, (int)sizeof(C));
+        if constexpr (TTC > 0 && ZCfg::S >= 8 && ZCfg::S <= 32 && (ZCfg::S & (ZCfg::S - 1)) == 0 && ZCfg::P % 2 == 0 &&
+                      (YCfg::S * TTC) % ZCfg::S == 0) {
+            constexpr int RPT = YCfg::S * TTC / ZCfg::S;
+            constexpr int GROUP = YCfg::S * TTC;
+            constexpr int NG = (2 * GROUP + 64 <= 1024 && FusedTile<ZCfg, RPT, YCfg, TTC, T, 2>::max_stages() >= 3) ? 2 : 1;
+            using FT = FusedTile<ZCfg, RPT, YCfg, TTC, T, NG>;
+            constexpr int NS = FT::max_stages();
+            if constexpr (FT::OK && NS >= 2 && FT::THREADS <= 1024) {
+                k.fz_fn[0] = (const void*)fft_zy_fused_kernel<ZCfg, RPT, YCfg, TTC, -1, T, NS, NG>;
+                k.fz_fn[1] = (const void*)fft_zy_fused_kernel<ZCfg, RPT, YCfg, TTC, +1, T, NS, NG>;
+                k.fz_rpt = RPT;
+                k.fz_tc = TTC;
+                k.fz_threads = FT::THREADS;
+                k.fz_smem = (size_t)FT::smem_bytes(NS);
+                k.fz_ng = NG;
+                k.fz_nstage = NS;
+            }
+        }
+    }
+}
 
 template <typename T>
 static KernelSet make_set(int dtype) {
@@ -56,7 +86,12 @@ static KernelSet make_set(int dtype) {
     if constexpr (TTC > 0) {
         // complex fp32 rows of the user's spectrum (M+1 entries) start on 8-byte boundaries for odd l:
         // the X passes shift those tiles' windows (ODDFIX, see fft_kernels.cuh)
+        // (fp64: the same shift puts the 64-byte windows of odd rows on 32-byte sectors of the user array)
+#ifdef FFT3D_NO_OF64
         constexpr bool OF = sizeof(C) % 16 != 0;
+#else
+        constexpr bool OF = true;
+#endif
         using TY = TmaTile<Cfg, TTC, T, false>;
         // X passes: same tile width (48-byte rows were tried to get a second ring stage back at
         // N = 1536 where the shifted windows land TC+2 columns: rows that are not a multiple of the
@@ -100,6 +135,7 @@ static KernelSet make_set(int dtype) {
             k.zb_smem = (size_t)ZT::smem_bytes(NS, NG);
         }
     }
+    add_fused<T, FFT3D_N>(k);
     return k;
 }
 

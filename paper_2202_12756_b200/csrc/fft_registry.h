@@ -37,6 +37,13 @@ struct KernelSet {
     int zb_nst, zb_radix[5], zb_twn;   // their factorisation (it may differ from the strided kernels')
     int zb_threads;            // consumer groups + one producer warp
     size_t zb_smem;
+    // fused z+y kernels of a cubic-like plan (Nz == Ny == N): fft_fused.cuh; null if not compiled
+    const void* fz_fn[2];      // [0 = F1+F2, 1 = I2+I3]
+    int fz_rpt;                // rows per z tile (Ny must be a multiple)
+    int fz_tc;                 // columns per y tile (Nz/2 must be a multiple)
+    int fz_threads;
+    size_t fz_smem;
+    int fz_ng, fz_nstage;      // consumer groups per CTA, shared-memory ring depth
 };
 
 // nullptr if this build has no kernels for (n, dtype)

@@ -1,0 +1,123 @@
+"""GPU parity of the fused z+y passes (csrc/fft_fused.cuh) against the fp64 CPU oracle.
+
+variant 3 forces the fused kernels wherever they are compiled (cubic-like plans, N >= 128), so the
+small shapes here run the very kernels that variant 0 picks by default at 1024^3 fp32
+(tests/test_gpu_fullsize.py covers that size).  Tolerances are BASELINE.json's.
+"""
+import math
+
+import numpy as np
+import pytest
+import torch
+
+pytestmark = pytest.mark.gpu
+
+
+def tol(shape, dtype):
+    n = shape[0] * shape[1] * shape[2]
+    return (2e-6 if dtype == torch.float32 else 1e-13) * math.log2(n)
+
+
+def rel_l2(a, b):
+    a = np.asarray(a)
+    b = np.asarray(b)
+    return float(np.linalg.norm((a - b).ravel()) / np.linalg.norm(b.ravel()))
+
+
+@pytest.fixture(scope="module")
+def fft():
+    import paper_2202_12756_b200 as m
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    m.load_library()
+    return m
+
+
+CASES = [
+    # shape (Ny == Nz), p
+    ((128, 128, 128), 4),
+    ((64, 256, 256), 8),        # fewer planes than CTAs per role; ring deeper than a role's lead
+    ((256, 256, 256), 8),       # BASELINE.json configs[1] shape
+    ((96, 384, 384), 12),       # 3*2^a lengths (radix 3) through the fused kernels
+    ((16, 512, 512), 2),        # Nx barely above the ring depth
+]
+
+
+@pytest.mark.parametrize("shape,p", CASES)
+@pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
+def test_fused_matches_oracle(fft, oracle_mod, shape, p, dtype):
+    from paper_2202_12756_b200 import inputs
+    f = inputs.uniform_grid(shape, dtype, seed=2)
+    plan = fft.Plan(*shape, dtype=dtype, virtual_slabs=p)
+    plan.set_variant(3)
+    if "zy_r2c_fused" not in plan.launch_names(0):
+        pytest.skip("fused kernels are not compiled for %s %s" % (shape, dtype))
+    assert "yz_c2r_fused" in plan.launch_names(1)
+    assert "z_r2c" not in plan.launch_names(0) and "z_c2r" not in plan.launch_names(1)
+    d_in = f.cuda()
+    keep = d_in.clone()
+    work = plan.empty_workspace("cuda")
+    d_out = plan.r2c(d_in, work=work)
+    torch.cuda.synchronize()
+    assert torch.equal(d_in, keep), "input must be preserved"
+    F_gpu = plan.to_natural(d_out).cpu().numpy().astype(np.complex128)
+    F_ref = oracle_mod.r2c(f.double().numpy())
+    assert rel_l2(F_gpu, F_ref) <= tol(shape, dtype)
+    # inverse of a random, NOT Hermitian-consistent half spectrum (reading R8)
+    S = inputs.random_spectrum(shape, plan.complex_dtype, seed=4)
+    f_ref = oracle_mod.c2r(S.to(torch.complex128).numpy(), shape[2])
+    d_S = plan.from_natural(S.cuda())
+    keep = d_S.clone()
+    f_gpu = plan.c2r(d_S, work=work)
+    torch.cuda.synchronize()
+    assert torch.equal(d_S, keep), "input must be preserved"
+    assert rel_l2(f_gpu.cpu().double().numpy(), f_ref) <= tol(shape, dtype)
+    # round trip, reusing the same workspace (the counters are re-zeroed by every call)
+    back = plan.c2r(d_out, work=work)
+    err = (back.cpu().double() - f.double()).abs().max().item() / f.double().abs().max().item()
+    assert err <= tol(shape, dtype)
+    plan.close()
+
+
+@pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
+def test_fused_is_deterministic_and_close_to_unfused(fft, dtype):
+    """Run to run and across virtual_slabs the fused path is bit-identical (no atomics on data, reading
+    R12); against the unfused kernels it may differ in the last bits only (separately compiled code)."""
+    from paper_2202_12756_b200 import inputs
+    shape = (128, 256, 256)
+    f = inputs.normal_grid(shape, dtype, seed=6).cuda()
+    ref = None
+    for p in (1, 8, 32):
+        for rep in range(2):
+            plan = fft.Plan(*shape, dtype=dtype, virtual_slabs=p)
+            plan.set_variant(3)
+            assert "zy_r2c_fused" in plan.launch_names(0)
+            out = plan.r2c(f)
+            back = plan.c2r(out)
+            nat = plan.to_natural(out).contiguous()
+            if ref is None:
+                ref = (nat.clone(), back.clone())
+            else:
+                assert torch.equal(torch.view_as_real(nat), torch.view_as_real(ref[0]))
+                assert torch.equal(back, ref[1])
+            plan.close()
+    plan = fft.Plan(*shape, dtype=dtype, virtual_slabs=8)
+    plan.set_variant(2)
+    assert "z_r2c" in plan.launch_names(0)
+    nat2 = plan.to_natural(plan.r2c(f))
+    scale = ref[0].abs().max().item()
+    eps = 1.2e-7 if dtype == torch.float32 else 2.3e-16
+    assert (nat2 - ref[0]).abs().max().item() <= 64 * eps * scale
+    plan.close()
+
+
+def test_default_variant_picks_fused_only_where_it_wins(fft):
+    small = fft.Plan(256, 256, 256, dtype=torch.float32, virtual_slabs=8)
+    assert small.launch_names(0)[0] == "z_r2c"            # L2-sized problem: unfused passes
+    small.set_variant(3)
+    assert small.launch_names(0)[0] == "zy_r2c_fused"
+    small.set_variant(1)
+    assert small.launch_names(0)[0] == "z_r2c" and "x_c2c_inv_col0" not in small.launch_names(1)
+    small.close()
+    with pytest.raises(fft.binding.Fft3dError):
+        bad = fft.Plan(64, 64, 64, dtype=torch.float32, virtual_slabs=4)
+        bad.set_variant(4)
