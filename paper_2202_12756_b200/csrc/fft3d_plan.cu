@@ -257,17 +257,18 @@ int launch_fused(const fft3d_plan_s* pl, int d, const void* in, void* out, void*
     unsigned* flags = reinterpret_cast<unsigned*>(w + pl->slab_bytes + pl->ring_bytes + pl->side_bytes);
     if (cudaMemsetAsync(flags, 0, pl->flags_bytes, st) != cudaSuccess) { cudaGetLastError(); return FFT3D_ECUDA; }
     TensorMapBlob ring_map, slab_map;
-    {   // the ring as [R][Ny][M]
-        const long long sz = 2 * pl->esize, W = sz / 8;
-        long long dm[3] = {pl->M * W, pl->Ny, pl->fz_R}, sb[2] = {pl->M * sz, pl->Ny * pl->M * sz};
-        int bx[3] = {(int)(ky->fz_tc * W), pl->y_rows_nat, 1};
-        if (!make_map(pl, &ring_map, ring, 3, dm, sb, bx)) return FFT3D_ECUDA;
+    {   // the ring as [R][M/TC][Ny][TC]; a z tile is the box (TC, M/TC, RPT, 1)
+        const long long sz = 2 * pl->esize, W = sz / 8, tc = ky->fz_tc, nb = pl->M / tc;
+        long long dm[4] = {tc * W, nb, pl->Ny, pl->fz_R};
+        long long sb[3] = {pl->Ny * tc * sz, tc * sz, pl->Ny * pl->M * sz};
+        int bx[4] = {(int)(tc * W), (int)nb, ky->fz_rpt, 1};
+        if (!make_map(pl, &ring_map, ring, 4, dm, sb, bx)) return FFT3D_ECUDA;
     }
     if (!map_slab_y(pl, &slab_map, slab, ky->fz_tc, pl->y_rows_slab)) return FFT3D_ECUDA;
     FusedArgs a{};
     a.in = in; a.out = out; a.ring = ring; a.tw_z = pl->tw_zb; a.twz = pl->twz; a.tw_y = pl->tw_y; a.flags = flags;
     a.Nx = (int)pl->Nx; a.Ny = (int)pl->Ny; a.L = (int)pl->L; a.R = pl->fz_R; a.kz = pl->fz_kz[d];
-    a.rows_ring = pl->y_rows_nat; a.rows_slab = pl->y_rows_slab;
+    a.rows_slab = pl->y_rows_slab;
     a.scale = 1.0 / ((double)pl->Nx * (double)pl->Ny * (double)pl->Nz);
 #ifdef FFT3D_TUNING
     if (const char* e = getenv("FFT3D_FZ_KZ")) a.kz = atoi(e);
@@ -384,7 +385,7 @@ int fft3d_plan(fft3d_plan_t** out, long long Nx, long long Ny, long long Nz, int
     // and a device that can hold one CTA per SM co-resident (cooperative launch)
     pl->slab_bytes = (size_t)Nx * Ny * pl->M * 2 * pl->esize;
     if (rc == FFT3D_OK && pl->tma_y && pl->bulk_z && ky->fz_fn[0] != nullptr && Nz == Ny && ky->fz_tc == ky->tma_tc &&
-        Ny % ky->fz_rpt == 0 && pl->M % ky->fz_tc == 0) {
+        Ny % ky->fz_rpt == 0 && pl->M % ky->fz_tc == 0 && pl->M / ky->fz_tc <= 256) {
         const size_t plane = (size_t)Ny * pl->M * 2 * pl->esize;
         int R = (int)(((size_t)48 << 20) / plane);
         if (R > 8) R = 8;
@@ -401,10 +402,9 @@ int fft3d_plan(fft3d_plan_t** out, long long Nx, long long Ny, long long Nz, int
             }
             if (ok) {
                 pl->fused = true; pl->fz_R = R;
-                // a z tile costs ~1.2x the instructions of a y tile: 54 % (forward; inverse 51 %, measured)
-                // of the SMs, rounded to whole TPCs
-                pl->fz_kz[0] = (int)(sms * 0.54 + 1.0) & ~1;
-                pl->fz_kz[1] = (int)(sms * 0.51 + 1.0) & ~1;
+                // a z tile costs ~1.2x the instructions of a y tile: 54 % of the SMs (80 of 148: best of a
+                // sweep 70..84 in both directions), rounded to whole TPCs
+                pl->fz_kz[0] = pl->fz_kz[1] = (int)(sms * 0.54 + 1.0) & ~1;
                 // measured on B200: the fused pass wins once the array is far larger than L2 and the CTA has
                 // two consumer groups on a 3-slot ring (fp32 1024^3: 2.64 vs 3.13 ms); below that the
                 // counters' latency and the single group (fp64: 2 slots) cost more than the HBM pass saved

@@ -13,10 +13,17 @@
 // ALL SMs, one CTA per SM, each CTA with a fixed ROLE: "z CTAs" transform z tiles (RPT whole rows),
 // "y CTAs" transform y tiles (TC columns of a plane).  Planes are handled in order; the tiles of a
 // role are dealt round-robin to the CTAs of that role.  The "phase-1" role (forward: z, inverse: y)
-// writes its result into ring slot x % R ([R][Ny][M] complex), the "phase-2" role reads it from
+// writes its result into ring slot x % R, the "phase-2" role reads it from
 // there as soon as the plane is complete -- so the ring lives in L2 (written with an evict_last
 // policy; the streaming input and output use evict_first) and HBM sees ONE read and ONE write of
 // the array for the two passes together.
+//
+// Ring layout: [R][M/TC][Ny][TC] -- a plane stored column tile by column tile, so that a y tile
+// (all Ny rows of TC columns) is ONE contiguous block that moves with plain bulk copies, and a z
+// tile (RPT whole rows) is ONE 4-D tensor box (TC, M/TC, RPT, 1) whose shared-memory image is the
+// dense [RPT][M] tile.  The transpose between the two 1-D FFTs is thus done by the TMA unit of the
+// z CTAs; each role has one cheap (contiguous) and one row-granular (64-byte rows) side, instead of
+// the y CTAs carrying two row-granular sides (measured: their TMA row rate was the floor).
 //
 // Why roles: the two tile bodies are ~35 KB of straight-line code each and the two SMs of a TPC
 // share an instruction cache; with both bodies alive in one TPC 60 % of the issue stalls in the
@@ -47,14 +54,14 @@ namespace fft3d {
 struct FusedArgs {
     const void* in;          // forward: the real input; inverse: unused (slab read through its tensor map)
     void* out;               // inverse: the real output; forward: unused (slab written through its tensor map)
-    void* ring;              // [R][Ny][M] complex
+    void* ring;              // [R][M/TC][Ny][TC] complex: column-tiled planes
     const void* tw_z;        // stage twiddles of the M-point FFT (forward)
     const void* twz;         // exp(-2 pi i k / Nz), k < M
     const void* tw_y;        // stage twiddles of the Ny-point FFT (forward)
     unsigned* flags;         // [2][Nx]: p1_done, p2_loaded
     int Nx, Ny, L;           // L = Ny / virtual_slabs
     int R;                   // ring planes
-    int rows_ring, rows_slab;   // rows per TMA box on the ring side / the slab side of a y tile
+    int rows_slab;           // rows per TMA box on the slab side of a y tile
     double scale;            // inverse: 1/(Nx Ny Nz)
     int kz;                  // SMs [0, kz) take the z tiles (0: split by CTA pairs)
 };
@@ -79,19 +86,10 @@ __device__ __forceinline__ void bulk_store_h(void* dst, const void* src, unsigne
     asm volatile("cp.async.bulk.global.shared::cta.bulk_group.L2::cache_hint [%0], [%1], %2, %3;"
                  ::"l"(dst), "r"(smem_u32(src)), "r"(bytes), "l"(pol) : "memory");
 }
-__device__ __forceinline__ void load3_h(void* dst, const void* map, unsigned long long* bar, int c0, int c1, int c2,
-                                        unsigned long long pol) {
-    asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1, {%3, %4, %5}], [%2], %6;"
-                 ::"r"(smem_u32(dst)), "l"(map), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2), "l"(pol) : "memory");
-}
 __device__ __forceinline__ void load4_h(void* dst, const void* map, unsigned long long* bar, int c0, int c1, int c2, int c3,
                                         unsigned long long pol) {
     asm volatile("cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1, {%3, %4, %5, %6}], [%2], %7;"
                  ::"r"(smem_u32(dst)), "l"(map), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "l"(pol) : "memory");
-}
-__device__ __forceinline__ void store3_h(const void* map, const void* src, int c0, int c1, int c2, unsigned long long pol) {
-    asm volatile("cp.async.bulk.tensor.3d.global.shared::cta.bulk_group.L2::cache_hint [%0, {%2, %3, %4}], [%1], %5;"
-                 ::"l"(map), "r"(smem_u32(src)), "r"(c0), "r"(c1), "r"(c2), "l"(pol) : "memory");
 }
 __device__ __forceinline__ void store4_h(const void* map, const void* src, int c0, int c1, int c2, int c3,
                                          unsigned long long pol) {
@@ -242,23 +240,24 @@ fft_zy_fused_kernel(const __grid_constant__ TensorMapBlob ring_map, const __grid
                 }
                 const bool isz = FWD ? it.p1 : !it.p1;
                 if (isz) {
-                    // forward: rows of the real input (HBM stream); inverse: rows of the ring
-                    const unsigned char* src = FWD
-                        ? reinterpret_cast<const unsigned char*>(a.in) + (long long)it.x * plane_bytes
-                        : reinterpret_cast<const unsigned char*>(a.ring) + (long long)(it.x % a.R) * plane_bytes;
-                    src += (long long)it.j * ZT::TILE_BYTES;
-                    const unsigned long long pol = FWD ? pol_stream : pol_keep;
-                    constexpr int CHUNK = 16384;
                     tma::mbar_expect_tx(&full[s], ZT::TILE_BYTES);
-                    for (int o = 0; o < ZT::TILE_BYTES; o += CHUNK)
-                        tma::bulk_load_h(dst + o, src + o, ZT::TILE_BYTES - o < CHUNK ? ZT::TILE_BYTES - o : CHUNK, &full[s], pol);
+                    if constexpr (FWD) {                 // rows of the real input (HBM stream)
+                        const unsigned char* src = reinterpret_cast<const unsigned char*>(a.in) + (long long)it.x * plane_bytes +
+                                                   (long long)it.j * ZT::TILE_BYTES;
+                        constexpr int CHUNK = 16384;
+                        for (int o = 0; o < ZT::TILE_BYTES; o += CHUNK)
+                            tma::bulk_load_h(dst + o, src + o, ZT::TILE_BYTES - o < CHUNK ? ZT::TILE_BYTES - o : CHUNK, &full[s], pol_stream);
+                    } else {                             // RPT rows gathered from the column-tiled ring: one box
+                        tma::load4_h(dst, &ring_map, &full[s], 0, 0, it.j * RPT, it.x % a.R, pol_keep);
+                    }
                 } else {
                     tma::mbar_expect_tx(&full[s], YT::TILE_BYTES);
-                    if constexpr (FWD) {                 // columns of the ring plane
-                        const int nb = NY / a.rows_ring;
-                        for (int b = 0; b < nb; ++b)
-                            tma::load3_h(dst + (size_t)b * a.rows_ring * YT::ROW_BYTES, &ring_map, &full[s],
-                                         it.j * TC * W, b * a.rows_ring, it.x % a.R, pol_keep);
+                    if constexpr (FWD) {                 // column tile j of the ring plane: one contiguous block
+                        const unsigned char* src = reinterpret_cast<const unsigned char*>(a.ring) +
+                                                   (long long)(it.x % a.R) * plane_bytes + (long long)it.j * YT::TILE_BYTES;
+                        constexpr int CHUNK = 16384;
+                        for (int o = 0; o < YT::TILE_BYTES; o += CHUNK)
+                            tma::bulk_load_h(dst + o, src + o, YT::TILE_BYTES - o < CHUNK ? YT::TILE_BYTES - o : CHUNK, &full[s], pol_keep);
                     } else {                             // columns of plane x gathered from the slab layout
                         const int nb = NY / a.rows_slab;
                         for (int b = 0; b < nb; ++b) {
@@ -287,14 +286,15 @@ fft_zy_fused_kernel(const __grid_constant__ TensorMapBlob ring_map, const __grid
                 }
                 const bool isz = FWD ? it.p1 : !it.p1;
                 if (isz) {
-                    unsigned char* dst = FWD
-                        ? reinterpret_cast<unsigned char*>(a.ring) + (long long)(it.x % a.R) * plane_bytes
-                        : reinterpret_cast<unsigned char*>(a.out) + (long long)it.x * plane_bytes;
-                    dst += (long long)it.j * ZT::TILE_BYTES;
-                    const unsigned long long pol = FWD ? pol_keep : pol_stream;
-                    constexpr int CHUNK = 16384;
-                    for (int o = 0; o < ZT::TILE_BYTES; o += CHUNK)
-                        tma::bulk_store_h(dst + o, src + o, ZT::TILE_BYTES - o < CHUNK ? ZT::TILE_BYTES - o : CHUNK, pol);
+                    if constexpr (FWD) {                 // RPT rows scattered into the column-tiled ring: one box
+                        tma::store4_h(&ring_map, src, 0, 0, it.j * RPT, it.x % a.R, pol_keep);
+                    } else {                             // rows of the real output (HBM stream)
+                        unsigned char* dst = reinterpret_cast<unsigned char*>(a.out) + (long long)it.x * plane_bytes +
+                                             (long long)it.j * ZT::TILE_BYTES;
+                        constexpr int CHUNK = 16384;
+                        for (int o = 0; o < ZT::TILE_BYTES; o += CHUNK)
+                            tma::bulk_store_h(dst + o, src + o, ZT::TILE_BYTES - o < CHUNK ? ZT::TILE_BYTES - o : CHUNK, pol_stream);
+                    }
                 } else {
                     if constexpr (FWD) {                 // rows go to their slab addresses (steps 2-4 as addressing)
                         const int nb = NY / a.rows_slab;
@@ -303,11 +303,12 @@ fft_zy_fused_kernel(const __grid_constant__ TensorMapBlob ring_map, const __grid
                             tma::store4_h(&slab_map, src + (size_t)b * a.rows_slab * YT::ROW_BYTES,
                                           it.j * TC * W, r0 % a.L, it.x, r0 / a.L, pol_stream);
                         }
-                    } else {
-                        const int nb = NY / a.rows_ring;
-                        for (int b = 0; b < nb; ++b)
-                            tma::store3_h(&ring_map, src + (size_t)b * a.rows_ring * YT::ROW_BYTES,
-                                          it.j * TC * W, b * a.rows_ring, it.x % a.R, pol_keep);
+                    } else {                             // column tile j of the ring plane: one contiguous block
+                        unsigned char* dst = reinterpret_cast<unsigned char*>(a.ring) +
+                                             (long long)(it.x % a.R) * plane_bytes + (long long)it.j * YT::TILE_BYTES;
+                        constexpr int CHUNK = 16384;
+                        for (int o = 0; o < YT::TILE_BYTES; o += CHUNK)
+                            tma::bulk_store_h(dst + o, src + o, YT::TILE_BYTES - o < CHUNK ? YT::TILE_BYTES - o : CHUNK, pol_keep);
                     }
                 }
                 tma::store_commit();
