@@ -156,11 +156,15 @@ __global__ void __launch_bounds__(Cfg::S * RPT * NG + 32, 1) fft_z_bulk_kernel(c
     C* scratch = reinterpret_cast<C*>(stages + NSTAGE * ZT::STAGE_BYTES);
     unsigned long long* full = reinterpret_cast<unsigned long long*>(reinterpret_cast<unsigned char*>(scratch) + NG * ZT::SCRATCH_BYTES);
     unsigned long long* done = full + NSTAGE;
+    // seen[s] = number of phases of full[s] some consumer group has observed complete.  The groups use a
+    // slot in turn when NSTAGE is not a multiple of NG, and a parity wait only tells the barrier's current
+    // phase from the one before it: a group must not start waiting for phase n+1 before phase n is over.
+    volatile int* seen = reinterpret_cast<volatile int*>(done + NSTAGE);
 
     const int tid = threadIdx.x;
     const bool is_producer = tid >= NCONS;
     if (tid == NCONS) {
-        for (int s = 0; s < NSTAGE; ++s) { tma::mbar_init(&full[s], 1); tma::mbar_init(&done[s], GROUP / 32); }
+        for (int s = 0; s < NSTAGE; ++s) { tma::mbar_init(&full[s], 1); tma::mbar_init(&done[s], GROUP / 32); seen[s] = 0; }
         tma::fence_mbar_init();
     }
     if (!is_producer) load_twiddles<DIR, T>(tw, reinterpret_cast<const C*>(a.tw), Cfg::TWN, tid, NCONS);
@@ -222,7 +226,10 @@ __global__ void __launch_bounds__(Cfg::S * RPT * NG + 32, 1) fft_z_bulk_kernel(c
     for (long long i = g; i < n_my; i += NG) {
         const int s = (int)(i % NSTAGE);
         C* buf = reinterpret_cast<C*>(stages + s * ZT::STAGE_BYTES);
-        tma::mbar_wait(&full[s], (unsigned)((i / NSTAGE) & 1));
+        const int n = (int)(i / NSTAGE);
+        while (seen[s] < n) { }
+        tma::mbar_wait(&full[s], (unsigned)(n & 1));
+        if (gt == 0) seen[s] = n + 1;
 #ifdef FFT3D_COPY_ONLY_Z   // experiment: data movement without the transform (wrong results by design)
         tma::fence_proxy_async(); __syncwarp();
         if ((tid & 31) == 0) tma::mbar_arrive(&done[s]);

@@ -121,3 +121,24 @@ def test_default_variant_picks_fused_only_where_it_wins(fft):
     with pytest.raises(fft.binding.Fft3dError):
         bad = fft.Plan(64, 64, 64, dtype=torch.float32, virtual_slabs=4)
         bad.set_variant(4)
+
+
+@pytest.mark.parametrize("variant", [3, 2])
+def test_repeated_calls_are_bit_identical(fft, variant):
+    """Race hunt by repetition: the persistent pipelines (mbarrier rings shared by two consumer groups, the
+    per-plane counters of the fused kernels) must give the same bits on every call; one workspace reused."""
+    from paper_2202_12756_b200 import inputs
+    shape = (256, 256, 256)
+    f = inputs.normal_grid(shape, torch.float32, seed=8).cuda()
+    plan = fft.Plan(*shape, dtype=torch.float32, virtual_slabs=8)
+    plan.set_variant(variant)
+    work = plan.empty_workspace("cuda")
+    out0 = plan.r2c(f, work=work).clone()
+    back0 = plan.c2r(out0, work=work).clone()
+    out, back = plan.empty_complex("cuda"), plan.empty_real("cuda")
+    for _ in range(60):
+        plan.r2c(f, out, work)
+        plan.c2r(out, back, work)
+        assert torch.equal(torch.view_as_real(out), torch.view_as_real(out0))
+        assert torch.equal(back, back0)
+    plan.close()
