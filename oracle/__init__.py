@@ -14,6 +14,8 @@ from .fft3d_oracle import (  # noqa: F401
     c2r,
     r2c_pencils,
     c2r_points,
+    dft3d_c2c_direct,
+    c2c,
     max_threads,
 )
 from .slab_layout import (  # noqa: F401

@@ -513,6 +513,68 @@ int oracle_c2r_points_f32(const float *F, long Nx, long Ny, long Nz, long p, int
                           const long *jxs, const long *jys, const long *jzs, double *out, int nthreads)
 { return points_generic(F, 1, Nx, Ny, Nz, p, K, jxs, jys, jzs, out, nthreads); }
 
+/* ------------------------------------------------------------------------------------
+ * 6. 3D complex-to-complex transform (the paper's library shares one
+ *    workspace between R2C, C2C and C2R).  sign = -1: forward, unnormalised,
+ *    F(k) = sum_j f(j) exp(-2 pi i [jx kx/Nx + jy ky/Ny + jz kz/Nz]) (Eq. (1) with complex f,
+ *    all kz); sign = +1: inverse, scaled by 1/(NxNyNz) (Eq. (2) with the convention of
+ *    reading R1).  oracle_dft3d_c2c_direct is that definition summed term by term,
+ *    O(N^6); oracle_c2c is the separable evaluation (z, y, x lines; x, y, z for the
+ *    inverse) with the recursive mixed-radix 1D transform above.
+ * ---------------------------------------------------------------------------------- */
+int oracle_dft3d_c2c_direct(const double *f_in, int Nx, int Ny, int Nz, int sign, double *F_out)
+{
+    const cplx *f = (const cplx *)f_in;
+    cplx *F = (cplx *)F_out;
+    if (sign != 1 && sign != -1) return 1;
+    const long double scale = sign > 0 ? 1.0L / ((long double)Nx * Ny * Nz) : 1.0L;
+    for (int kx = 0; kx < Nx; ++kx)
+    for (int ky = 0; ky < Ny; ++ky)
+    for (int kz = 0; kz < Nz; ++kz) {
+        long double sre = 0.0L, sim = 0.0L;
+        for (int jx = 0; jx < Nx; ++jx)
+        for (int jy = 0; jy < Ny; ++jy)
+        for (int jz = 0; jz < Nz; ++jz) {
+            long long den = (long long)Nx * Ny * Nz;
+            long long num = (long long)jx * kx * ((long long)Ny * Nz)
+                          + (long long)jy * ky * ((long long)Nx * Nz)
+                          + (long long)jz * kz * ((long long)Nx * Ny);
+            cplx w = root_of_unity(num, den, sign);
+            cplx v = f[((size_t)jx * Ny + jy) * Nz + jz];
+            sre += (long double)v.re * w.re - (long double)v.im * w.im;
+            sim += (long double)v.re * w.im + (long double)v.im * w.re;
+        }
+        cplx r = { (double)(sre * scale), (double)(sim * scale) };
+        F[((size_t)kx * Ny + ky) * Nz + kz] = r;
+    }
+    return 0;
+}
+
+int oracle_c2c(const double *in, long Nx, long Ny, long Nz, int sign, double *out, int nthreads)
+{
+    if (Nx < 1 || Ny < 1 || Nz < 1 || (sign != 1 && sign != -1)) return 1;
+    cplx *a = (cplx *)out;
+    const size_t n = (size_t)Nx * Ny * Nz;
+    memcpy(a, in, n * sizeof(cplx));
+    int err;
+    if (sign < 0) {
+        /* z rows, then y lines (stride Nz), then x lines (stride Ny*Nz): paper steps 1 and 5 */
+        err = fft_lines(a, Nz, 1, Nx * Ny, Nx * Ny, Nz, 0, sign, nthreads);
+        if (!err) err = fft_lines(a, Ny, Nz, Nx * Nz, Nz, 1, Ny * Nz, sign, nthreads);
+        if (!err) err = fft_lines(a, Nx, Ny * Nz, Ny * Nz, Ny * Nz, 1, 0, sign, nthreads);
+    } else {
+        /* reverse order */
+        err = fft_lines(a, Nx, Ny * Nz, Ny * Nz, Ny * Nz, 1, 0, sign, nthreads);
+        if (!err) err = fft_lines(a, Ny, Nz, Nx * Nz, Nz, 1, Ny * Nz, sign, nthreads);
+        if (!err) err = fft_lines(a, Nz, 1, Nx * Ny, Nx * Ny, Nz, 0, sign, nthreads);
+        if (!err) {
+            const double sc = 1.0 / ((double)Nx * (double)Ny * (double)Nz);
+            for (size_t i = 0; i < n; ++i) { a[i].re *= sc; a[i].im *= sc; }
+        }
+    }
+    return err;
+}
+
 int oracle_max_threads(void)
 {
 #ifdef _OPENMP

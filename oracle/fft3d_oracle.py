@@ -49,6 +49,8 @@ def _load():
             getattr(lib, nm).argtypes = [dp, L, L, L, I, dp, dp, dp, I]
         for nm in ("oracle_c2r_points_f64", "oracle_c2r_points_f32"):
             getattr(lib, nm).argtypes = [dp, L, L, L, L, I, dp, dp, dp, dp, I]
+        lib.oracle_dft3d_c2c_direct.argtypes = [dp, I, I, I, I, dp]
+        lib.oracle_c2c.argtypes = [dp, L, L, L, I, dp, I]
         lib.oracle_max_threads.restype = I
         _lib = lib
     return _lib
@@ -153,4 +155,24 @@ def c2r_points(F_flat: np.ndarray, shape, p: int, jxs, jys, jzs, nthreads: int =
     fn = _load().oracle_c2r_points_f32 if F_flat.dtype == np.complex64 else _load().oracle_c2r_points_f64
     _check(fn(_ptr(F_flat), Nx, Ny, Nz, int(p), K, _ptr(jxs), _ptr(jys), _ptr(jzs), _ptr(out), nt),
            "c2r_points")
+    return out
+
+
+def dft3d_c2c_direct(f: np.ndarray, sign: int) -> np.ndarray:
+    """The complex 3D DFT summed term by term, O(N^6): sign -1 forward (unnormalised), +1 inverse
+    (1/(NxNyNz)); tiny grids only."""
+    f = np.ascontiguousarray(f, dtype=np.complex128)
+    Nx, Ny, Nz = f.shape
+    out = np.empty_like(f)
+    _check(_load().oracle_dft3d_c2c_direct(_ptr(f), Nx, Ny, Nz, int(sign), _ptr(out)), "dft3d_c2c_direct")
+    return out
+
+
+def c2c(f: np.ndarray, sign: int, nthreads: int = 0) -> np.ndarray:
+    """3D C2C, natural order (Nx, Ny, Nz): sign -1 forward (unnormalised), +1 inverse (1/(NxNyNz))."""
+    f = np.ascontiguousarray(f, dtype=np.complex128)
+    Nx, Ny, Nz = f.shape
+    out = np.empty_like(f)
+    nt = nthreads if nthreads > 0 else max_threads()
+    _check(_load().oracle_c2c(_ptr(f), Nx, Ny, Nz, int(sign), _ptr(out), nt), "c2c")
     return out
