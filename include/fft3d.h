@@ -106,6 +106,23 @@ int fft3d_r2c(const fft3d_plan_t *plan, const void *d_real_in, void *d_cplx_out,
 int fft3d_c2r(const fft3d_plan_t *plan, const void *d_cplx_in, void *d_real_out,
               void *d_work, void *cuda_stream);
 
+/* 3D complex-to-complex transform (in the paper's library R2C, C2C and C2R share one
+ * workspace).  fft3d_plan_c2c creates a plan for an Nx x Ny x Nz COMPLEX grid over p virtual
+ * x-slabs: same requirements as fft3d_plan except that Nz may be odd-free of the "even" rule but must
+ * itself be a supported length >= 128 (fp32) / 64 (fp64) whose row kernel exists, and Nx*Ny must be a
+ * multiple of its tile (<= 32 rows); otherwise FFT3D_EUNSUPPORTED.  For such a plan
+ * fft3d_complex_bytes = Nx*Ny*Nz complex (input, output), fft3d_workspace_bytes the same,
+ * fft3d_real_bytes = 0, fft3d_index(kx,ky,kz) = ((q*Nx + kx)*(Ny/p) + ky % (Ny/p))*Nz + kz.
+ * fft3d_c2c: direction -1 = forward, unnormalised, d_in natural [Nx][Ny][Nz] -> d_out in the slab layout
+ * [p][Nx][Ny/p][Nz]; direction +1 = inverse scaled by 1/(NxNyNz), slab layout -> natural.  Three full-array
+ * passes (z rows, y lines with the slab permutation, x lines).  d_out is also used as scratch; d_in is
+ * preserved; all pointers 16-byte aligned device pointers, no overlap; asynchronous on the stream.
+ * fft3d_r2c / fft3d_c2r reject a C2C plan with FFT3D_EINVAL and vice versa. */
+int fft3d_plan_c2c(fft3d_plan_t **plan_out, long long Nx, long long Ny, long long Nz,
+                   int dtype, int virtual_slabs);
+int fft3d_c2c(const fft3d_plan_t *plan, const void *d_cplx_in, void *d_cplx_out,
+              void *d_work, int direction, void *cuda_stream);
+
 /* Host-buffer variants: H2D copy, transform, D2H copy, synchronous.  The plan lazily
  * allocates real + complex + workspace device buffers (fft3d_real_bytes + fft3d_complex_bytes
  * + fft3d_workspace_bytes) and keeps them until fft3d_destroy. */
@@ -117,7 +134,8 @@ int fft3d_c2r_host(fft3d_plan_t *plan, const void *h_cplx_in, void *h_real_out);
  * "x_c2c_fwd", "nyquist_unpack", "nyquist_pack", "x_c2c_inv", "x_c2c_inv_col0" (the packed
  * column 0 of the inverse x pass, TMA path only), "y_c2c_inv", "z_c2r", and -- when the z and y
  * passes of a plane run as one kernel through an L2-resident ring --
- * "zy_r2c_fused" (paper step 1 + steps 2-4) and "yz_c2r_fused" (their reverse). */
+ * "zy_r2c_fused" (paper step 1 + steps 2-4) and "yz_c2r_fused" (their reverse); C2C plans:
+ * "z_c2c_fwd", "y_c2c_fwd", "x_c2c_fwd" (which = 0) and "x_c2c_inv", "y_c2c_inv", "z_c2c_inv" (which = 1). */
 int fft3d_launches(const fft3d_plan_t *plan, int which);
 const char *fft3d_launch_name(const fft3d_plan_t *plan, int which, int i);
 

@@ -19,7 +19,7 @@ EXPORTS = (
     "fft3d_plan", "fft3d_supported_length", "fft3d_workspace_bytes", "fft3d_real_bytes",
     "fft3d_complex_bytes", "fft3d_index", "fft3d_r2c", "fft3d_c2r", "fft3d_r2c_host",
     "fft3d_c2r_host", "fft3d_launches", "fft3d_launch_name", "fft3d_set_variant", "fft3d_destroy", "fft3d_strerror",
-    "fft3d_timing_enable", "fft3d_timing_read",
+    "fft3d_timing_enable", "fft3d_timing_read", "fft3d_plan_c2c", "fft3d_c2c",
 )
 
 _lib = None
@@ -44,6 +44,10 @@ def load_library() -> ctypes.CDLL:
     vp, ll, i, sz = ctypes.c_void_p, ctypes.c_longlong, ctypes.c_int, ctypes.c_size_t
     lib.fft3d_plan.argtypes = [ctypes.POINTER(vp), ll, ll, ll, i, i]
     lib.fft3d_plan.restype = i
+    lib.fft3d_plan_c2c.argtypes = [ctypes.POINTER(vp), ll, ll, ll, i, i]
+    lib.fft3d_plan_c2c.restype = i
+    lib.fft3d_c2c.argtypes = [vp, vp, vp, vp, i, vp]
+    lib.fft3d_c2c.restype = i
     lib.fft3d_supported_length.argtypes = [ll]
     lib.fft3d_supported_length.restype = i
     for nm in ("fft3d_workspace_bytes", "fft3d_real_bytes", "fft3d_complex_bytes"):
@@ -219,3 +223,51 @@ class Plan:
             self.close()
         except Exception:
             pass
+
+
+class PlanC2C(Plan):
+    """fft3d_plan_c2c(Nx, Ny, Nz, dtype, virtual_slabs): 3D complex-to-complex transform (argument marshalling
+    only).  Forward output / inverse input are flat complex buffers in the slab layout [p][Nx][Ny/p][Nz]."""
+
+    def __init__(self, Nx: int, Ny: int, Nz: int, dtype=torch.float32, virtual_slabs: int = 1):
+        lib = load_library()
+        self.dtype_code = {torch.float32: F32, torch.float64: F64}[dtype]
+        self.shape = (int(Nx), int(Ny), int(Nz))
+        self.p = int(virtual_slabs)
+        h = ctypes.c_void_p()
+        rc = lib.fft3d_plan_c2c(ctypes.byref(h), Nx, Ny, Nz, self.dtype_code, self.p)
+        if rc != 0:
+            raise Fft3dError(rc, "fft3d_plan_c2c(%d,%d,%d,p=%d)" % (Nx, Ny, Nz, self.p))
+        self._h = h
+        self._lib = lib
+        self.real_dtype = _REAL[self.dtype_code]
+        self.complex_dtype = _CPLX[self.dtype_code]
+        self.real_bytes = lib.fft3d_real_bytes(h)
+        self.complex_bytes = lib.fft3d_complex_bytes(h)
+        self.workspace_bytes = lib.fft3d_workspace_bytes(h)
+        self.n_complex = Nx * Ny * Nz
+
+    def c2c(self, cplx_in, direction: int, cplx_out=None, work=None, stream=None):
+        self._check(cplx_in, self.complex_dtype, self.complex_bytes, "cplx_in")
+        if cplx_out is None:
+            cplx_out = self.empty_complex(cplx_in.device)
+        if work is None:
+            work = self.empty_workspace(cplx_in.device)
+        self._check(cplx_out, self.complex_dtype, self.complex_bytes, "cplx_out")
+        s = stream if stream is not None else torch.cuda.current_stream(cplx_in.device)
+        rc = self._lib.fft3d_c2c(self._h, cplx_in.data_ptr(), cplx_out.data_ptr(), work.data_ptr(), int(direction),
+                                 ctypes.c_void_p(s.cuda_stream))
+        if rc != 0:
+            raise Fft3dError(rc, "fft3d_c2c")
+        return cplx_out
+
+    def to_natural(self, cplx_flat: torch.Tensor) -> torch.Tensor:
+        Nx, Ny, Nz = self.shape
+        L = Ny // self.p
+        return cplx_flat.reshape(self.p, Nx, L, Nz).permute(1, 0, 2, 3).reshape(Nx, Ny, Nz)
+
+    def from_natural(self, cplx_nat: torch.Tensor) -> torch.Tensor:
+        Nx, Ny, Nz = self.shape
+        L = Ny // self.p
+        return cplx_nat.reshape(Nx, self.p, L, Nz).permute(1, 0, 2, 3).contiguous().reshape(-1)
+

@@ -59,7 +59,9 @@ struct TimingState {
 };
 
 struct fft3d_plan_s {
-    long long Nx, Ny, Nz, M, L;
+    long long Nx, Ny, Nz, M, L;         // M = columns of the intermediate rows: Nz/2 (R2C/C2R plans), Nz (C2C plans)
+    int kind;                           // 0 = R2C/C2R plan, 1 = C2C plan
+    void* tw_zc;                        // stage twiddles of the C2C row kernels
     int p, dtype, esize;       // esize = bytes per real
     int variant;
     const KernelSet *kz, *ky, *kx;
@@ -306,17 +308,20 @@ int fft3d_supported_length(long long n) {
     return find_kernels(n, FFT3D_F32) != nullptr ? 1 : 0;
 }
 
-int fft3d_plan(fft3d_plan_t** out, long long Nx, long long Ny, long long Nz, int dtype, int virtual_slabs) {
+static int plan_create(fft3d_plan_t** out, long long Nx, long long Ny, long long Nz, int dtype, int virtual_slabs, int kind) {
     if (out == nullptr) return FFT3D_EINVAL;
     *out = nullptr;
     if (dtype != FFT3D_F32 && dtype != FFT3D_F64) return FFT3D_EINVAL;
     if (Nx < 2 || Ny < 2 || Nz < 2 || virtual_slabs < 1) return FFT3D_EINVAL;
     if (Nx % virtual_slabs != 0 || Ny % virtual_slabs != 0) return FFT3D_EINVAL;
-    if (Nz % 2 != 0) return FFT3D_EUNSUPPORTED;
-    const KernelSet* kz = find_kernels(Nz / 2, dtype);
+    if (kind == 0 && Nz % 2 != 0) return FFT3D_EUNSUPPORTED;
+    const long long Mcols = kind == 0 ? Nz / 2 : Nz;
+    const KernelSet* kz = find_kernels(Mcols, dtype);
     const KernelSet* ky = find_kernels(Ny, dtype);
     const KernelSet* kx = find_kernels(Nx, dtype);
     if (kz == nullptr || ky == nullptr || kx == nullptr) return FFT3D_EUNSUPPORTED;
+    // C2C plans: the row pass exists only as the bulk-pipelined kernel (whole tiles of zc_rpt rows)
+    if (kind == 1 && (kz->zc_fn[0] == nullptr || (Nx * Ny) % kz->zc_rpt != 0)) return FFT3D_EUNSUPPORTED;
 
     int dev = 0, sms = 0;
     if (cudaGetDevice(&dev) != cudaSuccess ||
@@ -327,7 +332,7 @@ int fft3d_plan(fft3d_plan_t** out, long long Nx, long long Ny, long long Nz, int
     fft3d_plan_t* pl = new (std::nothrow) fft3d_plan_t();
     if (pl == nullptr) return FFT3D_ENOMEM;
     std::memset(pl, 0, sizeof(*pl));
-    pl->Nx = Nx; pl->Ny = Ny; pl->Nz = Nz; pl->M = Nz / 2; pl->p = virtual_slabs; pl->L = Ny / virtual_slabs;
+    pl->Nx = Nx; pl->Ny = Ny; pl->Nz = Nz; pl->M = Mcols; pl->kind = kind; pl->p = virtual_slabs; pl->L = Ny / virtual_slabs;
     pl->dtype = dtype; pl->esize = dtype == FFT3D_F32 ? 4 : 8;
     pl->kz = kz; pl->ky = ky; pl->kx = kx; pl->num_sms = sms;
 
@@ -336,7 +341,14 @@ int fft3d_plan(fft3d_plan_t** out, long long Nx, long long Ny, long long Nz, int
     if (rc == FFT3D_OK) rc = upload_stage_twiddles(kx->nst, kx->radix, kx->twn, pl->esize, &pl->tw_x);
     if (rc == FFT3D_OK && kz->zb_fn[0] != nullptr)
         rc = upload_stage_twiddles(kz->zb_nst, kz->zb_radix, kz->zb_twn, pl->esize, &pl->tw_zb);
-    if (rc == FFT3D_OK) rc = upload_z_twiddles(Nz, pl->M, pl->esize, &pl->twz);
+    if (rc == FFT3D_OK && kind == 0) rc = upload_z_twiddles(Nz, pl->M, pl->esize, &pl->twz);
+    if (rc == FFT3D_OK && kind == 1) {
+        rc = upload_stage_twiddles(kz->zc_nst, kz->zc_radix, kz->zc_twn, pl->esize, &pl->tw_zc);
+        for (int d = 0; d < 2 && rc == FFT3D_OK; ++d) {
+            int g = 0;
+            rc = prepare_kernel(kz->zc_fn[d], kz->zc_threads, kz->zc_smem, sms, &g);
+        }
+    }
     for (int d = 0; d < 2 && rc == FFT3D_OK; ++d) {
         rc = prepare_kernel(kz->z_fn[d], kz->z_threads, kz->z_smem, sms, &pl->grid_z[d]);
         const int ykind = d == 0 ? KIND_LIN_SLAB : KIND_SLAB_LIN;
@@ -364,7 +376,7 @@ int fft3d_plan(fft3d_plan_t** out, long long Nx, long long Ny, long long Nz, int
                 rc = prepare_kernel(ky->tma_fn[d == 0 ? TMA_Y_FWD : TMA_Y_INV], ky->tma_threads, ky->tma_smem_y, sms, &g);
             }
         }
-        if (rc == FFT3D_OK && fn != nullptr && strides_ok && kx->tma_fn[TMA_X_FWD] != nullptr && M % kx->tma_tc_x == 0 &&
+        if (rc == FFT3D_OK && kind == 0 && fn != nullptr && strides_ok && kx->tma_fn[TMA_X_FWD] != nullptr && M % kx->tma_tc_x == 0 &&
             (L * (M + 1) * sz) % 16 == 0 && (!kx->tma_oddfix || L % 2 == 0)) {
             pl->x_rows = (int)largest_divisor_le(Nx, 256);
             pl->tma_x = true;
@@ -374,7 +386,7 @@ int fft3d_plan(fft3d_plan_t** out, long long Nx, long long Ny, long long Nz, int
             }
         }
     }
-    if (rc == FFT3D_OK && kz->zb_fn[0] != nullptr && (Nx * Ny) % kz->zb_rpt == 0) {
+    if (rc == FFT3D_OK && kind == 0 && kz->zb_fn[0] != nullptr && (Nx * Ny) % kz->zb_rpt == 0) {
         pl->bulk_z = true;
         for (int d = 0; d < 2 && rc == FFT3D_OK; ++d) {
             int g = 0;
@@ -384,7 +396,7 @@ int fft3d_plan(fft3d_plan_t** out, long long Nx, long long Ny, long long Nz, int
     // fused z+y passes: cubic-like extents, whole tiles, a ring of >= 3 planes inside ~48 MB of L2,
     // and a device that can hold one CTA per SM co-resident (cooperative launch)
     pl->slab_bytes = (size_t)Nx * Ny * pl->M * 2 * pl->esize;
-    if (rc == FFT3D_OK && pl->tma_y && pl->bulk_z && ky->fz_fn[0] != nullptr && Nz == Ny && ky->fz_tc == ky->tma_tc &&
+    if (rc == FFT3D_OK && kind == 0 && pl->tma_y && pl->bulk_z && ky->fz_fn[0] != nullptr && Nz == Ny && ky->fz_tc == ky->tma_tc &&
         Ny % ky->fz_rpt == 0 && pl->M % ky->fz_tc == 0 && pl->M / ky->fz_tc <= 256) {
         const size_t plane = (size_t)Ny * pl->M * 2 * pl->esize;
         int R = (int)(((size_t)48 << 20) / plane);
@@ -420,20 +432,30 @@ int fft3d_plan(fft3d_plan_t** out, long long Nx, long long Ny, long long Nz, int
     return FFT3D_OK;
 }
 
+int fft3d_plan(fft3d_plan_t** out, long long Nx, long long Ny, long long Nz, int dtype, int virtual_slabs) {
+    return plan_create(out, Nx, Ny, Nz, dtype, virtual_slabs, 0);
+}
+int fft3d_plan_c2c(fft3d_plan_t** out, long long Nx, long long Ny, long long Nz, int dtype, int virtual_slabs) {
+    return plan_create(out, Nx, Ny, Nz, dtype, virtual_slabs, 1);
+}
+
 size_t fft3d_workspace_bytes(const fft3d_plan_t* pl) {
     return pl ? pl->slab_bytes + pl->ring_bytes + pl->side_bytes + pl->flags_bytes : 0;
 }
 size_t fft3d_real_bytes(const fft3d_plan_t* pl) {
-    return pl ? (size_t)pl->Nx * pl->Ny * pl->Nz * pl->esize : 0;
+    return (pl && pl->kind == 0) ? (size_t)pl->Nx * pl->Ny * pl->Nz * pl->esize : 0;
 }
 size_t fft3d_complex_bytes(const fft3d_plan_t* pl) {
-    return pl ? (size_t)pl->Nx * pl->Ny * (pl->M + 1) * 2 * pl->esize : 0;
+    if (pl == nullptr) return 0;
+    return (size_t)pl->Nx * pl->Ny * (pl->kind == 0 ? pl->M + 1 : pl->Nz) * 2 * pl->esize;
 }
 
 long long fft3d_index(const fft3d_plan_t* pl, long long kx, long long ky, long long kz) {
-    if (pl == nullptr || kx < 0 || kx >= pl->Nx || ky < 0 || ky >= pl->Ny || kz < 0 || kz > pl->M) return -1;
+    if (pl == nullptr || kx < 0 || kx >= pl->Nx || ky < 0 || ky >= pl->Ny || kz < 0) return -1;
+    const long long pitch = pl->kind == 0 ? pl->M + 1 : pl->Nz;
+    if (kz >= pitch) return -1;
     const long long q = ky / pl->L, l = ky % pl->L;
-    return ((q * pl->Nx + kx) * pl->L + l) * (pl->M + 1) + kz;
+    return ((q * pl->Nx + kx) * pl->L + l) * pitch + kz;
 }
 
 static bool use_fused(const fft3d_plan_t* pl) {
@@ -443,6 +465,7 @@ static bool use_tma(const fft3d_plan_t* pl) { return pl->variant != 1; }
 
 int fft3d_launches(const fft3d_plan_t* pl, int which) {
     if (pl == nullptr || which < 0 || which > 1) return 0;
+    if (pl->kind == 1) return 3;
     // c2r on the TMA path runs the packed column 0 of the x pass as a separate small kernel
     int n = (which == 1 && use_tma(pl) && pl->tma_x) ? 5 : 4;
     return use_fused(pl) ? n - 1 : n;
@@ -450,6 +473,11 @@ int fft3d_launches(const fft3d_plan_t* pl, int which) {
 
 const char* fft3d_launch_name(const fft3d_plan_t* pl, int which, int i) {
     if (pl == nullptr || i < 0 || i >= fft3d_launches(pl, which)) return nullptr;
+    if (pl->kind == 1) {
+        static const char* const cf[] = {"z_c2c_fwd", "y_c2c_fwd", "x_c2c_fwd"};
+        static const char* const ci[] = {"x_c2c_inv", "y_c2c_inv", "z_c2c_inv"};
+        return which == 0 ? cf[i] : ci[i];
+    }
     const bool fz = use_fused(pl);
     if (which == 0) {
         static const char* const u[] = {"z_r2c", "y_c2c_fwd", "x_c2c_fwd", "nyquist_unpack"};
@@ -477,7 +505,7 @@ int fft3d_set_variant(fft3d_plan_t* pl, int variant) {
 }
 
 int fft3d_r2c(const fft3d_plan_t* pl, const void* d_in, void* d_out, void* d_work, void* stream) {
-    if (pl == nullptr || d_in == nullptr || d_out == nullptr || d_work == nullptr) return FFT3D_EINVAL;
+    if (pl == nullptr || pl->kind != 0 || d_in == nullptr || d_out == nullptr || d_work == nullptr) return FFT3D_EINVAL;
     const size_t rb = fft3d_real_bytes(pl), cb = fft3d_complex_bytes(pl), wb = fft3d_workspace_bytes(pl);
     if (((uintptr_t)d_in | (uintptr_t)d_out | (uintptr_t)d_work) & 15) return FFT3D_EINVAL;
     if (overlap(d_in, rb, d_out, cb) || overlap(d_in, rb, d_work, wb) || overlap(d_out, cb, d_work, wb))
@@ -563,7 +591,7 @@ int fft3d_r2c(const fft3d_plan_t* pl, const void* d_in, void* d_out, void* d_wor
 }
 
 int fft3d_c2r(const fft3d_plan_t* pl, const void* d_in, void* d_out, void* d_work, void* stream) {
-    if (pl == nullptr || d_in == nullptr || d_out == nullptr || d_work == nullptr) return FFT3D_EINVAL;
+    if (pl == nullptr || pl->kind != 0 || d_in == nullptr || d_out == nullptr || d_work == nullptr) return FFT3D_EINVAL;
     const size_t rb = fft3d_real_bytes(pl), cb = fft3d_complex_bytes(pl), wb = fft3d_workspace_bytes(pl);
     if (((uintptr_t)d_in | (uintptr_t)d_out | (uintptr_t)d_work) & 15) return FFT3D_EINVAL;
     if (overlap(d_in, cb, d_out, rb) || overlap(d_in, cb, d_work, wb) || overlap(d_out, rb, d_work, wb))
@@ -666,6 +694,83 @@ int fft3d_c2r(const fft3d_plan_t* pl, const void* d_in, void* d_out, void* d_wor
     return rc;
 }
 
+// 3D C2C (the paper's R2C, C2C and C2R share one workspace).  direction -1: forward,
+// unnormalised (z rows, y lines with the slab permutation of steps 2-4, x lines: steps 1 and 5);
+// +1: inverse, scaled by 1/(NxNyNz), the passes in reverse order.
+int fft3d_c2c(const fft3d_plan_t* pl, const void* d_in, void* d_out, void* d_work, int direction, void* stream) {
+    if (pl == nullptr || pl->kind != 1 || d_in == nullptr || d_out == nullptr || d_work == nullptr) return FFT3D_EINVAL;
+    if (direction != -1 && direction != 1) return FFT3D_EINVAL;
+    const size_t cb = fft3d_complex_bytes(pl), wb = fft3d_workspace_bytes(pl);
+    if (((uintptr_t)d_in | (uintptr_t)d_out | (uintptr_t)d_work) & 15) return FFT3D_EINVAL;
+    if (overlap(d_in, cb, d_out, cb) || overlap(d_in, cb, d_work, wb) || overlap(d_out, cb, d_work, wb))
+        return FFT3D_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    const long long Nx = pl->Nx, Ny = pl->Ny, M = pl->M, L = pl->L, p = pl->p;
+    const KernelSet *kz = pl->kz, *ky = pl->ky, *kx = pl->kx;
+    const int d = direction < 0 ? 0 : 1;
+    const bool tma_on = use_tma(pl);
+    Recorder rec(pl, d, st);
+    int slot = 0, rc = FFT3D_OK;
+    rec.mark(slot++);
+
+    auto z_pass = [&](const void* in, void* out) -> int {
+        ZBulkArgs z{};
+        z.in = in; z.out = out; z.tw = pl->tw_zc; z.twz = nullptr;
+        z.ntiles = Nx * Ny / kz->zc_rpt;
+        z.scale = 1.0 / ((double)Nx * (double)Ny * (double)pl->Nz);
+        long long g = z.ntiles < pl->num_sms ? z.ntiles : pl->num_sms;
+        void* argv[1] = {&z};
+        cudaError_t e = cudaLaunchKernel(kz->zc_fn[d], dim3((unsigned)g), dim3((unsigned)kz->zc_threads), argv, kz->zc_smem, st);
+        if (e != cudaSuccess) { cudaGetLastError(); return FFT3D_ECUDA; }
+        return FFT3D_OK;
+    };
+    auto y_pass = [&](const void* in, void* out) -> int {       // forward: natural -> slab; inverse: slab -> natural
+        if (tma_on && pl->tma_y) {
+            TensorMapBlob mi, mo;
+            bool ok = d == 0 ? (map_natural(pl, &mi, in, ky->tma_tc, pl->y_rows_nat) && map_slab_y(pl, &mo, out, ky->tma_tc, pl->y_rows_slab))
+                             : (map_slab_y(pl, &mi, in, ky->tma_tc, pl->y_rows_slab) && map_natural(pl, &mo, out, ky->tma_tc, pl->y_rows_nat));
+            if (!ok) return FFT3D_ECUDA;
+            TmaArgs ta{};
+            ta.tw = pl->tw_y; ta.ntz = (int)(M / ky->tma_tc); ta.ntiles = Nx * ta.ntz;
+            ta.L = (int)L; ta.Nx = (int)Nx; ta.Mp1 = (int)M;
+            ta.in_rows = d == 0 ? pl->y_rows_nat : pl->y_rows_slab; ta.out_rows = d == 0 ? pl->y_rows_slab : pl->y_rows_nat;
+            return launch_tma(ky->tma_fn[d == 0 ? TMA_Y_FWD : TMA_Y_INV], ky->tma_threads, ky->tma_smem_y, pl->num_sms, mi, mi, mo, ta, st);
+        }
+        StridedArgs a{};
+        a.in = in; a.out = out; a.col0 = nullptr; a.tw = pl->tw_y;
+        a.ntz = (int)((M + ky->tc - 1) / ky->tc); a.ncols = (int)M; a.a_lo = 1; a.L = (int)L;
+        a.ntiles = Nx * a.ntz;
+        if (d == 0) {
+            a.in_hi = Ny * M; a.in_lo = 0; a.in_rq = 0; a.in_rl = M;
+            a.out_hi = L * M; a.out_lo = 0; a.out_rq = Nx * L * M; a.out_rl = M;
+            return launch(ky->s_fn[0][KIND_LIN_SLAB], a.ntiles, pl->grid_y[0], ky->s_threads, ky->s_smem, &a, st);
+        }
+        a.in_hi = L * M; a.in_lo = 0; a.in_rq = Nx * L * M; a.in_rl = M;
+        a.out_hi = Ny * M; a.out_lo = 0; a.out_rq = 0; a.out_rl = M;
+        return launch(ky->s_fn[1][KIND_SLAB_LIN], a.ntiles, pl->grid_y[1], ky->s_threads, ky->s_smem, &a, st);
+    };
+    auto x_pass = [&](const void* in, void* out) -> int {       // lines along x inside every virtual slab, pitch M
+        StridedArgs b{};
+        b.in = in; b.out = out; b.col0 = nullptr; b.tw = pl->tw_x;
+        b.ntz = (int)((M + kx->tc - 1) / kx->tc); b.ncols = (int)M; b.a_lo = (int)L; b.L = (int)Nx;
+        b.ntiles = (long long)p * L * b.ntz;
+        b.in_hi = Nx * L * M; b.in_lo = M; b.in_rq = 0; b.in_rl = L * M;
+        b.out_hi = Nx * L * M; b.out_lo = M; b.out_rq = 0; b.out_rl = L * M;
+        return launch(kx->s_fn[d][KIND_LIN_LIN], b.ntiles, pl->grid_x[d], kx->s_threads, kx->s_smem, &b, st);
+    };
+
+    if (d == 0) {
+        rc = z_pass(d_in, d_out);           rec.mark(slot++); if (rc != FFT3D_OK) return rc;
+        rc = y_pass(d_out, d_work);         rec.mark(slot++); if (rc != FFT3D_OK) return rc;
+        rc = x_pass(d_work, d_out);         rec.mark(slot++);
+    } else {
+        rc = x_pass(d_in, d_out);           rec.mark(slot++); if (rc != FFT3D_OK) return rc;
+        rc = y_pass(d_out, d_work);         rec.mark(slot++); if (rc != FFT3D_OK) return rc;
+        rc = z_pass(d_work, d_out);         rec.mark(slot++);
+    }
+    return rc;
+}
+
 static void timing_free(fft3d_plan_t* pl) {
     if (pl->timing == nullptr) return;
     for (int w = 0; w < 2; ++w)
@@ -729,7 +834,7 @@ static int ensure_host_buffers(fft3d_plan_t* pl) {
 }
 
 int fft3d_r2c_host(fft3d_plan_t* pl, const void* h_in, void* h_out) {
-    if (pl == nullptr || h_in == nullptr || h_out == nullptr) return FFT3D_EINVAL;
+    if (pl == nullptr || pl->kind != 0 || h_in == nullptr || h_out == nullptr) return FFT3D_EINVAL;
     int rc = ensure_host_buffers(pl);
     if (rc != FFT3D_OK) return rc;
     cudaStream_t st = pl->h_stream;
@@ -748,7 +853,7 @@ int fft3d_r2c_host(fft3d_plan_t* pl, const void* h_in, void* h_out) {
 }
 
 int fft3d_c2r_host(fft3d_plan_t* pl, const void* h_in, void* h_out) {
-    if (pl == nullptr || h_in == nullptr || h_out == nullptr) return FFT3D_EINVAL;
+    if (pl == nullptr || pl->kind != 0 || h_in == nullptr || h_out == nullptr) return FFT3D_EINVAL;
     int rc = ensure_host_buffers(pl);
     if (rc != FFT3D_OK) return rc;
     cudaStream_t st = pl->h_stream;
@@ -768,7 +873,7 @@ int fft3d_c2r_host(fft3d_plan_t* pl, const void* h_in, void* h_out) {
 
 int fft3d_destroy(fft3d_plan_t* pl) {
     if (pl == nullptr) return FFT3D_OK;
-    cudaFree(pl->tw_zb); cudaFree(pl->tw_z); cudaFree(pl->tw_y); cudaFree(pl->tw_x); cudaFree(pl->twz);
+    cudaFree(pl->tw_zb); cudaFree(pl->tw_zc); cudaFree(pl->tw_z); cudaFree(pl->tw_y); cudaFree(pl->tw_x); cudaFree(pl->twz);
     cudaFree(pl->h_real); cudaFree(pl->h_cplx); cudaFree(pl->h_work);
     if (pl->h_stream) cudaStreamDestroy(pl->h_stream);
     timing_free(pl);

@@ -135,6 +135,23 @@ static KernelSet make_set(int dtype) {
             k.zb_smem = (size_t)ZT::smem_bytes(NS, NG);
         }
     }
+    // C2C row kernels: 256 threads per tile of 256/S rows, any S that divides 256
+    if constexpr (ZCfg::S <= 256 && 256 % ZCfg::S == 0 && ZCfg::N * sizeof(C) >= 1024) {
+        constexpr int RPT = 256 / ZCfg::S;
+        using ZT = ZTile<ZCfg, RPT, T>;
+        constexpr int NG = ZT::max_stages(2) >= 3 ? 2 : 1;
+        constexpr int NS = ZT::max_stages(NG) > 4 ? 4 : ZT::max_stages(NG);
+        if constexpr (NS >= 2) {
+            k.zc_fn[0] = (const void*)fft_z_bulk_kernel<ZCfg, RPT, -1, T, NS, NG, true>;
+            k.zc_fn[1] = (const void*)fft_z_bulk_kernel<ZCfg, RPT, +1, T, NS, NG, true>;
+            k.zc_rpt = RPT;
+            k.zc_nst = ZCfg::NST;
+            for (int s = 0; s < 5; ++s) k.zc_radix[s] = s < ZCfg::NST ? ZCfg::radix(s) : 1;
+            k.zc_twn = ZCfg::TWN;
+            k.zc_threads = ZT::GROUP * NG + 32;
+            k.zc_smem = (size_t)ZT::smem_bytes(NS, NG);
+        }
+    }
     add_fused<T, FFT3D_N>(k);
     return k;
 }

@@ -37,6 +37,10 @@ struct KernelSet {
     int zb_nst, zb_radix[5], zb_twn;   // their factorisation (it may differ from the strided kernels')
     int zb_threads;            // consumer groups + one producer warp
     size_t zb_smem;
+    // C2C row kernels (z pass of the 3D C2C transform): the bulk-pipelined kernel without the Hermitian step
+    const void* zc_fn[2];      // [0 = forward, 1 = inverse (scaled)]
+    int zc_rpt, zc_nst, zc_radix[5], zc_twn, zc_threads;
+    size_t zc_smem;
     // fused z+y kernels of a cubic-like plan (Nz == Ny == N): fft_fused.cuh; null if not compiled
     const void* fz_fn[2];      // [0 = F1+F2, 1 = I2+I3]
     int fz_rpt;                // rows per z tile (Ny must be a multiple)

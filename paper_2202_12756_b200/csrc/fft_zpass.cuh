@@ -143,13 +143,15 @@ __device__ __forceinline__ void hermitian_step(cx<T> (&v)[Cfg::P], cx<T> wt, int
 }
 
 // DIR = -1: R2C (pass F1);  DIR = +1: C2R with normalisation (pass I3)
-template <class Cfg, int RPT, int DIR, typename T, int NSTAGE, int NG>
+// C2C = true: rows of M complex numbers, plain forward / inverse (scaled) transform -- the z pass of the
+// 3D C2C transform; no Hermitian step, so a row's threads need not share a warp
+template <class Cfg, int RPT, int DIR, typename T, int NSTAGE, int NG, bool C2C = false>
 __global__ void __launch_bounds__(Cfg::S * RPT * NG + 32, 1) fft_z_bulk_kernel(const ZBulkArgs a) {
     using C = cx<T>;
     using ZT = ZTile<Cfg, RPT, T>;
     constexpr int P = Cfg::P, S = Cfg::S, M = Cfg::N, GROUP = ZT::GROUP, NCONS = GROUP * NG;
-    static_assert(S <= 32 && (S & (S - 1)) == 0, "a row's threads must sit inside one warp");
-    static_assert(GROUP % 32 == 0 && P % 2 == 0, "group size / even P");
+    static_assert(C2C || (S <= 32 && (S & (S - 1)) == 0), "a row's threads must sit inside one warp");
+    static_assert(GROUP % 32 == 0 && (C2C || P % 2 == 0), "group size / even P");
     extern __shared__ __align__(1024) unsigned char smem_dyn[];
     C* tw = reinterpret_cast<C*>(smem_dyn);
     unsigned char* stages = smem_dyn + ZT::TW_BYTES;
@@ -219,8 +221,11 @@ __global__ void __launch_bounds__(Cfg::S * RPT * NG + 32, 1) fft_z_bulk_kernel(c
     const GroupSync sync{1 + g, GROUP};
     C* scr = scratch + g * (RPT * P) + rr * P;
     // exp(-2 pi i t/Nz), conjugated for the inverse
-    C wt = reinterpret_cast<const C*>(a.twz)[t];
-    if constexpr (DIR > 0) wt.y = -wt.y;
+    C wt = mk<T>((T)1, (T)0);
+    if constexpr (!C2C) {
+        wt = reinterpret_cast<const C*>(a.twz)[t];
+        if constexpr (DIR > 0) wt.y = -wt.y;
+    }
     const T scale = (T)a.scale;
 
     for (long long i = g; i < n_my; i += NG) {
@@ -237,7 +242,7 @@ __global__ void __launch_bounds__(Cfg::S * RPT * NG + 32, 1) fft_z_bulk_kernel(c
 #endif
         C v[P];
         read_own<Cfg, T>(v, buf, t, dense);
-        if constexpr (DIR > 0) {
+        if constexpr (DIR > 0 && !C2C) {
             if (t == 0) {
 #pragma unroll
                 for (int m = 0; m < P; ++m) scr[m] = v[m];
@@ -248,7 +253,7 @@ __global__ void __launch_bounds__(Cfg::S * RPT * NG + 32, 1) fft_z_bulk_kernel(c
         }
         if constexpr (Cfg::NST > 1) sync();                      // all inputs read: slot becomes the exchange buffer
         fft_stages<Cfg, 0, DIR, T>(v, buf, tw, t, padded, sync);
-        if constexpr (DIR < 0) {
+        if constexpr (DIR < 0 && !C2C) {
             if (t == 0) {
 #pragma unroll
                 for (int m = 0; m < P; ++m) scr[m] = v[m];
@@ -256,7 +261,7 @@ __global__ void __launch_bounds__(Cfg::S * RPT * NG + 32, 1) fft_z_bulk_kernel(c
             __syncwarp();
             hermitian_step<Cfg, false, T>(v, wt, t, scr);
             __syncwarp();
-        } else {
+        } else if constexpr (DIR > 0) {
 #pragma unroll
             for (int m = 0; m < P; ++m) v[m] = mk<T>(v[m].x * scale, v[m].y * scale);
         }

@@ -176,6 +176,15 @@ def random_spectrum(shape, dtype=torch.complex64, seed=0, device="cpu") -> torch
     return torch.view_as_complex(flat).reshape(Nx, Ny, Nz // 2 + 1)
 
 
+def complex_grid(shape, dtype=torch.complex64, seed=0, device="cpu") -> torch.Tensor:
+    """i.i.d. complex grid (Nx,Ny,Nz), re and im uniform[-1,1): input of the C2C transform."""
+    Nx, Ny, Nz = shape
+    rdt = torch.float32 if dtype == torch.complex64 else torch.float64
+    flat = _fill((Nx * Ny * Nz, 2), rdt, device,
+                 lambda a, b: 2.0 * _uniform01(a, b, seed, 9, device) - 1.0, chunk=1 << 24)
+    return torch.view_as_complex(flat).reshape(Nx, Ny, Nz)
+
+
 def index_tag_grid(shape, dtype=torch.float64, device="cpu") -> torch.Tensor:
     """Each element carries its own linear index (layout tests)."""
     n = int(np.prod(shape))

@@ -1,0 +1,95 @@
+"""GPU parity of the 3D C2C transform (fft3d_plan_c2c / fft3d_c2c) against the fp64 CPU
+oracle, through the C ABI.  Tolerances as for R2C/C2R: rel-L2 <= 2e-6*log2(NxNyNz) (fp32), 1e-13*log2 (fp64)."""
+import math
+
+import numpy as np
+import pytest
+import torch
+
+pytestmark = pytest.mark.gpu
+
+
+def tol(shape, dtype):
+    n = shape[0] * shape[1] * shape[2]
+    return (2e-6 if dtype == torch.float32 else 1e-13) * math.log2(n)
+
+
+def rel_l2(a, b):
+    return float(np.linalg.norm((np.asarray(a) - np.asarray(b)).ravel()) / np.linalg.norm(np.asarray(b).ravel()))
+
+
+@pytest.fixture(scope="module")
+def fft():
+    import paper_2202_12756_b200 as m
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    m.load_library()
+    return m
+
+
+CASES = [
+    ((32, 32, 128), 4),
+    ((16, 64, 256), 8),
+    ((64, 16, 192), 2),          # radix-3 rows
+    ((48, 96, 384), 3),
+    ((128, 128, 128), 8),
+    ((32, 256, 1024), 16),       # 64 KiB row tiles; y pass through the TMA kernels
+    ((8, 64, 1536), 1),          # rows whose threads span two warps (no Hermitian step, so allowed)
+]
+
+
+@pytest.mark.parametrize("shape,p", CASES)
+@pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
+def test_c2c_matches_oracle(fft, oracle_mod, shape, p, dtype):
+    from paper_2202_12756_b200 import inputs
+    try:
+        plan = fft.PlanC2C(*shape, dtype=dtype, virtual_slabs=p)
+    except fft.Fft3dError as e:
+        assert e.status == 2
+        pytest.skip("no C2C row kernel for %s %s" % (shape, dtype))
+    cd = plan.complex_dtype
+    f = inputs.complex_grid(shape, cd, seed=11)
+    d_in = f.cuda().reshape(-1)
+    keep = d_in.clone()
+    out = plan.c2c(d_in, -1)
+    torch.cuda.synchronize()
+    assert torch.equal(torch.view_as_real(d_in), torch.view_as_real(keep)), "input must be preserved"
+    F_gpu = plan.to_natural(out).cpu().numpy().astype(np.complex128)
+    F_ref = oracle_mod.c2c(f.to(torch.complex128).numpy(), -1)
+    assert rel_l2(F_gpu, F_ref) <= tol(shape, dtype)
+    # slab layout == fft3d_index
+    flat = out.cpu().numpy()
+    rng = np.random.Generator(np.random.PCG64(2))
+    for _ in range(32):
+        kx, ky, kz = (int(rng.integers(0, n)) for n in shape)
+        off = plan.index(kx, ky, kz)
+        L = shape[1] // p
+        assert off == (((ky // L) * shape[0] + kx) * L + ky % L) * shape[2] + kz
+        assert flat[off] == F_gpu[kx, ky, kz].astype(flat.dtype)
+    assert plan.index(0, 0, shape[2]) == -1
+    # inverse of an unrelated field, then the round trip
+    g = inputs.complex_grid(shape, cd, seed=12)
+    g_ref = oracle_mod.c2c(g.to(torch.complex128).numpy(), +1)
+    g_gpu = plan.c2c(plan.from_natural(g.cuda()), +1).reshape(shape).cpu().numpy().astype(np.complex128)
+    assert rel_l2(g_gpu, g_ref) <= tol(shape, dtype)
+    back = plan.c2c(out, +1).reshape(shape).cpu()
+    err = (back - f).abs().max().item() / f.abs().max().item()
+    assert err <= tol(shape, dtype)
+    assert plan.launch_names(0) == ("z_c2c_fwd", "y_c2c_fwd", "x_c2c_fwd")
+    assert plan.launch_names(1) == ("x_c2c_inv", "y_c2c_inv", "z_c2c_inv")
+    plan.close()
+
+
+def test_plan_kinds_do_not_mix(fft):
+    c = fft.PlanC2C(32, 32, 128, dtype=torch.float32, virtual_slabs=2)
+    r = fft.Plan(32, 32, 128, dtype=torch.float32, virtual_slabs=2)
+    x = torch.zeros(32 * 32 * 128, dtype=torch.complex64, device="cuda")
+    with pytest.raises(fft.Fft3dError):
+        fft.PlanC2C.c2c(r, torch.zeros(r.n_complex, dtype=torch.complex64, device="cuda"), -1)
+    lib = fft.load_library()
+    w = c.empty_workspace("cuda")
+    assert lib.fft3d_r2c(c._h, x.data_ptr(), x.data_ptr(), w.data_ptr(), None) == 1      # FFT3D_EINVAL
+    assert lib.fft3d_c2c(c._h, x.data_ptr(), x.data_ptr(), w.data_ptr(), -1, None) == 1  # in == out rejected
+    assert lib.fft3d_c2c(c._h, x.data_ptr(), w.data_ptr(), w.data_ptr(), 0, None) == 1   # bad direction
+    with pytest.raises(fft.Fft3dError):
+        fft.PlanC2C(32, 32, 16, dtype=torch.float32, virtual_slabs=2)                     # rows too short: unsupported
+    c.close(); r.close()
