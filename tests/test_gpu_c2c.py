@@ -93,3 +93,52 @@ def test_plan_kinds_do_not_mix(fft):
     with pytest.raises(fft.Fft3dError):
         fft.PlanC2C(32, 32, 16, dtype=torch.float32, virtual_slabs=2)                     # rows too short: unsupported
     c.close(); r.close()
+
+
+def test_c2c_512_full_oracle_and_1024_properties(fft, oracle_mod):
+    """512^3 fp32 against the full fp64 oracle; 1024^3 fp32 (8 GiB per array) by properties that hold at any
+    size: a sum of plane waves gives exactly those spikes (closed form), Parseval, round trip."""
+    from paper_2202_12756_b200 import inputs
+    shape, p = (512, 512, 512), 8
+    plan = fft.PlanC2C(*shape, dtype=torch.float32, virtual_slabs=p)
+    f = inputs.complex_grid(shape, torch.complex64, seed=21)
+    out = plan.c2c(f.cuda().reshape(-1), -1)
+    F_gpu = plan.to_natural(out).cpu().numpy()
+    F_ref = oracle_mod.c2c(f.to(torch.complex128).numpy(), -1)
+    num = np.linalg.norm((F_gpu - F_ref).ravel())
+    assert num / np.linalg.norm(F_ref.ravel()) <= tol(shape, torch.float32)
+    del F_ref, F_gpu, out
+    plan.close()
+
+    n = 1024
+    shape = (n, n, n)
+    plan = fft.PlanC2C(*shape, dtype=torch.float32, virtual_slabs=64)
+    modes = [((3, 1000, 17), 1.5 - 0.5j), ((512, 0, 1023), -0.75 + 2.0j), ((77, 301, 640), 0.25 + 0.125j)]
+    ax = torch.arange(n, device="cuda", dtype=torch.float64)
+    f = torch.zeros(shape, dtype=torch.complex64, device="cuda")
+    for (kx, ky, kz), amp in modes:                       # separable phases built in fp64, rounded once
+        ex = torch.exp(2j * math.pi * ((ax * kx) % n) / n)
+        ey = torch.exp(2j * math.pi * ((ax * ky) % n) / n)
+        ez = torch.exp(2j * math.pi * ((ax * kz) % n) / n)
+        for x0 in range(0, n, 128):
+            blk = amp * ex[x0:x0 + 128, None, None] * ey[None, :, None] * ez[None, None, :]
+            f[x0:x0 + 128] += blk.to(torch.complex64)
+    work = plan.empty_workspace("cuda")
+    out = plan.c2c(f.reshape(-1), -1, work=work)
+    energy_in = sum((f[i].abs().double() ** 2).sum().item() for i in range(n))
+    energy_out = sum((out[i * n * n:(i + 1) * n * n].abs().double() ** 2).sum().item() for i in range(n))
+    assert abs(energy_out / n ** 3 - energy_in) <= 1e-5 * energy_in
+    peak = 0.0
+    for (kx, ky, kz), amp in modes:
+        got = out[plan.index(kx, ky, kz)].item()
+        assert abs(got - amp * n ** 3) <= 2e-5 * abs(amp) * n ** 3
+        peak = max(peak, abs(amp) * n ** 3)
+        out[plan.index(kx, ky, kz)] = 0
+    rest = max(out[i * n * n:(i + 1) * n * n].abs().max().item() for i in range(n))
+    assert rest <= 2e-5 * peak                             # everything else is rounding noise
+    for (kx, ky, kz), amp in modes:
+        out[plan.index(kx, ky, kz)] = amp * n ** 3
+    back = plan.c2c(out, +1, work=work).reshape(shape)
+    err = max((back[i] - f[i]).abs().max().item() for i in range(n))
+    assert err <= tol(shape, torch.float32) * 2.6
+    plan.close()
