@@ -76,6 +76,7 @@ struct fft3d_plan_s {
     // TMA-pipelined strided passes
     void* encode_fn;           // cuTensorMapEncodeTiled, resolved at run time (no libcuda link dependency)
     bool tma_y, tma_x;         // usable for this plan's extents / alignment
+    bool tma_xc;               // C2C plans: TMA-pipelined x pass usable
     bool bulk_z;               // bulk-pipelined z kernels usable (row count a multiple of the tile)
     int y_rows_nat, y_rows_slab, x_rows;   // rows per TMA box
     // fused z+y passes (fft_fused.cuh): the workspace is [slab array | ring | side | flags]
@@ -222,8 +223,8 @@ bool map_slab_x(const fft3d_plan_s* pl, TensorMapBlob* m, const void* base, int 
     int b[4] = {(int)(tc * W), 1, rows, 1};
     return make_map(pl, m, base, 4, d, st, b);
 }
-bool map_user_x(const fft3d_plan_s* pl, TensorMapBlob* m, const void* base, int tc, int rows) {    // [p][Nx][L*(M+1)], rows along x
-    const long long sz = 2 * pl->esize, W = sz / 8, L = pl->L, Mp1 = pl->M + 1;
+bool map_user_x(const fft3d_plan_s* pl, TensorMapBlob* m, const void* base, int tc, int rows, long long pitch = 0) {    // [p][Nx][L*pitch], rows along x
+    const long long sz = 2 * pl->esize, W = sz / 8, L = pl->L, Mp1 = pitch > 0 ? pitch : pl->M + 1;
     long long d[3] = {L * Mp1 * W, pl->Nx, pl->p}, st[2] = {L * Mp1 * sz, pl->Nx * L * Mp1 * sz};
     int b[3] = {(int)(tc * W), rows, 1};
     return make_map(pl, m, base, 3, d, st, b);
@@ -343,6 +344,7 @@ static int plan_create(fft3d_plan_t** out, long long Nx, long long Ny, long long
         rc = upload_stage_twiddles(kz->zb_nst, kz->zb_radix, kz->zb_twn, pl->esize, &pl->tw_zb);
     if (rc == FFT3D_OK && kind == 0) rc = upload_z_twiddles(Nz, pl->M, pl->esize, &pl->twz);
     if (rc == FFT3D_OK && kind == 1) {
+        pl->x_rows = (int)largest_divisor_le(Nx, 256);
         rc = upload_stage_twiddles(kz->zc_nst, kz->zc_radix, kz->zc_twn, pl->esize, &pl->tw_zc);
         for (int d = 0; d < 2 && rc == FFT3D_OK; ++d) {
             int g = 0;
@@ -374,6 +376,13 @@ static int plan_create(fft3d_plan_t** out, long long Nx, long long Ny, long long
             for (int d = 0; d < 2 && rc == FFT3D_OK; ++d) {
                 int g = 0;
                 rc = prepare_kernel(ky->tma_fn[d == 0 ? TMA_Y_FWD : TMA_Y_INV], ky->tma_threads, ky->tma_smem_y, sms, &g);
+            }
+        }
+        if (rc == FFT3D_OK && kind == 1 && fn != nullptr && strides_ok && kx->xc_fn[0] != nullptr && M % kx->tma_tc_x == 0) {
+            pl->tma_xc = true;
+            for (int d = 0; d < 2 && rc == FFT3D_OK; ++d) {
+                int g = 0;
+                rc = prepare_kernel(kx->xc_fn[d], kx->tma_threads_x, kx->xc_smem, sms, &g);
             }
         }
         if (rc == FFT3D_OK && kind == 0 && fn != nullptr && strides_ok && kx->tma_fn[TMA_X_FWD] != nullptr && M % kx->tma_tc_x == 0 &&
@@ -750,6 +759,19 @@ int fft3d_c2c(const fft3d_plan_t* pl, const void* d_in, void* d_out, void* d_wor
         return launch(ky->s_fn[1][KIND_SLAB_LIN], a.ntiles, pl->grid_y[1], ky->s_threads, ky->s_smem, &a, st);
     };
     auto x_pass = [&](const void* in, void* out) -> int {       // lines along x inside every virtual slab, pitch M
+        if (tma_on && pl->tma_xc) {
+            // X_FWD reads the 4-D slab view and writes the flattened one, X_INV the other way round; with one
+            // pitch M on both sides the two views describe the same layout
+            TensorMapBlob mi, mo;
+            const int tc = kx->tma_tc_x;
+            bool ok = d == 0 ? (map_slab_x(pl, &mi, in, tc, pl->x_rows) && map_user_x(pl, &mo, out, tc, pl->x_rows, M))
+                             : (map_user_x(pl, &mi, in, tc, pl->x_rows, M) && map_slab_x(pl, &mo, out, tc, pl->x_rows));
+            if (!ok) return FFT3D_ECUDA;
+            TmaArgs ta{};
+            ta.tw = pl->tw_x; ta.ntz = (int)(M / tc); ta.ntiles = (long long)p * L * ta.ntz;
+            ta.L = (int)L; ta.Nx = (int)Nx; ta.Mp1 = (int)M; ta.in_rows = pl->x_rows; ta.out_rows = pl->x_rows;
+            return launch_tma(kx->xc_fn[d], kx->tma_threads_x, kx->xc_smem, pl->num_sms, mi, mi, mo, ta, st);
+        }
         StridedArgs b{};
         b.in = in; b.out = out; b.col0 = nullptr; b.tw = pl->tw_x;
         b.ntz = (int)((M + kx->tc - 1) / kx->tc); b.ncols = (int)M; b.a_lo = (int)L; b.L = (int)Nx;

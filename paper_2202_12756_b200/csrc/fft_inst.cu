@@ -110,6 +110,15 @@ static KernelSet make_set(int dtype) {
             k.tma_fn[TMA_X_INV] = (const void*)fft_strided_tma_kernel<Cfg, TTCX, TMA_X_INV, T, NSX, OF>;
             k.tma_smem_x = (size_t)TX::smem_bytes(NSX);
         }
+        {   // C2C plans: both sides of the x pass have pitch Nz (aligned rows): the plain windows
+            using TXC = TmaTile<Cfg, TTCX, T, false>;
+            constexpr int NSC = TXC::max_stages();
+            if constexpr (NSC >= 1) {
+                k.xc_fn[0] = (const void*)fft_strided_tma_kernel<Cfg, TTCX, TMA_X_FWD, T, NSC, false>;
+                k.xc_fn[1] = (const void*)fft_strided_tma_kernel<Cfg, TTCX, TMA_X_INV, T, NSC, false>;
+                k.xc_smem = (size_t)TXC::smem_bytes(NSC);
+            }
+        }
         k.tma_oddfix = OF ? 1 : 0;
         k.tma_tc = TTC;
         k.tma_threads = TY::NCONS + 32;

@@ -37,6 +37,9 @@ struct KernelSet {
     int zb_nst, zb_radix[5], zb_twn;   // their factorisation (it may differ from the strided kernels')
     int zb_threads;            // consumer groups + one producer warp
     size_t zb_smem;
+    // TMA-pipelined X kernels for layouts whose two sides share one aligned pitch (C2C plans): no shifted windows
+    const void* xc_fn[2];      // [0 = X_FWD, 1 = X_INV]
+    size_t xc_smem;
     // C2C row kernels (z pass of the 3D C2C transform): the bulk-pipelined kernel without the Hermitian step
     const void* zc_fn[2];      // [0 = forward, 1 = inverse (scaled)]
     int zc_rpt, zc_nst, zc_radix[5], zc_twn, zc_threads;
