@@ -362,6 +362,77 @@ def run_cuda(args):
         dist.destroy_process_group()
 
 
+# ------------------------------------------------------------------------------------------
+# CUDA arm, 3D C2C transform (--transform c2c; single GPU, the widening row SURVEY.md 8(f)-3)
+# ------------------------------------------------------------------------------------------
+def run_cuda_c2c(args):
+    import torch
+    import paper_2202_12756_b200 as pkg
+    from paper_2202_12756_b200 import inputs
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the FFT path has no CPU fallback")
+    torch.cuda.set_device(0)
+    n, p = args.n, args.slabs
+    shape = (n, n, n)
+    plan = pkg.PlanC2C(*shape, dtype=torch.float32, virtual_slabs=p)
+    f = inputs.complex_grid(shape, torch.complex64, seed=0, device="cuda").reshape(-1)
+    spec, back, work = plan.empty_complex("cuda"), plan.empty_complex("cuda"), plan.empty_workspace("cuda")
+    stream = torch.cuda.current_stream()
+
+    def step():
+        plan.c2c(f, -1, spec, work, stream)
+        plan.c2c(spec, +1, back, work, stream)
+
+    for _ in range(args.warmup):
+        step()
+    torch.cuda.synchronize()
+    plan.timing_enable(args.steps)
+    sampler = ClockSampler(0)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(args.steps):
+        step()
+    e1.record(stream)
+    torch.cuda.synchronize()
+    ms_step = e0.elapsed_time(e1) / args.steps
+    clocks = sampler.stop()
+    per_kernel = {}
+    for which in (0, 1):
+        d, calls = plan.timing_read(which)
+        per_kernel.update({k: v / max(1, calls) for k, v in d.items()})
+    plan.timing_enable(0)
+    rt_err = max((back[i:i + (1 << 26)] - f[i:i + (1 << 26)]).abs().max().item() for i in range(0, n ** 3, 1 << 26))
+    tol = 2e-6 * math.log2(n ** 3) * 2.6          # |f| <= sqrt(2), components uniform[-1,1)
+    pass_b = 2 * plan.complex_bytes              # one read + one write of the complex array
+    dom = max(per_kernel, key=per_kernel.get)
+    peak, peak_src = measured_peak()
+    achieved = pass_b / (per_kernel[dom] * 1e-3) / 1e9
+    flops = 2 * 5.0 * n ** 3 * math.log2(n ** 3)  # 5 N log2 N per complex transform, two transforms
+    line = {
+        "metric": "GFLOP/s per 3D C2C forward+inverse pair (10*N^3*log2(N^3) flop per pair), fp32",
+        "value": flops / (ms_step * 1e-3) / 1e9, "unit": "GFLOP/s", "n_gpus": 1, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": "%d^3 complex64 grid, re/im i.i.d. uniform[-1,1), C2C forward+inverse pair, "
+                               "virtual_slabs=%d" % (n, p),
+                   "l2": "arrays (%.1f GiB each) are far larger than the 126 MB L2; no flush needed"
+                         % (plan.complex_bytes / 2 ** 30),
+                   "round_trip_max_abs_err": rt_err, "round_trip_bound": tol},
+        "clocks": clocks, "e2e": None,
+        "gpu_launches": args.steps * (plan.launches(0) + plan.launches(1)),
+        "roofline": {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
+                     "frac": achieved / peak, "traffic": stored_traffic("c2c:" + dom), "peak_source": peak_src,
+                     "algorithmic_bytes": pass_b, "ms_per_launch": per_kernel[dom], "all_kernels_ms": per_kernel,
+                     "array_passes_per_pair": 6,
+                     "pair_frac_of_pass_roofline": (6 * pass_b / peak / 1e9) / (ms_step * 1e-3)},
+        "cpu_baseline": None,
+    }
+    print(json.dumps(line), flush=True)
+    if not (rt_err <= tol):
+        raise SystemExit("round trip error %.3e exceeds %.3e: the timed path is wrong" % (rt_err, tol))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -373,10 +444,14 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--transform", default="r2c", choices=["r2c", "c2c"],
+                    help="r2c (default): the headline R2C+C2R pair; c2c: the 3D C2C pair (single GPU, no e2e leg)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "cuda" else args.warmup
     if args.impl == "reference":
         run_reference(args)
+    elif args.transform == "c2c":
+        run_cuda_c2c(args)
     else:
         run_cuda(args)
 
