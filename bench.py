@@ -424,8 +424,9 @@ def run_cuda_c2c(args):
         "roofline": {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
                      "frac": achieved / peak, "traffic": stored_traffic("c2c:" + dom), "peak_source": peak_src,
                      "algorithmic_bytes": pass_b, "ms_per_launch": per_kernel[dom], "all_kernels_ms": per_kernel,
-                     "array_passes_per_pair": 6,
-                     "pair_frac_of_pass_roofline": (6 * pass_b / peak / 1e9) / (ms_step * 1e-3)},
+                     "array_passes_per_pair": len(per_kernel),
+                     "pair_frac_of_pass_roofline": (len(per_kernel) * pass_b / peak / 1e9) / (ms_step * 1e-3),
+                     "pair_frac_of_6pass_roofline": (6 * pass_b / peak / 1e9) / (ms_step * 1e-3)},
         "cpu_baseline": None,
     }
     print(json.dumps(line), flush=True)

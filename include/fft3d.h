@@ -115,7 +115,8 @@ int fft3d_c2r(const fft3d_plan_t *plan, const void *d_cplx_in, void *d_real_out,
  * fft3d_real_bytes = 0, fft3d_index(kx,ky,kz) = ((q*Nx + kx)*(Ny/p) + ky % (Ny/p))*Nz + kz.
  * fft3d_c2c: direction -1 = forward, unnormalised, d_in natural [Nx][Ny][Nz] -> d_out in the slab layout
  * [p][Nx][Ny/p][Nz]; direction +1 = inverse scaled by 1/(NxNyNz), slab layout -> natural.  Three full-array
- * passes (z rows, y lines with the slab permutation, x lines).  d_out is also used as scratch; d_in is
+ * passes (z rows, y lines with the slab permutation, x lines), or two where the z and y passes run fused
+ * (Nz == Ny; fft3d_set_variant applies as for R2C plans).  d_out is also used as scratch; d_in is
  * preserved; all pointers 16-byte aligned device pointers, no overlap; asynchronous on the stream.
  * fft3d_r2c / fft3d_c2r reject a C2C plan with FFT3D_EINVAL and vice versa. */
 int fft3d_plan_c2c(fft3d_plan_t **plan_out, long long Nx, long long Ny, long long Nz,
@@ -135,7 +136,8 @@ int fft3d_c2r_host(fft3d_plan_t *plan, const void *h_cplx_in, void *h_real_out);
  * column 0 of the inverse x pass, TMA path only), "y_c2c_inv", "z_c2r", and -- when the z and y
  * passes of a plane run as one kernel through an L2-resident ring --
  * "zy_r2c_fused" (paper step 1 + steps 2-4) and "yz_c2r_fused" (their reverse); C2C plans:
- * "z_c2c_fwd", "y_c2c_fwd", "x_c2c_fwd" (which = 0) and "x_c2c_inv", "y_c2c_inv", "z_c2c_inv" (which = 1). */
+ * "z_c2c_fwd", "y_c2c_fwd", "x_c2c_fwd" (which = 0) and "x_c2c_inv", "y_c2c_inv", "z_c2c_inv" (which = 1), or
+ * "zy_c2c_fused_fwd", "x_c2c_fwd" and "x_c2c_inv", "yz_c2c_fused_inv" when fused. */
 int fft3d_launches(const fft3d_plan_t *plan, int which);
 const char *fft3d_launch_name(const fft3d_plan_t *plan, int which, int i);
 

@@ -255,21 +255,26 @@ int launch_zbulk(const fft3d_plan_s* pl, int d, const void* in, void* out, doubl
 // F1+F2 (d = 0: real `in` -> slab array) or I2+I3 (d = 1: slab array -> real `out`) as one cooperative launch
 int launch_fused(const fft3d_plan_s* pl, int d, const void* in, void* out, void* slab, void* d_work, cudaStream_t st) {
     const KernelSet* ky = pl->ky;
+    const bool c2c = pl->kind == 1;
+    const void* fn = c2c ? ky->fc_fn[d] : ky->fz_fn[d];
+    const int f_tc = c2c ? ky->fc_tc : ky->fz_tc, f_rpt = c2c ? ky->fc_rpt : ky->fz_rpt;
+    const int f_threads = c2c ? ky->fc_threads : ky->fz_threads;
+    const size_t f_smem = c2c ? ky->fc_smem : ky->fz_smem;
     unsigned char* w = reinterpret_cast<unsigned char*>(d_work);
     void* ring = w + pl->slab_bytes;
     unsigned* flags = reinterpret_cast<unsigned*>(w + pl->slab_bytes + pl->ring_bytes + pl->side_bytes);
     if (cudaMemsetAsync(flags, 0, pl->flags_bytes, st) != cudaSuccess) { cudaGetLastError(); return FFT3D_ECUDA; }
     TensorMapBlob ring_map, slab_map;
     {   // the ring as [R][M/TC][Ny][TC]; a z tile is the box (TC, M/TC, RPT, 1)
-        const long long sz = 2 * pl->esize, W = sz / 8, tc = ky->fz_tc, nb = pl->M / tc;
+        const long long sz = 2 * pl->esize, W = sz / 8, tc = f_tc, nb = pl->M / tc;
         long long dm[4] = {tc * W, nb, pl->Ny, pl->fz_R};
         long long sb[3] = {pl->Ny * tc * sz, tc * sz, pl->Ny * pl->M * sz};
-        int bx[4] = {(int)(tc * W), (int)nb, ky->fz_rpt, 1};
+        int bx[4] = {(int)(tc * W), (int)nb, f_rpt, 1};
         if (!make_map(pl, &ring_map, ring, 4, dm, sb, bx)) return FFT3D_ECUDA;
     }
-    if (!map_slab_y(pl, &slab_map, slab, ky->fz_tc, pl->y_rows_slab)) return FFT3D_ECUDA;
+    if (!map_slab_y(pl, &slab_map, slab, f_tc, pl->y_rows_slab)) return FFT3D_ECUDA;
     FusedArgs a{};
-    a.in = in; a.out = out; a.ring = ring; a.tw_z = pl->tw_zb; a.twz = pl->twz; a.tw_y = pl->tw_y; a.flags = flags;
+    a.in = in; a.out = out; a.ring = ring; a.tw_z = c2c ? pl->tw_zc : pl->tw_zb; a.twz = pl->twz; a.tw_y = pl->tw_y; a.flags = flags;
     a.Nx = (int)pl->Nx; a.Ny = (int)pl->Ny; a.L = (int)pl->L; a.R = pl->fz_R; a.kz = pl->fz_kz[d];
     a.rows_slab = pl->y_rows_slab;
     a.scale = 1.0 / ((double)pl->Nx * (double)pl->Ny * (double)pl->Nz);
@@ -277,8 +282,7 @@ int launch_fused(const fft3d_plan_s* pl, int d, const void* in, void* out, void*
     if (const char* e = getenv("FFT3D_FZ_KZ")) a.kz = atoi(e);
 #endif
     void* argv[3] = {(void*)&ring_map, (void*)&slab_map, (void*)&a};
-    cudaError_t e = cudaLaunchCooperativeKernel(ky->fz_fn[d], dim3((unsigned)pl->num_sms), dim3((unsigned)ky->fz_threads),
-                                                argv, ky->fz_smem, st);
+    cudaError_t e = cudaLaunchCooperativeKernel(fn, dim3((unsigned)pl->num_sms), dim3((unsigned)f_threads), argv, f_smem, st);
     if (e != cudaSuccess) { cudaGetLastError(); return FFT3D_ECUDA; }
     return FFT3D_OK;
 }
@@ -436,6 +440,29 @@ static int plan_create(fft3d_plan_t** out, long long Nx, long long Ny, long long
             }
         }
     }
+    // C2C plans: the same fused pipeline over rows of Nz complex points (Nz == Ny)
+    if (rc == FFT3D_OK && kind == 1 && pl->tma_y && ky->fc_fn[0] != nullptr && Nz == Ny && ky->fc_tc == ky->tma_tc &&
+        Ny % ky->fc_rpt == 0 && pl->M % ky->fc_tc == 0 && pl->M / ky->fc_tc <= 256 && kz->zc_fn[0] != nullptr) {
+        const size_t plane = (size_t)Ny * pl->M * 2 * pl->esize;
+        int R = (int)(((size_t)48 << 20) / plane);
+        if (R > 8) R = 8;
+        int coop = 0;
+        cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
+        if (R >= 2 && Nx >= R && coop) {
+            bool ok = true;
+            for (int d = 0; d < 2 && ok; ++d) {
+                int g = 0;
+                ok = prepare_kernel(ky->fc_fn[d], ky->fc_threads, ky->fc_smem, sms, &g) == FFT3D_OK && g >= sms;
+            }
+            if (ok) {
+                pl->fused = true; pl->fz_R = R;
+                pl->fz_kz[0] = pl->fz_kz[1] = (sms / 2 + 1) & ~1;      // z and y tiles cost about the same here
+                pl->fused_default = pl->slab_bytes >= ((size_t)2 << 30);
+                pl->ring_bytes = plane * R;
+                pl->flags_bytes = ((size_t)2 * Nx * sizeof(unsigned) + 255) & ~(size_t)255;
+            }
+        }
+    }
     if (rc != FFT3D_OK) { fft3d_destroy(pl); return rc; }
     *out = pl;
     return FFT3D_OK;
@@ -474,7 +501,7 @@ static bool use_tma(const fft3d_plan_t* pl) { return pl->variant != 1; }
 
 int fft3d_launches(const fft3d_plan_t* pl, int which) {
     if (pl == nullptr || which < 0 || which > 1) return 0;
-    if (pl->kind == 1) return 3;
+    if (pl->kind == 1) return use_fused(pl) ? 2 : 3;
     // c2r on the TMA path runs the packed column 0 of the x pass as a separate small kernel
     int n = (which == 1 && use_tma(pl) && pl->tma_x) ? 5 : 4;
     return use_fused(pl) ? n - 1 : n;
@@ -485,6 +512,9 @@ const char* fft3d_launch_name(const fft3d_plan_t* pl, int which, int i) {
     if (pl->kind == 1) {
         static const char* const cf[] = {"z_c2c_fwd", "y_c2c_fwd", "x_c2c_fwd"};
         static const char* const ci[] = {"x_c2c_inv", "y_c2c_inv", "z_c2c_inv"};
+        static const char* const ff[] = {"zy_c2c_fused_fwd", "x_c2c_fwd"};
+        static const char* const fi[] = {"x_c2c_inv", "yz_c2c_fused_inv"};
+        if (use_fused(pl)) return which == 0 ? ff[i] : fi[i];
         return which == 0 ? cf[i] : ci[i];
     }
     const bool fz = use_fused(pl);
@@ -781,6 +811,16 @@ int fft3d_c2c(const fft3d_plan_t* pl, const void* d_in, void* d_out, void* d_wor
         return launch(kx->s_fn[d][KIND_LIN_LIN], b.ntiles, pl->grid_x[d], kx->s_threads, kx->s_smem, &b, st);
     };
 
+    if (use_fused(pl)) {
+        if (d == 0) {
+            rc = launch_fused(pl, 0, d_in, nullptr, d_work, d_work, st);   rec.mark(slot++); if (rc != FFT3D_OK) return rc;
+            rc = x_pass(d_work, d_out);                                    rec.mark(slot++);
+        } else {
+            rc = x_pass(d_in, d_work);                                     rec.mark(slot++); if (rc != FFT3D_OK) return rc;
+            rc = launch_fused(pl, 1, nullptr, d_out, d_work, d_work, st);  rec.mark(slot++);
+        }
+        return rc;
+    }
     if (d == 0) {
         rc = z_pass(d_in, d_out);           rec.mark(slot++); if (rc != FFT3D_OK) return rc;
         rc = y_pass(d_out, d_work);         rec.mark(slot++); if (rc != FFT3D_OK) return rc;

@@ -155,7 +155,8 @@ struct FusedTile {
 
 struct FItem { int p1, x, j; };
 
-template <class ZCfg, int RPT, class YCfg, int TC, int DIR, typename T, int NSTAGE, int NG_>
+// C2C = true: the rows are Nz complex numbers and the z tiles run the plain C2C transform (3D C2C plans)
+template <class ZCfg, int RPT, class YCfg, int TC, int DIR, typename T, int NSTAGE, int NG_, bool C2C = false>
 __global__ void __launch_bounds__((FusedTile<ZCfg, RPT, YCfg, TC, T, NG_>::THREADS), 1)
 fft_zy_fused_kernel(const __grid_constant__ TensorMapBlob ring_map, const __grid_constant__ TensorMapBlob slab_map,
                     const FusedArgs a) {
@@ -167,7 +168,7 @@ fft_zy_fused_kernel(const __grid_constant__ TensorMapBlob ring_map, const __grid
     constexpr int M = ZCfg::N, NY = YCfg::N;
     constexpr bool FWD = DIR < 0;
     static_assert(FT::OK, "z tile and y tile must use the same number of consumer threads");
-    static_assert(ZCfg::S <= 32 && (ZCfg::S & (ZCfg::S - 1)) == 0, "a row's threads must sit inside one warp");
+    static_assert(C2C || (ZCfg::S <= 32 && (ZCfg::S & (ZCfg::S - 1)) == 0), "a row's threads must sit inside one warp");
 
     extern __shared__ __align__(1024) unsigned char smem_dyn[];
     C* twz_s = reinterpret_cast<C*>(smem_dyn);                                   // z stage twiddles
@@ -336,8 +337,11 @@ fft_zy_fused_kernel(const __grid_constant__ TensorMapBlob ring_map, const __grid
     const SmLayout<1, 0> z_dense{rr * M};
     const SmLayout<1, ZT::PADR> z_padded{rr * ZT::PITCH};
     C* scr = scratch + gq * (RPT * ZCfg::P) + rr * ZCfg::P;
-    C wt = reinterpret_cast<const C*>(a.twz)[tz];        // exp(-2 pi i t/Nz), conjugated for the inverse
-    if constexpr (DIR > 0) wt.y = -wt.y;
+    C wt = mk<T>((T)1, (T)0);                            // exp(-2 pi i t/Nz), conjugated for the inverse
+    if constexpr (!C2C) {
+        wt = reinterpret_cast<const C*>(a.twz)[tz];
+        if constexpr (DIR > 0) wt.y = -wt.y;
+    }
     const T scale = (T)a.scale;
     // y-tile role: thread ty of column cc
     const int cc = gt % TC, ty = gt / TC;
@@ -366,7 +370,7 @@ fft_zy_fused_kernel(const __grid_constant__ TensorMapBlob ring_map, const __grid
             constexpr int P = ZCfg::P;
             C v[P];
             read_own<ZCfg, T>(v, buf, tz, z_dense);
-            if constexpr (DIR > 0) {
+            if constexpr (DIR > 0 && !C2C) {
                 if (tz == 0) {
 #pragma unroll
                     for (int m = 0; m < P; ++m) scr[m] = v[m];
@@ -377,7 +381,7 @@ fft_zy_fused_kernel(const __grid_constant__ TensorMapBlob ring_map, const __grid
             }
             if constexpr (ZCfg::NST > 1) sync();
             fft_stages<ZCfg, 0, DIR, T>(v, buf, twz_s, tz, z_padded, sync);
-            if constexpr (DIR < 0) {
+            if constexpr (DIR < 0 && !C2C) {
                 if (tz == 0) {
 #pragma unroll
                     for (int m = 0; m < P; ++m) scr[m] = v[m];
@@ -385,7 +389,7 @@ fft_zy_fused_kernel(const __grid_constant__ TensorMapBlob ring_map, const __grid
                 __syncwarp();
                 hermitian_step<ZCfg, false, T>(v, wt, tz, scr);
                 __syncwarp();
-            } else {
+            } else if constexpr (DIR > 0) {
 #pragma unroll
                 for (int m = 0; m < P; ++m) v[m] = mk<T>(v[m].x * scale, v[m].y * scale);
             }

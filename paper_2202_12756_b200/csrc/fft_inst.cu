@@ -44,6 +44,30 @@ static void add_fused(KernelSet& k) {
     }
 }
 
+// fused z+y kernels of C2C plans with Nz == Ny == N
+template <typename T, int N>
+static void add_fused_c2c(KernelSet& k) {
+    if constexpr (N >= 128) {
+        using C = cx<T>;
+        using YCfg = typename CfgFor<T, N>::type;
+        using ZCfg = typename ZCfgFor<T, N>::type;
+        constexpr int TTC = tma_tile_cols(YCfg::N, YCfg::S, (int)sizeof(C));
+        if constexpr (TTC > 0 && (YCfg::S * TTC) % ZCfg::S == 0 && ZCfg::S <= YCfg::S * TTC) {
+            constexpr int RPT = YCfg::S * TTC / ZCfg::S;
+            constexpr int GROUP = YCfg::S * TTC;
+            constexpr int NG = (2 * GROUP + 128 <= 1024 && FusedTile<ZCfg, RPT, YCfg, TTC, T, 2>::max_stages() >= 3) ? 2 : 1;
+            using FT = FusedTile<ZCfg, RPT, YCfg, TTC, T, NG>;
+            constexpr int NS = FT::max_stages();
+            if constexpr (FT::OK && NS >= 3 && NG >= 2 && FT::THREADS <= 1024) {      // only where fusion can win
+                k.fc_fn[0] = (const void*)fft_zy_fused_kernel<ZCfg, RPT, YCfg, TTC, -1, T, NS, NG, true>;
+                k.fc_fn[1] = (const void*)fft_zy_fused_kernel<ZCfg, RPT, YCfg, TTC, +1, T, NS, NG, true>;
+                k.fc_rpt = RPT; k.fc_tc = TTC; k.fc_threads = FT::THREADS; k.fc_smem = (size_t)FT::smem_bytes(NS);
+                k.fc_ng = NG; k.fc_nstage = NS;
+            }
+        }
+    }
+}
+
 template <typename T>
 static KernelSet make_set(int dtype) {
     using Cfg = typename CfgFor<T, FFT3D_N>::type;
@@ -162,6 +186,7 @@ static KernelSet make_set(int dtype) {
         }
     }
     add_fused<T, FFT3D_N>(k);
+    add_fused_c2c<T, FFT3D_N>(k);
     return k;
 }
 

@@ -51,6 +51,10 @@ struct KernelSet {
     int fz_threads;
     size_t fz_smem;
     int fz_ng, fz_nstage;      // consumer groups per CTA, shared-memory ring depth
+    // the same for C2C plans (Nz == Ny == N: rows of N complex points)
+    const void* fc_fn[2];
+    int fc_rpt, fc_tc, fc_threads, fc_ng, fc_nstage;
+    size_t fc_smem;
 };
 
 // nullptr if this build has no kernels for (n, dtype)

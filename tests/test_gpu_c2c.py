@@ -27,6 +27,8 @@ def fft():
 
 
 CASES = [
+    ((64, 256, 256), 8),         # Nz == Ny: also runs fused (variant 3)
+    ((48, 384, 384), 12),
     ((32, 32, 128), 4),
     ((16, 64, 256), 8),
     ((64, 16, 192), 2),          # radix-3 rows
@@ -39,13 +41,20 @@ CASES = [
 
 @pytest.mark.parametrize("shape,p", CASES)
 @pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
-def test_c2c_matches_oracle(fft, oracle_mod, shape, p, dtype):
+@pytest.mark.parametrize("variant", [2, 3])     # 2: three passes per direction; 3: z+y fused wherever compiled (Nz == Ny)
+def test_c2c_matches_oracle(fft, oracle_mod, shape, p, dtype, variant):
     from paper_2202_12756_b200 import inputs
     try:
         plan = fft.PlanC2C(*shape, dtype=dtype, virtual_slabs=p)
     except fft.Fft3dError as e:
         assert e.status == 2
         pytest.skip("no C2C row kernel for %s %s" % (shape, dtype))
+    plan.set_variant(variant)
+    fused = plan.launch_names(0)[0] == "zy_c2c_fused_fwd"
+    if variant == 3 and not fused:
+        plan.close()
+        pytest.skip("no fused C2C kernels for %s %s" % (shape, dtype))
+    assert fused == (variant == 3)
     cd = plan.complex_dtype
     f = inputs.complex_grid(shape, cd, seed=11)
     d_in = f.cuda().reshape(-1)
@@ -74,8 +83,12 @@ def test_c2c_matches_oracle(fft, oracle_mod, shape, p, dtype):
     back = plan.c2c(out, +1).reshape(shape).cpu()
     err = (back - f).abs().max().item() / f.abs().max().item()
     assert err <= tol(shape, dtype)
-    assert plan.launch_names(0) == ("z_c2c_fwd", "y_c2c_fwd", "x_c2c_fwd")
-    assert plan.launch_names(1) == ("x_c2c_inv", "y_c2c_inv", "z_c2c_inv")
+    if fused:
+        assert plan.launch_names(0) == ("zy_c2c_fused_fwd", "x_c2c_fwd")
+        assert plan.launch_names(1) == ("x_c2c_inv", "yz_c2c_fused_inv")
+    else:
+        assert plan.launch_names(0) == ("z_c2c_fwd", "y_c2c_fwd", "x_c2c_fwd")
+        assert plan.launch_names(1) == ("x_c2c_inv", "y_c2c_inv", "z_c2c_inv")
     plan.close()
 
 
@@ -113,6 +126,7 @@ def test_c2c_512_full_oracle_and_1024_properties(fft, oracle_mod):
     n = 1024
     shape = (n, n, n)
     plan = fft.PlanC2C(*shape, dtype=torch.float32, virtual_slabs=64)
+    assert plan.launch_names(0)[0] == "zy_c2c_fused_fwd"      # the default at this size
     modes = [((3, 1000, 17), 1.5 - 0.5j), ((512, 0, 1023), -0.75 + 2.0j), ((77, 301, 640), 0.25 + 0.125j)]
     ax = torch.arange(n, device="cuda", dtype=torch.float64)
     f = torch.zeros(shape, dtype=torch.complex64, device="cuda")
