@@ -156,7 +156,8 @@ int fft3d_timing_read(fft3d_plan_t *plan, int which, float *ms_sum, int *calls);
 /* Kernel selection.  variant 0 (default) = the fastest known path for the extents: z and y
  * passes of each x-plane fused into one persistent kernel where that wins (cubic-like fp32
  * plans of >= 2 GiB, Ny == Nz: four array passes per R2C+C2R pair) and TMA-pipelined passes
- * elsewhere; variant 2 = the unfused TMA-pipelined passes (six array passes per pair);
+ * elsewhere; variant 2 = the first-generation unfused TMA-pipelined passes (six array passes per pair; whole
+ * tiles even where only one ring stage fits);
  * variant 3 = the fused z+y passes wherever they are compiled (any cubic-like plan with
  * N >= 128); variant 1 = plain-load kernels everywhere (ablation / cross-check).  Variants 0-2
  * without fusion give bit-identical results; the fused kernels run the same butterflies but are

@@ -22,6 +22,7 @@
 #include "fft_kernels.cuh"
 #include "fft_zpass.cuh"
 #include "fft_fused.cuh"
+#include "fft_split2.cuh"
 #include "fft_registry.h"
 
 namespace fft3d {
@@ -77,6 +78,9 @@ struct fft3d_plan_s {
     void* encode_fn;           // cuTensorMapEncodeTiled, resolved at run time (no libcuda link dependency)
     bool tma_y, tma_x;         // usable for this plan's extents / alignment
     bool tma_xc;               // C2C plans: TMA-pipelined x pass usable
+    bool split_y;              // Y passes as two half tiles + a radix-2 combine (fft_split2.cuh)
+    void* tw_y2;               // stage twiddles of the Ny/2-point transform
+    int y2_rows_nat, y2_rows_slab;   // rows per TMA box of the even/odd row views
     bool bulk_z;               // bulk-pipelined z kernels usable (row count a multiple of the tile)
     int y_rows_nat, y_rows_slab, x_rows;   // rows per TMA box
     // fused z+y passes (fft_fused.cuh): the workspace is [slab array | ring | side | flags]
@@ -287,6 +291,37 @@ int launch_fused(const fft3d_plan_s* pl, int d, const void* in, void* out, void*
     return FFT3D_OK;
 }
 
+// Y pass as two half tiles (fft_split2.cuh): d = 0 natural `in` -> slab `out`, d = 1 slab `in` -> natural `out`
+int launch_y_split2(const fft3d_plan_s* pl, int d, const void* in, void* out, cudaStream_t st) {
+    const KernelSet* ky = pl->ky;
+    const long long sz = 2 * pl->esize, W = sz / 8, M = pl->M, L = pl->L, Ny = pl->Ny, Nx = pl->Nx;
+    const int tc = ky->tma_tc;
+    TensorMapBlob ev, od, mo;
+    for (int h = 0; h < 2; ++h) {
+        const unsigned char* base = reinterpret_cast<const unsigned char*>(in) + (size_t)h * M * sz;
+        bool ok;
+        if (d == 0) {       // even / odd rows of [Nx][Ny][M]
+            long long dm[3] = {M * W, Ny / 2, Nx}, sb[2] = {2 * M * sz, Ny * M * sz};
+            int bx[3] = {(int)(tc * W), pl->y2_rows_nat, 1};
+            ok = make_map(pl, h ? &od : &ev, base, 3, dm, sb, bx);
+        } else {            // even / odd rows l of [p][Nx][L][M]
+            const long long Lh = L / 2;
+            long long dm[4] = {M * W, Lh, Nx, pl->p}, sb[3] = {2 * M * sz, L * M * sz, Nx * L * M * sz};
+            const int rows = pl->y2_rows_slab;
+            int bx[4] = {(int)(tc * W), (int)(rows < Lh ? rows : Lh), 1, (int)(rows < Lh ? 1 : rows / Lh)};
+            ok = make_map(pl, h ? &od : &ev, base, 4, dm, sb, bx);
+        }
+        if (!ok) return FFT3D_ECUDA;
+    }
+    if (!(d == 0 ? map_slab_y(pl, &mo, out, tc, pl->y_rows_slab) : map_natural(pl, &mo, out, tc, pl->y_rows_nat))) return FFT3D_ECUDA;
+    TmaArgs ta{};
+    ta.tw = pl->tw_y2; ta.ntz = (int)(M / tc); ta.ntiles = Nx * ta.ntz;
+    ta.L = (int)L; ta.Nx = (int)Nx; ta.Mp1 = (int)(M + 1);
+    ta.in_rows = d == 0 ? pl->y2_rows_nat : pl->y2_rows_slab;
+    ta.out_rows = d == 0 ? pl->y_rows_slab : pl->y_rows_nat;
+    return launch_tma(ky->y2_fn[d], ky->y2_threads, ky->y2_smem, pl->num_sms, ev, od, mo, ta, st);
+}
+
 // event slot `i` of the call being recorded for direction `which`, or no-op
 struct Recorder {
     TimingState* t;
@@ -380,6 +415,20 @@ static int plan_create(fft3d_plan_t** out, long long Nx, long long Ny, long long
             for (int d = 0; d < 2 && rc == FFT3D_OK; ++d) {
                 int g = 0;
                 rc = prepare_kernel(ky->tma_fn[d == 0 ? TMA_Y_FWD : TMA_Y_INV], ky->tma_threads, ky->tma_smem_y, sms, &g);
+            }
+            // whole tiles that leave room for a single ring stage: run them as two half tiles instead
+            if (rc == FFT3D_OK && ky->y2_fn[0] != nullptr && L % 2 == 0) {
+                const long long Lh = L / 2, H = Ny / 2;
+                pl->y2_rows_nat = (int)largest_divisor_le(H, 256);
+                pl->y2_rows_slab = (int)(Lh <= 256 ? Lh * largest_divisor_le(pl->p, 256 / Lh) : largest_divisor_le(Lh, 256));
+                if (H % pl->y_rows_nat == 0 && H % pl->y_rows_slab == 0 && H % pl->y2_rows_slab == 0) {
+                    pl->split_y = true;
+                    for (int d = 0; d < 2 && rc == FFT3D_OK; ++d) {
+                        int g = 0;
+                        rc = prepare_kernel(ky->y2_fn[d], ky->y2_threads, ky->y2_smem, sms, &g);
+                    }
+                    if (rc == FFT3D_OK) rc = upload_stage_twiddles(ky->y2_nst, ky->y2_radix, ky->y2_twn, pl->esize, &pl->tw_y2);
+                }
             }
         }
         if (rc == FFT3D_OK && kind == 1 && fn != nullptr && strides_ok && kx->xc_fn[0] != nullptr && M % kx->tma_tc_x == 0) {
@@ -580,7 +629,9 @@ int fft3d_r2c(const fft3d_plan_t* pl, const void* d_in, void* d_out, void* d_wor
     a.ntiles = Nx * a.ntz;
     a.in_hi = Ny * M; a.in_lo = 0; a.in_rq = 0; a.in_rl = M;
     a.out_hi = L * M; a.out_lo = 0; a.out_rq = Nx * L * M; a.out_rl = M;
-    if (tma_on && pl->tma_y) {
+    if (tma_on && pl->split_y && pl->variant != 2) {
+        rc = launch_y_split2(pl, 0, d_out, d_work, st);
+    } else if (tma_on && pl->tma_y) {
         TensorMapBlob mi, mo;
         if (!map_natural(pl, &mi, d_out, ky->tma_tc, pl->y_rows_nat) ||
             !map_slab_y(pl, &mo, d_work, ky->tma_tc, pl->y_rows_slab)) return FFT3D_ECUDA;
@@ -708,7 +759,9 @@ int fft3d_c2r(const fft3d_plan_t* pl, const void* d_in, void* d_out, void* d_wor
     a.ntiles = Nx * a.ntz;
     a.in_hi = L * M; a.in_lo = 0; a.in_rq = Nx * L * M; a.in_rl = M;
     a.out_hi = Ny * M; a.out_lo = 0; a.out_rq = 0; a.out_rl = M;
-    if (tma_on && pl->tma_y) {
+    if (tma_on && pl->split_y && pl->variant != 2) {
+        rc = launch_y_split2(pl, 1, d_out, d_work, st);
+    } else if (tma_on && pl->tma_y) {
         TensorMapBlob mi, mo;
         if (!map_slab_y(pl, &mi, d_out, ky->tma_tc, pl->y_rows_slab) ||
             !map_natural(pl, &mo, d_work, ky->tma_tc, pl->y_rows_nat)) return FFT3D_ECUDA;
@@ -764,6 +817,7 @@ int fft3d_c2c(const fft3d_plan_t* pl, const void* d_in, void* d_out, void* d_wor
         return FFT3D_OK;
     };
     auto y_pass = [&](const void* in, void* out) -> int {       // forward: natural -> slab; inverse: slab -> natural
+        if (tma_on && pl->split_y && pl->variant != 2) return launch_y_split2(pl, d, in, out, st);
         if (tma_on && pl->tma_y) {
             TensorMapBlob mi, mo;
             bool ok = d == 0 ? (map_natural(pl, &mi, in, ky->tma_tc, pl->y_rows_nat) && map_slab_y(pl, &mo, out, ky->tma_tc, pl->y_rows_slab))
@@ -935,7 +989,7 @@ int fft3d_c2r_host(fft3d_plan_t* pl, const void* h_in, void* h_out) {
 
 int fft3d_destroy(fft3d_plan_t* pl) {
     if (pl == nullptr) return FFT3D_OK;
-    cudaFree(pl->tw_zb); cudaFree(pl->tw_zc); cudaFree(pl->tw_z); cudaFree(pl->tw_y); cudaFree(pl->tw_x); cudaFree(pl->twz);
+    cudaFree(pl->tw_zb); cudaFree(pl->tw_zc); cudaFree(pl->tw_y2); cudaFree(pl->tw_z); cudaFree(pl->tw_y); cudaFree(pl->tw_x); cudaFree(pl->twz);
     cudaFree(pl->h_real); cudaFree(pl->h_cplx); cudaFree(pl->h_work);
     if (pl->h_stream) cudaStreamDestroy(pl->h_stream);
     timing_free(pl);

@@ -3,6 +3,7 @@
 #include "fft_kernels.cuh"
 #include "fft_zpass.cuh"
 #include "fft_fused.cuh"
+#include "fft_split2.cuh"
 #include "fft_configs.cuh"
 #include "fft_registry.h"
 
@@ -39,6 +40,32 @@ static void add_fused(KernelSet& k) {
                 k.fz_smem = (size_t)FT::smem_bytes(NS);
                 k.fz_ng = NG;
                 k.fz_nstage = NS;
+            }
+        }
+    }
+}
+
+// Y passes of length N as two N/2-point half tiles (only where the whole tile leaves room for one ring stage)
+template <typename T, int N>
+static void add_split2(KernelSet& k) {
+    if constexpr (N >= 256 && N % 2 == 0) {
+        using C = cx<T>;
+        using Cfg = typename CfgFor<T, N>::type;
+        using HCfg = typename CfgFor<T, N / 2>::type;
+        constexpr int TTC = tma_tile_cols(Cfg::N, Cfg::S, (int)sizeof(C));
+        constexpr int HTC = tma_tile_cols(HCfg::N, HCfg::S, (int)sizeof(C));
+        if constexpr (TTC > 0 && HTC == TTC) {
+            using TY = TmaTile<Cfg, TTC, T, false>;
+            using TH = TmaTile<HCfg, TTC, T, false>;
+            if constexpr (TY::max_stages() <= 1 && TH::max_stages() >= 3) {
+                constexpr int NS = 3;
+                k.y2_fn[0] = (const void*)fft_y_split2_kernel<HCfg, TTC, TMA_Y_FWD, T, NS>;
+                k.y2_fn[1] = (const void*)fft_y_split2_kernel<HCfg, TTC, TMA_Y_INV, T, NS>;
+                k.y2_threads = TH::NCONS + 32;
+                k.y2_smem = (size_t)TH::smem_bytes(NS);
+                k.y2_nst = HCfg::NST;
+                for (int s = 0; s < 5; ++s) k.y2_radix[s] = s < HCfg::NST ? HCfg::radix(s) : 1;
+                k.y2_twn = HCfg::TWN;
             }
         }
     }
@@ -187,6 +214,7 @@ static KernelSet make_set(int dtype) {
     }
     add_fused<T, FFT3D_N>(k);
     add_fused_c2c<T, FFT3D_N>(k);
+    add_split2<T, FFT3D_N>(k);
     return k;
 }
 

@@ -1,0 +1,149 @@
+// fft_split2.cuh -- Y passes (F2, I2; paper step 1 y half + steps 2-4, P:69-76 / P:86) for lengths whose
+// [N rows][TC columns] tile is too large for more than ONE ring stage (N = 2048 fp32: 128 KiB), so that
+// load, transform and store take turns (3.5 TB/s).
+//
+// One decimation-in-time step is taken OUT of the tile: the even rows and the odd rows of a tile are two
+// independent N/2-point transforms E and O, each a half tile of 64 KiB that moves through a 3-slot ring
+// like any other tile; when the second one is done the two are combined in place, element by element,
+//     X[k] = E[k] + w^k O[k],   X[k + N/2] = E[k] - w^k O[k],   w = exp(-+2 pi i / N),
+// after which the slot that held E holds output rows [0, N/2) and the slot that held O rows [N/2, N).
+// The loads of the next tile's even half overlap the transform of this tile's odd half, and so on.
+// Each thread combines exactly the elements it wrote itself (t + m*S), so the combine needs no barrier;
+// w^(t + m S) = w^t * exp(-+2 pi i m / (2P)): one per-thread value times compile-time constants.
+//
+// Even / odd rows are addressed by tensor maps with a doubled row stride (built per call on the host).
+#pragma once
+#include "fft_kernels.cuh"
+
+namespace fft3d {
+
+// X[k] = E[k] + w^k O[k] -> e, X[k+H] = E[k] - w^k O[k] -> o, for the thread's own elements k = t + m*S
+// (O in registers, E in its slot's dense layout)
+template <class HCfg, int DIR, typename T, class Lay, int MM = 0>
+__device__ __forceinline__ void combine_halves(cx<T> (&v)[HCfg::P], cx<T>* __restrict__ e, cx<T>* __restrict__ o,
+                                               cx<T> wt, int t, const Lay& lay) {
+    if constexpr (MM < HCfg::P) {
+        constexpr int P = HCfg::P, S = HCfg::S;
+        const int idx = lay.at(t + MM * S);
+        const cx<T> wo = cmul(mul_root<MM, 2 * P, DIR, T>(wt), v[MM]);
+        const cx<T> ev = e[idx];
+        e[idx] = cadd(ev, wo);
+        o[idx] = csub(ev, wo);
+        combine_halves<HCfg, DIR, T, Lay, MM + 1>(v, e, o, wt, t, lay);
+    }
+}
+
+// HCfg: the N/2-point transform.  PASS: TMA_Y_FWD (natural -> slab) or TMA_Y_INV (slab -> natural).
+template <class HCfg, int TC, int PASS, typename T, int NSTAGE>
+__global__ void __launch_bounds__(HCfg::S * TC + 32, 1)
+fft_y_split2_kernel(const __grid_constant__ TensorMapBlob in_even, const __grid_constant__ TensorMapBlob in_odd,
+                    const __grid_constant__ TensorMapBlob out_map, const TmaArgs a) {
+    using C = cx<T>;
+    using TT = TmaTile<HCfg, TC, T, false>;
+    constexpr int P = HCfg::P, S = HCfg::S, W = TT::W, NCONS = TT::NCONS, H = HCfg::N;   // H = N/2 rows per half
+    constexpr int DIR = (PASS == TMA_Y_FWD) ? -1 : +1;
+    static_assert(PASS == TMA_Y_FWD || PASS == TMA_Y_INV, "Y passes only");
+    static_assert(NSTAGE >= 3, "a pair of half tiles plus one in flight");
+    extern __shared__ __align__(1024) unsigned char smem_dyn[];
+    C* tw = reinterpret_cast<C*>(smem_dyn);
+    unsigned char* stages = smem_dyn + TT::TW_BYTES;
+    unsigned long long* full = reinterpret_cast<unsigned long long*>(stages + NSTAGE * TT::STAGE_BYTES);
+    unsigned long long* done = full + NSTAGE;
+
+    const int tid = threadIdx.x;
+    const bool is_producer = tid >= NCONS;
+    if (tid == NCONS) {
+        for (int s = 0; s < NSTAGE; ++s) { tma::mbar_init(&full[s], 1); tma::mbar_init(&done[s], NCONS / 32); }
+        tma::fence_mbar_init();
+    }
+    if (!is_producer) load_twiddles<DIR, T>(tw, reinterpret_cast<const C*>(a.tw), HCfg::TWN, tid, NCONS);
+    __syncthreads();
+
+    const long long first = blockIdx.x, stride = gridDim.x;
+    const long long n_tiles = first < a.ntiles ? (a.ntiles - first + stride - 1) / stride : 0;
+    const long long n_items = 2 * n_tiles;               // item i = (tile i/2, half i&1)
+    const int Lh = a.L / 2;                              // half rows per virtual slab
+
+    if (is_producer) {
+        if (tid != NCONS) return;
+        auto issue_load = [=, &in_even, &in_odd](long long i) {
+            const long long t_id = first + (i >> 1) * stride;
+            const int h = (int)(i & 1), s = (int)(i % NSTAGE);
+            const int tz = (int)(t_id % a.ntz), x = (int)(t_id / a.ntz);
+            unsigned char* dst = stages + s * TT::STAGE_BYTES;
+            const TensorMapBlob* map = h ? &in_odd : &in_even;
+            const int nb = H / a.in_rows;
+            tma::mbar_expect_tx(&full[s], TT::TILE_BYTES);
+            for (int b = 0; b < nb; ++b) {
+                void* d = dst + (size_t)b * a.in_rows * TT::ROW_BYTES;
+                const int r0 = b * a.in_rows;                    // index among the even (odd) rows
+                if constexpr (PASS == TMA_Y_FWD) tma::load3(d, map, &full[s], tz * TC * W, r0, x);
+                else tma::load4(d, map, &full[s], tz * TC * W, r0 % Lh, x, r0 / Lh);
+            }
+        };
+        // output rows [h*H, (h+1)*H) of the tile sit in the slot of its half h
+        auto issue_store = [=, &out_map](long long i) {
+            const long long t_id = first + (i >> 1) * stride;
+            const int h = (int)(i & 1), s = (int)(i % NSTAGE);
+            const int tz = (int)(t_id % a.ntz), x = (int)(t_id / a.ntz);
+            const unsigned char* src = stages + s * TT::STAGE_BYTES;
+            const int nb = H / a.out_rows;
+            for (int b = 0; b < nb; ++b) {
+                const void* d = src + (size_t)b * a.out_rows * TT::ROW_BYTES;
+                const int r0 = h * H + b * a.out_rows;
+                if constexpr (PASS == TMA_Y_FWD) tma::store4(&out_map, d, tz * TC * W, r0 % a.L, x, r0 / a.L);
+                else tma::store3(&out_map, d, tz * TC * W, r0, x);
+            }
+        };
+        long long stored_pairs = 0;
+        auto ensure_stored = [&](long long j) {                  // item j's slot is reusable after its pair is out
+            const long long pr = j >> 1;
+            if (pr < stored_pairs) return;
+            for (long long k = 2 * pr; k < 2 * pr + 2; ++k)
+                tma::mbar_wait(&done[k % NSTAGE], (unsigned)((k / NSTAGE) & 1));
+            issue_store(2 * pr);
+            issue_store(2 * pr + 1);
+            tma::store_commit();
+            tma::store_wait_read0();
+            stored_pairs = pr + 1;
+        };
+        for (long long i = 0; i < n_items; ++i) {
+            if (i >= NSTAGE) ensure_stored(i - NSTAGE);
+            issue_load(i);
+        }
+        for (long long pr = stored_pairs; pr < n_tiles; ++pr) ensure_stored(2 * pr);
+        tma::store_wait_all();
+        return;
+    }
+
+    // ---------------- consumers ----------------
+    const int c = tid % TC, t = tid / TC;
+    const SmLayout<TC, 0> dense{c};
+    const SmLayout<TC, TT::PADR> padded{c};
+    const NamedSync<1, NCONS> sync{};
+    // w^t = exp(DIR 2 pi i t / N), N = 2H, in double once per thread (no fast-math intrinsics)
+    double ws, wc;
+    sincospi((double)DIR * (double)t / (double)H, &ws, &wc);
+    const C wt = mk<T>((T)wc, (T)ws);
+    for (long long i = 0; i < n_items; ++i) {
+        const int s = (int)(i % NSTAGE);
+        C* buf = reinterpret_cast<C*>(stages + s * TT::STAGE_BYTES);
+        tma::mbar_wait(&full[s], (unsigned)((i / NSTAGE) & 1));
+        C v[P];
+        read_own<HCfg, T>(v, buf, t, dense);
+        if constexpr (HCfg::NST > 1) sync();
+        fft_stages<HCfg, 0, DIR, T>(v, buf, tw, t, padded, sync);
+        if constexpr (HCfg::NST > 1) sync();                     // all exchange reads done
+        if ((i & 1) == 0) {
+            write_own<HCfg, T>(v, buf, t, dense);                // E stays in its slot until O is there
+        } else {
+            C* ebuf = reinterpret_cast<C*>(stages + (int)((i - 1) % NSTAGE) * TT::STAGE_BYTES);
+            combine_halves<HCfg, DIR, T>(v, ebuf, buf, wt, t, dense);
+            tma::fence_proxy_async();
+            __syncwarp();
+            if ((tid & 31) == 0) { tma::mbar_arrive(&done[(i - 1) % NSTAGE]); tma::mbar_arrive(&done[s]); }
+        }
+    }
+}
+
+}  // namespace fft3d
