@@ -80,6 +80,9 @@ struct fft3d_plan_s {
     bool tma_xc;               // C2C plans: TMA-pipelined x pass usable
     bool split_y;              // Y passes as two half tiles + a radix-2 combine (fft_split2.cuh)
     void* tw_y2;               // stage twiddles of the Ny/2-point transform
+    bool split_x;              // X passes as two half tiles (R2C/C2R plans)
+    void* tw_x2;               // stage twiddles of the Nx/2-point transform
+    int x2_rows;               // rows per TMA box of the even/odd x-row views
     int y2_rows_nat, y2_rows_slab;   // rows per TMA box of the even/odd row views
     bool bulk_z;               // bulk-pipelined z kernels usable (row count a multiple of the tile)
     int y_rows_nat, y_rows_slab, x_rows;   // rows per TMA box
@@ -322,6 +325,43 @@ int launch_y_split2(const fft3d_plan_s* pl, int d, const void* in, void* out, cu
     return launch_tma(ky->y2_fn[d], ky->y2_threads, ky->y2_smem, pl->num_sms, ev, od, mo, ta, st);
 }
 
+// X pass as two half tiles (fft_split2.cuh): d = 0 packed slab `in` -> user spectrum `out`, d = 1 the reverse
+int launch_x_split2(const fft3d_plan_s* pl, int d, const void* in, void* out, cudaStream_t st) {
+    const KernelSet* kx = pl->kx;
+    const long long sz = 2 * pl->esize, W = sz / 8, M = pl->M, L = pl->L, Nx = pl->Nx, p = pl->p, Mp1 = M + 1;
+    const int tc = kx->tma_tc_x, rows = pl->x2_rows;
+    TensorMapBlob ld[2][2], mo;          // [wide][odd x rows]
+    for (int wide = 0; wide < 2; ++wide)
+        for (int h = 0; h < 2; ++h) {
+            const int cols = tc + 2 * wide;
+            bool ok;
+            if (d == 0) {       // even / odd x rows of [p][Nx][L][M]
+                const unsigned char* base = reinterpret_cast<const unsigned char*>(in) + (size_t)h * L * M * sz;
+                long long dm[4] = {M * W, L, Nx / 2, p}, sb[3] = {M * sz, 2 * L * M * sz, Nx * L * M * sz};
+                int bx[4] = {(int)(cols * W), 1, rows, 1};
+                ok = make_map(pl, &ld[wide][h], base, 4, dm, sb, bx);
+            } else {            // even / odd x rows of [p][Nx][L*(M+1)]
+                const unsigned char* base = reinterpret_cast<const unsigned char*>(in) + (size_t)h * L * Mp1 * sz;
+                long long dm[3] = {L * Mp1 * W, Nx / 2, p}, sb[2] = {2 * L * Mp1 * sz, Nx * L * Mp1 * sz};
+                int bx[3] = {(int)(cols * W), rows, 1};
+                ok = make_map(pl, &ld[wide][h], base, 3, dm, sb, bx);
+            }
+            if (!ok) return FFT3D_ECUDA;
+        }
+    if (!(d == 0 ? map_user_x(pl, &mo, out, tc, pl->x_rows) : map_slab_x(pl, &mo, out, tc, pl->x_rows))) return FFT3D_ECUDA;
+    TmaArgs ta{};
+    ta.user_out = out;
+    ta.tw = pl->tw_x2; ta.ntz = (int)(M / tc);
+    ta.ntiles = (long long)p * (L / 2) * (2 * ta.ntz + (d == 0 ? 1 : 0));
+    ta.L = (int)L; ta.Nx = (int)Nx; ta.Mp1 = (int)Mp1; ta.in_rows = rows; ta.out_rows = pl->x_rows;
+    long long g = ta.ntiles < pl->num_sms ? ta.ntiles : pl->num_sms;
+    if (g <= 0) return FFT3D_OK;
+    void* argv[6] = {(void*)&ld[0][0], (void*)&ld[0][1], (void*)&ld[1][0], (void*)&ld[1][1], (void*)&mo, (void*)&ta};
+    cudaError_t e = cudaLaunchKernel(kx->x2_fn[d], dim3((unsigned)g), dim3((unsigned)kx->x2_threads), argv, kx->x2_smem, st);
+    if (e != cudaSuccess) { cudaGetLastError(); return FFT3D_ECUDA; }
+    return FFT3D_OK;
+}
+
 // event slot `i` of the call being recorded for direction `which`, or no-op
 struct Recorder {
     TimingState* t;
@@ -445,6 +485,15 @@ static int plan_create(fft3d_plan_t** out, long long Nx, long long Ny, long long
             for (int d = 0; d < 2 && rc == FFT3D_OK; ++d) {
                 int g = 0;
                 rc = prepare_kernel(kx->tma_fn[d == 0 ? TMA_X_FWD : TMA_X_INV], kx->tma_threads_x, kx->tma_smem_x, sms, &g);
+            }
+            if (rc == FFT3D_OK && kx->x2_fn[0] != nullptr && kx->tma_oddfix && Nx % 2 == 0 && (Nx / 2) % pl->x_rows == 0) {
+                pl->split_x = true;
+                pl->x2_rows = (int)largest_divisor_le(Nx / 2, 256);
+                for (int d = 0; d < 2 && rc == FFT3D_OK; ++d) {
+                    int g = 0;
+                    rc = prepare_kernel(kx->x2_fn[d], kx->x2_threads, kx->x2_smem, sms, &g);
+                }
+                if (rc == FFT3D_OK) rc = upload_stage_twiddles(kx->y2_nst, kx->y2_radix, kx->y2_twn, pl->esize, &pl->tw_x2);
             }
         }
     }
@@ -654,7 +703,9 @@ int fft3d_r2c(const fft3d_plan_t* pl, const void* d_in, void* d_out, void* d_wor
     b.ntiles = (long long)p * L * b.ntz;
     b.in_hi = Nx * L * M; b.in_lo = M; b.in_rq = 0; b.in_rl = L * M;
     b.out_hi = Nx * L * (M + 1); b.out_lo = M + 1; b.out_rq = 0; b.out_rl = L * (M + 1);
-    if (tma_on && pl->tma_x) {
+    if (tma_on && pl->split_x && pl->variant != 2) {
+        rc = launch_x_split2(pl, 0, d_work, d_out, st);
+    } else if (tma_on && pl->tma_x) {
         TensorMapBlob mi, mo;
         TensorMapBlob mi2;
         const int tc = kx->tma_tc_x, of = kx->tma_oddfix;
@@ -725,7 +776,8 @@ int fft3d_c2r(const fft3d_plan_t* pl, const void* d_in, void* d_out, void* d_wor
         ta.tw = pl->tw_x; ta.ntz = (int)(M / tc);
         ta.ntiles = of ? (long long)p * (L / 2) * (2 * ta.ntz) : (long long)p * L * ta.ntz;
         ta.L = (int)L; ta.Nx = (int)Nx; ta.Mp1 = (int)(M + 1); ta.in_rows = pl->x_rows; ta.out_rows = pl->x_rows;
-        rc = launch_tma(kx->tma_fn[TMA_X_INV], kx->tma_threads_x, kx->tma_smem_x, pl->num_sms, mi, mi2, mo, ta, st);
+        if (pl->split_x && pl->variant != 2) rc = launch_x_split2(pl, 1, d_in, x_out, st);
+        else rc = launch_tma(kx->tma_fn[TMA_X_INV], kx->tma_threads_x, kx->tma_smem_x, pl->num_sms, mi, mi2, mo, ta, st);
         rec.mark(slot++);
         // packed column 0 of the result: x-transform of the side buffer, written over the (meaningless)
         // column the tiles produced from the user's raw kz = 0 plane
@@ -989,7 +1041,7 @@ int fft3d_c2r_host(fft3d_plan_t* pl, const void* h_in, void* h_out) {
 
 int fft3d_destroy(fft3d_plan_t* pl) {
     if (pl == nullptr) return FFT3D_OK;
-    cudaFree(pl->tw_zb); cudaFree(pl->tw_zc); cudaFree(pl->tw_y2); cudaFree(pl->tw_z); cudaFree(pl->tw_y); cudaFree(pl->tw_x); cudaFree(pl->twz);
+    cudaFree(pl->tw_zb); cudaFree(pl->tw_zc); cudaFree(pl->tw_y2); cudaFree(pl->tw_x2); cudaFree(pl->tw_z); cudaFree(pl->tw_y); cudaFree(pl->tw_x); cudaFree(pl->twz);
     cudaFree(pl->h_real); cudaFree(pl->h_cplx); cudaFree(pl->h_work);
     if (pl->h_stream) cudaStreamDestroy(pl->h_stream);
     timing_free(pl);

@@ -57,15 +57,24 @@ static void add_split2(KernelSet& k) {
         if constexpr (TTC > 0 && HTC == TTC) {
             using TY = TmaTile<Cfg, TTC, T, false>;
             using TH = TmaTile<HCfg, TTC, T, false>;
+            k.y2_nst = HCfg::NST;
+            for (int s = 0; s < 5; ++s) k.y2_radix[s] = s < HCfg::NST ? HCfg::radix(s) : 1;
+            k.y2_twn = HCfg::TWN;
             if constexpr (TY::max_stages() <= 1 && TH::max_stages() >= 3) {
                 constexpr int NS = 3;
                 k.y2_fn[0] = (const void*)fft_y_split2_kernel<HCfg, TTC, TMA_Y_FWD, T, NS>;
                 k.y2_fn[1] = (const void*)fft_y_split2_kernel<HCfg, TTC, TMA_Y_INV, T, NS>;
                 k.y2_threads = TH::NCONS + 32;
                 k.y2_smem = (size_t)TH::smem_bytes(NS);
-                k.y2_nst = HCfg::NST;
-                for (int s = 0; s < 5; ++s) k.y2_radix[s] = s < HCfg::NST ? HCfg::radix(s) : 1;
-                k.y2_twn = HCfg::TWN;
+            }
+            using TXW = TmaTile<Cfg, TTC, T, true>;
+            using THW = TmaTile<HCfg, TTC, T, true>;
+            if constexpr (TXW::max_stages() <= 1 && THW::max_stages() >= 3) {
+                constexpr int NS = 3;
+                k.x2_fn[0] = (const void*)fft_x_split2_kernel<HCfg, TTC, TMA_X_FWD, T, NS>;
+                k.x2_fn[1] = (const void*)fft_x_split2_kernel<HCfg, TTC, TMA_X_INV, T, NS>;
+                k.x2_threads = THW::NCONS + 32;
+                k.x2_smem = (size_t)THW::smem_bytes(NS);
             }
         }
     }

@@ -42,8 +42,11 @@ struct KernelSet {
     size_t xc_smem;
     // Y passes as two half tiles + one radix-2 combine (fft_split2.cuh); null unless the whole tile has a single stage
     const void* y2_fn[2];      // [0 = Y_FWD, 1 = Y_INV]
-    int y2_threads, y2_nst, y2_radix[5], y2_twn;
+    int y2_threads, y2_nst, y2_radix[5], y2_twn;   // y2_nst.. = the factorisation of the N/2-point transform (X kernels too)
     size_t y2_smem;
+    const void* x2_fn[2];      // the same for the X passes with shifted windows: [0 = X_FWD, 1 = X_INV]
+    int x2_threads;
+    size_t x2_smem;
     // C2C row kernels (z pass of the 3D C2C transform): the bulk-pipelined kernel without the Hermitian step
     const void* zc_fn[2];      // [0 = forward, 1 = inverse (scaled)]
     int zc_rpt, zc_nst, zc_radix[5], zc_twn, zc_threads;

@@ -40,7 +40,7 @@ fft_y_split2_kernel(const __grid_constant__ TensorMapBlob in_even, const __grid_
                     const __grid_constant__ TensorMapBlob out_map, const TmaArgs a) {
     using C = cx<T>;
     using TT = TmaTile<HCfg, TC, T, false>;
-    constexpr int P = HCfg::P, S = HCfg::S, W = TT::W, NCONS = TT::NCONS, H = HCfg::N;   // H = N/2 rows per half
+    constexpr int P = HCfg::P, W = TT::W, NCONS = TT::NCONS, H = HCfg::N;   // H = N/2 rows per half
     constexpr int DIR = (PASS == TMA_Y_FWD) ? -1 : +1;
     static_assert(PASS == TMA_Y_FWD || PASS == TMA_Y_INV, "Y passes only");
     static_assert(NSTAGE >= 3, "a pair of half tiles plus one in flight");
@@ -139,6 +139,145 @@ fft_y_split2_kernel(const __grid_constant__ TensorMapBlob in_even, const __grid_
         } else {
             C* ebuf = reinterpret_cast<C*>(stages + (int)((i - 1) % NSTAGE) * TT::STAGE_BYTES);
             combine_halves<HCfg, DIR, T>(v, ebuf, buf, wt, t, dense);
+            tma::fence_proxy_async();
+            __syncwarp();
+            if ((tid & 31) == 0) { tma::mbar_arrive(&done[(i - 1) % NSTAGE]); tma::mbar_arrive(&done[s]); }
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// The same for the X passes (F3, I1; paper step 5, P:77 / P:86) with the shifted windows of odd rows
+// (fft_kernels.cuh, ODDFIX): used where a whole tile with its TC+2 landing columns leaves room for one
+// ring stage only (Nx = 1536 fp32: 120 KiB) but a half tile for three (60 KiB).
+//   loads: ld_even / ld_odd = the even / odd x rows of the loading side, plain windows (TC columns);
+//          ldw_even / ldw_odd = the same with TC+2 columns (windows of odd-l rows);  store: the whole array.
+// ---------------------------------------------------------------------------------------------
+template <class HCfg, int TC, int PASS, typename T, int NSTAGE>
+__global__ void __launch_bounds__(HCfg::S * TC + 32, 1)
+fft_x_split2_kernel(const __grid_constant__ TensorMapBlob ld_even, const __grid_constant__ TensorMapBlob ld_odd,
+                    const __grid_constant__ TensorMapBlob ldw_even, const __grid_constant__ TensorMapBlob ldw_odd,
+                    const __grid_constant__ TensorMapBlob out_map, const TmaArgs a) {
+    using C = cx<T>;
+    using TT = TmaTile<HCfg, TC, T, true>;
+    constexpr int P = HCfg::P, S = HCfg::S, W = TT::W, NCONS = TT::NCONS, H = HCfg::N;
+    constexpr int DIR = (PASS == TMA_X_FWD) ? -1 : +1;
+    static_assert(PASS == TMA_X_FWD || PASS == TMA_X_INV, "X passes only");
+    static_assert(NSTAGE >= 3, "a pair of half tiles plus one in flight");
+    extern __shared__ __align__(1024) unsigned char smem_dyn[];
+    C* tw = reinterpret_cast<C*>(smem_dyn);
+    unsigned char* stages = smem_dyn + TT::TW_BYTES;
+    unsigned long long* full = reinterpret_cast<unsigned long long*>(stages + NSTAGE * TT::STAGE_BYTES);
+    unsigned long long* done = full + NSTAGE;
+
+    const int tid = threadIdx.x;
+    const bool is_producer = tid >= NCONS;
+    if (tid == NCONS) {
+        for (int s = 0; s < NSTAGE; ++s) { tma::mbar_init(&full[s], 1); tma::mbar_init(&done[s], NCONS / 32); }
+        tma::fence_mbar_init();
+    }
+    if (!is_producer) load_twiddles<DIR, T>(tw, reinterpret_cast<const C*>(a.tw), HCfg::TWN, tid, NCONS);
+    __syncthreads();
+
+    const long long first = blockIdx.x, stride = gridDim.x;
+    const long long n_tiles = first < a.ntiles ? (a.ntiles - first + stride - 1) / stride : 0;
+    const long long n_items = 2 * n_tiles;
+
+    if (is_producer) {
+        if (tid != NCONS) return;
+        auto issue_load = [=, &ld_even, &ld_odd, &ldw_even, &ldw_odd](long long i) {
+            const XTile xt = decode_xtile<PASS, true>(first + (i >> 1) * stride, a);
+            const int h = (int)(i & 1), s = (int)(i % NSTAGE);
+            unsigned char* dst = stages + s * TT::STAGE_BYTES;
+            const int rowb = xt.odd ? TT::ROW_BYTES_WIDE : TT::ROW_BYTES;
+            const TensorMapBlob* map = xt.odd ? (h ? &ldw_odd : &ldw_even) : (h ? &ld_odd : &ld_even);
+            const int nb = H / a.in_rows;
+            tma::mbar_expect_tx(&full[s], (unsigned)(H * rowb));
+            for (int b = 0; b < nb; ++b) {
+                void* d = dst + (size_t)b * a.in_rows * rowb;
+                const int r0 = b * a.in_rows;                    // index among the even (odd) x rows
+                if constexpr (PASS == TMA_X_FWD)
+                    tma::load4(d, map, &full[s], (xt.w * TC - 2 * xt.odd) * W, xt.l, r0, xt.q);
+                else
+                    tma::load3(d, map, &full[s], (xt.l * a.Mp1 + xt.w * TC - xt.odd) * W, r0, xt.q);
+            }
+        };
+        auto issue_store = [=, &out_map](long long i) {
+            const XTile xt = decode_xtile<PASS, true>(first + (i >> 1) * stride, a);
+            if (xt.thin) return;                                 // stored by the consumers
+            const int h = (int)(i & 1), s = (int)(i % NSTAGE);
+            const unsigned char* src = stages + s * TT::STAGE_BYTES;
+            const int nb = H / a.out_rows;
+            for (int b = 0; b < nb; ++b) {
+                const void* d = src + (size_t)b * a.out_rows * TT::ROW_BYTES;
+                const int r0 = h * H + b * a.out_rows;
+                if constexpr (PASS == TMA_X_FWD)
+                    tma::store3(&out_map, d, (xt.l * a.Mp1 + xt.w * TC - xt.odd) * W, r0, xt.q);
+                else
+                    tma::store4(&out_map, d, xt.w * TC * W, xt.l, r0, xt.q);
+            }
+        };
+        long long stored_pairs = 0;
+        auto ensure_stored = [&](long long j) {
+            const long long pr = j >> 1;
+            if (pr < stored_pairs) return;
+            for (long long k = 2 * pr; k < 2 * pr + 2; ++k)
+                tma::mbar_wait(&done[k % NSTAGE], (unsigned)((k / NSTAGE) & 1));
+            issue_store(2 * pr);
+            issue_store(2 * pr + 1);
+            tma::store_commit();
+            tma::store_wait_read0();
+            stored_pairs = pr + 1;
+        };
+        for (long long i = 0; i < n_items; ++i) {
+            if (i >= NSTAGE) ensure_stored(i - NSTAGE);
+            issue_load(i);
+        }
+        for (long long pr = stored_pairs; pr < n_tiles; ++pr) ensure_stored(2 * pr);
+        tma::store_wait_all();
+        return;
+    }
+
+    // ---------------- consumers ----------------
+    const int c = tid % TC, t = tid / TC;
+    const SmLayout<TC, 0> dense{c};
+    const SmLayout<TC + 2, 0> dense_wide{c + 1};
+    const SmLayout<TC, TT::PADR> padded{c};
+    const NamedSync<1, NCONS> sync{};
+    double ws, wc;
+    sincospi((double)DIR * (double)t / (double)H, &ws, &wc);
+    const C wt = mk<T>((T)wc, (T)ws);
+    for (long long i = 0; i < n_items; ++i) {
+        const XTile xt = decode_xtile<PASS, true>(first + (i >> 1) * stride, a);
+        const int s = (int)(i % NSTAGE);
+        C* buf = reinterpret_cast<C*>(stages + s * TT::STAGE_BYTES);
+        tma::mbar_wait(&full[s], (unsigned)((i / NSTAGE) & 1));
+        C v[P];
+        if (xt.odd) read_own<HCfg, T>(v, buf, t, dense_wide);
+        else read_own<HCfg, T>(v, buf, t, dense);
+        if constexpr (HCfg::NST > 1) sync();
+        fft_stages<HCfg, 0, DIR, T>(v, buf, tw, t, padded, sync);
+        if constexpr (HCfg::NST > 1) sync();
+        if ((i & 1) == 0) {
+            write_own<HCfg, T>(v, buf, t, dense);
+        } else {
+            C* ebuf = reinterpret_cast<C*>(stages + (int)((i - 1) % NSTAGE) * TT::STAGE_BYTES);
+            combine_halves<HCfg, DIR, T>(v, ebuf, buf, wt, t, dense);
+            if (PASS == TMA_X_FWD && xt.thin) {
+                // thin tile: only column M-1 (thread column 0) is real; plain stores to the user's rows
+                __syncwarp();
+                if (c == 0) {
+                    const long long rstride = (long long)a.L * a.Mp1;
+                    C* p = reinterpret_cast<C*>(a.user_out) +
+                           (((long long)xt.q * a.Nx * a.L + xt.l) * a.Mp1 + (a.Mp1 - 2));
+#pragma unroll
+                    for (int m = 0; m < P; ++m) {
+                        const int k = t + m * S;
+                        p[(long long)k * rstride] = ebuf[dense.at(k)];
+                        p[(long long)(k + H) * rstride] = buf[dense.at(k)];
+                    }
+                }
+            }
             tma::fence_proxy_async();
             __syncwarp();
             if ((tid & 31) == 0) { tma::mbar_arrive(&done[(i - 1) % NSTAGE]); tma::mbar_arrive(&done[s]); }

@@ -60,6 +60,8 @@ SMALL = [
     ((256, 128, 256), 2),       # several TMA boxes per tile on x, slab boxes spanning whole slabs on y
     ((64, 512, 64), 1),         # L = 512 > 256: slab boxes are parts of one slab
     ((384, 192, 48), 12),       # 3*2^a lengths through the TMA path
+    ((1536, 8, 32), 4),         # Nx = 1536: x passes as two 768-point half tiles with the shifted windows of odd rows
+    ((1536, 32, 64), 16),
     ((8, 2048, 16), 4),         # Ny = 2048: y passes as two half tiles + a radix-2 combine (fft_split2.cuh)
     ((128, 2048, 16), 128),     # ... with slab boxes spanning several virtual slabs (L = 16)
 ]
