@@ -294,6 +294,14 @@ int launch_fused(const fft3d_plan_s* pl, int d, const void* in, void* out, void*
     return FFT3D_OK;
 }
 
+// fp32 X_FWD: four row classes l % 4 put every user-side window on a 32-byte sector (fft_kernels.cuh, XTile)
+bool x_fwd_cls4(const fft3d_plan_s* pl) {
+#ifdef FFT3D_TUNING
+    if (const char* e = getenv("FFT3D_CLS4")) return atoi(e) != 0 && pl->esize == 4 && pl->L % 4 == 0 && pl->M % 4 == 0;
+#endif
+    return pl->esize == 4 && pl->L % 4 == 0 && pl->M % 4 == 0;
+}
+
 // Y pass as two half tiles (fft_split2.cuh): d = 0 natural `in` -> slab `out`, d = 1 slab `in` -> natural `out`
 int launch_y_split2(const fft3d_plan_s* pl, int d, const void* in, void* out, cudaStream_t st) {
     const KernelSet* ky = pl->ky;
@@ -353,6 +361,7 @@ int launch_x_split2(const fft3d_plan_s* pl, int d, const void* in, void* out, cu
     ta.user_out = out;
     ta.tw = pl->tw_x2; ta.ntz = (int)(M / tc);
     ta.ntiles = (long long)p * (L / 2) * (2 * ta.ntz + (d == 0 ? 1 : 0));
+    if (d == 0 && x_fwd_cls4(pl)) { ta.cls4 = 1; ta.ntiles = (long long)p * (L / 4) * (4 * ta.ntz + 3); }
     ta.L = (int)L; ta.Nx = (int)Nx; ta.Mp1 = (int)Mp1; ta.in_rows = rows; ta.out_rows = pl->x_rows;
     long long g = ta.ntiles < pl->num_sms ? ta.ntiles : pl->num_sms;
     if (g <= 0) return FFT3D_OK;
@@ -715,6 +724,7 @@ int fft3d_r2c(const fft3d_plan_t* pl, const void* d_in, void* d_out, void* d_wor
         ta.user_out = d_out;
         ta.tw = pl->tw_x; ta.ntz = (int)(M / tc);
         ta.ntiles = of ? (long long)p * (L / 2) * (2 * ta.ntz + 1) : (long long)p * L * ta.ntz;
+        if (of && x_fwd_cls4(pl)) { ta.cls4 = 1; ta.ntiles = (long long)p * (L / 4) * (4 * ta.ntz + 3); }
         ta.L = (int)L; ta.Nx = (int)Nx; ta.Mp1 = (int)(M + 1); ta.in_rows = pl->x_rows; ta.out_rows = pl->x_rows;
         rc = launch_tma(kx->tma_fn[TMA_X_FWD], kx->tma_threads_x, kx->tma_smem_x, pl->num_sms, mi, mi2, mo, ta, st);
     } else {

@@ -166,6 +166,7 @@ struct TmaArgs {
     int Nx;
     int Mp1;                 // M + 1 (pitch of the user spectrum)
     int in_rows, out_rows;   // rows per TMA box on each side
+    int cls4;                // X_FWD, fp32: four row classes l % 4 (every user-side window on a 32-byte sector)
 };
 
 namespace tma {
@@ -205,6 +206,16 @@ __device__ __forceinline__ void store3(const void* map, const void* src, int c0,
 __device__ __forceinline__ void store4(const void* map, const void* src, int c0, int c1, int c2, int c3) {
     asm volatile("cp.async.bulk.tensor.4d.global.shared::cta.bulk_group [%0, {%2, %3, %4, %5}], [%1];"
                  ::"l"(map), "r"(smem_u32(src)), "r"(c0), "r"(c1), "r"(c2), "r"(c3) : "memory");
+}
+// bulk tensor store with an L2 eviction-priority hint
+__device__ __forceinline__ unsigned long long make_policy_evict_last() {
+    unsigned long long p;
+    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+__device__ __forceinline__ void store3_hint(const void* map, const void* src, int c0, int c1, int c2, unsigned long long pol) {
+    asm volatile("cp.async.bulk.tensor.3d.global.shared::cta.bulk_group.L2::cache_hint [%0, {%2, %3, %4}], [%1], %5;"
+                 ::"l"(map), "r"(smem_u32(src)), "r"(c0), "r"(c1), "r"(c2), "l"(pol) : "memory");
 }
 __device__ __forceinline__ void store_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void store_wait_read0() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
@@ -249,12 +260,50 @@ struct TmaTile {
 //          covered by one extra thin tile whose single useful column is stored with plain 8-byte stores.
 //   X_INV  load user cols [w*TC-1, w*TC+TC+1), transform cols w*TC.., store the aligned packed window.
 // Tiles are enumerated per row pair (l even, l+1): ntz even-row tiles, then the odd-row tiles.
-struct XTile { int q, l, w, odd, thin; };
+// X_FWD with four row classes (fp32, L % 4 == 0).  Element (l, k) of the user spectrum sits at 8-byte word
+// l*(M+1) + k and M+1 = 1 (mod 4), so a 64-byte window of row l starts on a 32-byte sector iff k0 = -l (mod 4):
+//   l % 4 = 0: k0 = w*TC             l % 4 = 1: k0 = w*TC - 1 (+ thin tile for column M-1)
+//   l % 4 = 2: k0 = w*TC - 2, except the first window (k0 = 0, unshifted: its left neighbours are the previous
+//              row's last real columns) and a thin tile for columns M-2, M-1
+//   l % 4 = 3: k0 = w*TC + 1 (the last window runs into the row's own Nyquist slot) + a thin tile for column 0
+// With two classes only (even / odd l) half of the windows straddle sectors; their partial sectors are read
+// back from DRAM before they are written whenever the neighbouring tile is not quick enough (ncu at 2048^3:
+// 50.7 GB read for 34.4).  odd = the window starts at an odd column: the loading side fetches TC+2 columns
+// from k0-1.  Thin tiles store columns [c_lo, c_hi) of their window with plain stores.
+struct XTile { int q, l, w, odd, thin, k0, c_lo, c_hi; };
 
 template <int PASS, bool ODDFIX>
-__device__ __forceinline__ XTile decode_xtile(long long t_id, const TmaArgs& a) {
+__device__ __forceinline__ XTile decode_xtile(long long t_id, const TmaArgs& a, int TC = 0) {
     XTile x;
+    x.c_lo = 0; x.c_hi = 1;
     if constexpr (ODDFIX) {
+        if (PASS == TMA_X_FWD && a.cls4) {
+            const int M = a.Mp1 - 1;
+            const int per_quad = 4 * a.ntz + 3;
+            const long long qd = t_id / per_quad;
+            int r = (int)(t_id % per_quad);
+            const int quads = a.L / 4;
+            x.q = (int)(qd / quads);
+            const int l4 = (int)(qd % quads);
+            int cls, idx;
+            if (r < a.ntz) { cls = 0; idx = r; }
+            else { r -= a.ntz; cls = 1 + r / (a.ntz + 1); idx = r % (a.ntz + 1); }
+            x.l = 4 * l4 + cls;
+            x.w = idx;
+            x.thin = 0;
+            if (cls == 0) x.k0 = idx * TC;
+            else if (cls == 1) { x.k0 = idx * TC - 1; x.thin = idx == a.ntz; }
+            else if (cls == 2) {
+                if (idx == 0) x.k0 = 0;
+                else if (idx < a.ntz) x.k0 = idx * TC - 2;
+                else { x.k0 = M - 2; x.thin = 1; x.c_hi = 2; }
+            } else {
+                if (idx < a.ntz) x.k0 = idx * TC + 1;
+                else { x.k0 = 1 - TC; x.thin = 1; x.c_lo = TC - 1; x.c_hi = TC; }
+            }
+            x.odd = x.k0 & 1;
+            return x;
+        }
         const int per_pair = 2 * a.ntz + (PASS == TMA_X_FWD ? 1 : 0);
         const long long pr = t_id / per_pair;
         const int r = (int)(t_id % per_pair);
@@ -272,6 +321,7 @@ __device__ __forceinline__ XTile decode_xtile(long long t_id, const TmaArgs& a) 
         x.odd = 0;
         x.thin = 0;
     }
+    x.k0 = x.w * TC - x.odd;
     return x;
 }
 
@@ -323,15 +373,15 @@ fft_strided_tma_kernel(const __grid_constant__ TensorMapBlob in_map, const __gri
                     else tma::load4(d, &in_map, &full[s], tz * TC * W, r0 % a.L, x, r0 / a.L);                  // slab
                 }
             } else {
-                const XTile xt = decode_xtile<PASS, ODDFIX>(t_id, a);
+                const XTile xt = decode_xtile<PASS, ODDFIX>(t_id, a, TC);
                 const int rowb = xt.odd ? TT::ROW_BYTES_WIDE : TT::ROW_BYTES;
                 tma::mbar_expect_tx(&full[s], (unsigned)(Cfg::N * rowb));
                 for (int b = 0; b < nb; ++b) {
                     void* d = dst + (size_t)b * a.in_rows * rowb;
                     const int r0 = b * a.in_rows;
                     if constexpr (PASS == TMA_X_FWD) {           // packed slab, tile (q, l)
-                        if (!xt.odd) tma::load4(d, &in_map, &full[s], xt.w * TC * W, xt.l, r0, xt.q);
-                        else tma::load4(d, &in_map2, &full[s], (xt.w * TC - 2) * W, xt.l, r0, xt.q);
+                        if (!xt.odd) tma::load4(d, &in_map, &full[s], xt.k0 * W, xt.l, r0, xt.q);
+                        else tma::load4(d, &in_map2, &full[s], (xt.k0 - 1) * W, xt.l, r0, xt.q);
                     } else {                                     // user spectrum, rows of one (q,x) flattened
                         if (!xt.odd) tma::load3(d, &in_map, &full[s], (xt.l * a.Mp1 + xt.w * TC) * W, r0, xt.q);
                         else tma::load3(d, &in_map2, &full[s], (xt.l * a.Mp1 + xt.w * TC - 1) * W, r0, xt.q);
@@ -339,6 +389,9 @@ fft_strided_tma_kernel(const __grid_constant__ TensorMapBlob in_map, const __gri
                 }
             }
         };
+        // X_FWD: half of the 64-byte windows straddle sectors of the user array; keep the partial sectors in L2
+        // until the neighbouring tile completes them (otherwise they are read back from DRAM before the write)
+        const unsigned long long pol_keep = tma::make_policy_evict_last();
         auto issue_store = [=, &out_map](long long i) {
             const long long t_id = first + i * stride;
             const int s = (int)(i % NSTAGE);
@@ -354,13 +407,13 @@ fft_strided_tma_kernel(const __grid_constant__ TensorMapBlob in_map, const __gri
                     else tma::store3(&out_map, d, tz * TC * W, r0, x);                                              // -> natural
                 }
             } else {
-                const XTile xt = decode_xtile<PASS, ODDFIX>(t_id, a);
+                const XTile xt = decode_xtile<PASS, ODDFIX>(t_id, a, TC);
                 if (xt.thin) return;                             // stored by the consumers
                 for (int b = 0; b < nb; ++b) {
                     const void* d = src + (size_t)b * a.out_rows * TT::ROW_BYTES;
                     const int r0 = b * a.out_rows;
                     if constexpr (PASS == TMA_X_FWD)             // -> user spectrum (window shifted by -1 on odd rows)
-                        tma::store3(&out_map, d, (xt.l * a.Mp1 + xt.w * TC - xt.odd) * W, r0, xt.q);
+                        tma::store3_hint(&out_map, d, (xt.l * a.Mp1 + xt.k0) * W, r0, xt.q, pol_keep);
                     else                                         // -> packed slab
                         tma::store4(&out_map, d, xt.w * TC * W, xt.l, r0, xt.q);
                 }
@@ -392,7 +445,7 @@ fft_strided_tma_kernel(const __grid_constant__ TensorMapBlob in_map, const __gri
         const int s = (int)(i % NSTAGE);
         C* buf = reinterpret_cast<C*>(stages + s * TT::STAGE_BYTES);
         XTile xt{};
-        if constexpr (XPASS) xt = decode_xtile<PASS, ODDFIX>(first + i * stride, a);
+        if constexpr (XPASS) xt = decode_xtile<PASS, ODDFIX>(first + i * stride, a, TC);
         tma::mbar_wait(&full[s], (unsigned)((i / NSTAGE) & 1));
 #ifdef FFT3D_COPY_ONLY   // experiment: data movement without the transform (wrong results by design)
         tma::fence_proxy_async(); __syncwarp();
@@ -405,11 +458,11 @@ fft_strided_tma_kernel(const __grid_constant__ TensorMapBlob in_map, const __gri
         if constexpr (Cfg::NST > 1) sync();                      // all inputs read: slot becomes the exchange buffer
         fft_stages<Cfg, 0, DIR, T>(v, buf, tw, t, padded, sync);
         if (PASS == TMA_X_FWD && ODDFIX && xt.thin) {
-            // thin tile: only column M-1 (thread column 0) is real; plain 8-byte stores to the user's rows
-            if (c == 0) {
+            // thin tile: only columns [c_lo, c_hi) of the window are real; plain 8-byte stores to the user's rows
+            if (c >= xt.c_lo && c < xt.c_hi) {
                 const long long rstride = (long long)a.L * a.Mp1;
                 C* p = reinterpret_cast<C*>(a.user_out) +
-                       (((long long)xt.q * a.Nx * a.L + xt.l) * a.Mp1 + (a.Mp1 - 2)) + t * rstride;
+                       (((long long)xt.q * a.Nx * a.L + xt.l) * a.Mp1 + (xt.k0 + c)) + t * rstride;
 #pragma unroll
                 for (int m = 0; m < P; ++m) { *p = v[m]; p += rstride * S; }
             }

@@ -186,7 +186,7 @@ fft_x_split2_kernel(const __grid_constant__ TensorMapBlob ld_even, const __grid_
     if (is_producer) {
         if (tid != NCONS) return;
         auto issue_load = [=, &ld_even, &ld_odd, &ldw_even, &ldw_odd](long long i) {
-            const XTile xt = decode_xtile<PASS, true>(first + (i >> 1) * stride, a);
+            const XTile xt = decode_xtile<PASS, true>(first + (i >> 1) * stride, a, TC);
             const int h = (int)(i & 1), s = (int)(i % NSTAGE);
             unsigned char* dst = stages + s * TT::STAGE_BYTES;
             const int rowb = xt.odd ? TT::ROW_BYTES_WIDE : TT::ROW_BYTES;
@@ -197,13 +197,14 @@ fft_x_split2_kernel(const __grid_constant__ TensorMapBlob ld_even, const __grid_
                 void* d = dst + (size_t)b * a.in_rows * rowb;
                 const int r0 = b * a.in_rows;                    // index among the even (odd) x rows
                 if constexpr (PASS == TMA_X_FWD)
-                    tma::load4(d, map, &full[s], (xt.w * TC - 2 * xt.odd) * W, xt.l, r0, xt.q);
+                    tma::load4(d, map, &full[s], (xt.k0 - xt.odd) * W, xt.l, r0, xt.q);
                 else
                     tma::load3(d, map, &full[s], (xt.l * a.Mp1 + xt.w * TC - xt.odd) * W, r0, xt.q);
             }
         };
+        const unsigned long long pol_keep = tma::make_policy_evict_last();   // see fft_strided_tma_kernel
         auto issue_store = [=, &out_map](long long i) {
-            const XTile xt = decode_xtile<PASS, true>(first + (i >> 1) * stride, a);
+            const XTile xt = decode_xtile<PASS, true>(first + (i >> 1) * stride, a, TC);
             if (xt.thin) return;                                 // stored by the consumers
             const int h = (int)(i & 1), s = (int)(i % NSTAGE);
             const unsigned char* src = stages + s * TT::STAGE_BYTES;
@@ -212,7 +213,7 @@ fft_x_split2_kernel(const __grid_constant__ TensorMapBlob ld_even, const __grid_
                 const void* d = src + (size_t)b * a.out_rows * TT::ROW_BYTES;
                 const int r0 = h * H + b * a.out_rows;
                 if constexpr (PASS == TMA_X_FWD)
-                    tma::store3(&out_map, d, (xt.l * a.Mp1 + xt.w * TC - xt.odd) * W, r0, xt.q);
+                    tma::store3_hint(&out_map, d, (xt.l * a.Mp1 + xt.k0) * W, r0, xt.q, pol_keep);
                 else
                     tma::store4(&out_map, d, xt.w * TC * W, xt.l, r0, xt.q);
             }
@@ -248,7 +249,7 @@ fft_x_split2_kernel(const __grid_constant__ TensorMapBlob ld_even, const __grid_
     sincospi((double)DIR * (double)t / (double)H, &ws, &wc);
     const C wt = mk<T>((T)wc, (T)ws);
     for (long long i = 0; i < n_items; ++i) {
-        const XTile xt = decode_xtile<PASS, true>(first + (i >> 1) * stride, a);
+        const XTile xt = decode_xtile<PASS, true>(first + (i >> 1) * stride, a, TC);
         const int s = (int)(i % NSTAGE);
         C* buf = reinterpret_cast<C*>(stages + s * TT::STAGE_BYTES);
         tma::mbar_wait(&full[s], (unsigned)((i / NSTAGE) & 1));
@@ -266,10 +267,10 @@ fft_x_split2_kernel(const __grid_constant__ TensorMapBlob ld_even, const __grid_
             if (PASS == TMA_X_FWD && xt.thin) {
                 // thin tile: only column M-1 (thread column 0) is real; plain stores to the user's rows
                 __syncwarp();
-                if (c == 0) {
+                if (c >= xt.c_lo && c < xt.c_hi) {
                     const long long rstride = (long long)a.L * a.Mp1;
                     C* p = reinterpret_cast<C*>(a.user_out) +
-                           (((long long)xt.q * a.Nx * a.L + xt.l) * a.Mp1 + (a.Mp1 - 2));
+                           (((long long)xt.q * a.Nx * a.L + xt.l) * a.Mp1 + (xt.k0 + c));
 #pragma unroll
                     for (int m = 0; m < P; ++m) {
                         const int k = t + m * S;
