@@ -83,6 +83,9 @@ struct fft3d_plan_s {
     bool split_x;              // X passes as two half tiles (R2C/C2R plans)
     void* tw_x2;               // stage twiddles of the Nx/2-point transform
     int x2_rows;               // rows per TMA box of the even/odd x-row views
+    bool split4_x;             // X passes as four quarter tiles
+    void* tw_x4;               // stage twiddles of the Nx/4-point transform
+    int x4_rows;
     int y2_rows_nat, y2_rows_slab;   // rows per TMA box of the even/odd row views
     bool bulk_z;               // bulk-pipelined z kernels usable (row count a multiple of the tile)
     int y_rows_nat, y_rows_slab, x_rows;   // rows per TMA box
@@ -371,6 +374,45 @@ int launch_x_split2(const fft3d_plan_s* pl, int d, const void* in, void* out, cu
     return FFT3D_OK;
 }
 
+// X pass as four quarter tiles (fft_split2.cuh, fft_x_split4_kernel): d = 0 packed slab -> user spectrum, d = 1 reverse
+int launch_x_split4(const fft3d_plan_s* pl, int d, const void* in, void* out, cudaStream_t st) {
+    const KernelSet* kx = pl->kx;
+    const long long sz = 2 * pl->esize, W = sz / 8, M = pl->M, L = pl->L, Nx = pl->Nx, p = pl->p, Mp1 = M + 1;
+    const int tc = kx->tma_tc_x, rows = pl->x4_rows;
+    Split4Maps maps;
+    TensorMapBlob mo;
+    for (int wide = 0; wide < 2; ++wide)
+        for (int m = 0; m < 4; ++m) {
+            const int cols = tc + 2 * wide;
+            bool ok;
+            if (d == 0) {
+                const unsigned char* base = reinterpret_cast<const unsigned char*>(in) + (size_t)m * L * M * sz;
+                long long dm[4] = {M * W, L, Nx / 4, p}, sb[3] = {M * sz, 4 * L * M * sz, Nx * L * M * sz};
+                int bx[4] = {(int)(cols * W), 1, rows, 1};
+                ok = make_map(pl, &maps.ld[wide][m], base, 4, dm, sb, bx);
+            } else {
+                const unsigned char* base = reinterpret_cast<const unsigned char*>(in) + (size_t)m * L * Mp1 * sz;
+                long long dm[3] = {L * Mp1 * W, Nx / 4, p}, sb[2] = {4 * L * Mp1 * sz, Nx * L * Mp1 * sz};
+                int bx[3] = {(int)(cols * W), rows, 1};
+                ok = make_map(pl, &maps.ld[wide][m], base, 3, dm, sb, bx);
+            }
+            if (!ok) return FFT3D_ECUDA;
+        }
+    if (!(d == 0 ? map_user_x(pl, &mo, out, tc, pl->x_rows) : map_slab_x(pl, &mo, out, tc, pl->x_rows))) return FFT3D_ECUDA;
+    TmaArgs ta{};
+    ta.user_out = out;
+    ta.tw = pl->tw_x4; ta.ntz = (int)(M / tc);
+    ta.ntiles = (long long)p * (L / 2) * (2 * ta.ntz + (d == 0 ? 1 : 0));
+    if (d == 0 && x_fwd_cls4(pl)) { ta.cls4 = 1; ta.ntiles = (long long)p * (L / 4) * (4 * ta.ntz + 3); }
+    ta.L = (int)L; ta.Nx = (int)Nx; ta.Mp1 = (int)Mp1; ta.in_rows = rows; ta.out_rows = pl->x_rows;
+    long long g = ta.ntiles < pl->num_sms ? ta.ntiles : pl->num_sms;
+    if (g <= 0) return FFT3D_OK;
+    void* argv[3] = {(void*)&maps, (void*)&mo, (void*)&ta};
+    cudaError_t e = cudaLaunchKernel(kx->x4_fn[d], dim3((unsigned)g), dim3((unsigned)kx->x4_threads), argv, kx->x4_smem, st);
+    if (e != cudaSuccess) { cudaGetLastError(); return FFT3D_ECUDA; }
+    return FFT3D_OK;
+}
+
 // event slot `i` of the call being recorded for direction `which`, or no-op
 struct Recorder {
     TimingState* t;
@@ -494,6 +536,15 @@ static int plan_create(fft3d_plan_t** out, long long Nx, long long Ny, long long
             for (int d = 0; d < 2 && rc == FFT3D_OK; ++d) {
                 int g = 0;
                 rc = prepare_kernel(kx->tma_fn[d == 0 ? TMA_X_FWD : TMA_X_INV], kx->tma_threads_x, kx->tma_smem_x, sms, &g);
+            }
+            if (rc == FFT3D_OK && kx->x4_fn[0] != nullptr && kx->tma_oddfix && Nx % 4 == 0 && (Nx / 4) % pl->x_rows == 0) {
+                pl->split4_x = true;
+                pl->x4_rows = (int)largest_divisor_le(Nx / 4, 256);
+                for (int d = 0; d < 2 && rc == FFT3D_OK; ++d) {
+                    int g = 0;
+                    rc = prepare_kernel(kx->x4_fn[d], kx->x4_threads, kx->x4_smem, sms, &g);
+                }
+                if (rc == FFT3D_OK) rc = upload_stage_twiddles(kx->x4_nst, kx->x4_radix, kx->x4_twn, pl->esize, &pl->tw_x4);
             }
             if (rc == FFT3D_OK && kx->x2_fn[0] != nullptr && kx->tma_oddfix && Nx % 2 == 0 && (Nx / 2) % pl->x_rows == 0) {
                 pl->split_x = true;
@@ -712,6 +763,8 @@ int fft3d_r2c(const fft3d_plan_t* pl, const void* d_in, void* d_out, void* d_wor
     b.ntiles = (long long)p * L * b.ntz;
     b.in_hi = Nx * L * M; b.in_lo = M; b.in_rq = 0; b.in_rl = L * M;
     b.out_hi = Nx * L * (M + 1); b.out_lo = M + 1; b.out_rq = 0; b.out_rl = L * (M + 1);
+    // (the quarter-tile kernel is used for the inverse only: measured at 2048^3, F3 25.1 ms against 23.4 ms whole
+    // tiles -- its thin tiles cost four loads each -- but I1 20.0 against 22.8)
     if (tma_on && pl->split_x && pl->variant != 2) {
         rc = launch_x_split2(pl, 0, d_work, d_out, st);
     } else if (tma_on && pl->tma_x) {
@@ -786,7 +839,8 @@ int fft3d_c2r(const fft3d_plan_t* pl, const void* d_in, void* d_out, void* d_wor
         ta.tw = pl->tw_x; ta.ntz = (int)(M / tc);
         ta.ntiles = of ? (long long)p * (L / 2) * (2 * ta.ntz) : (long long)p * L * ta.ntz;
         ta.L = (int)L; ta.Nx = (int)Nx; ta.Mp1 = (int)(M + 1); ta.in_rows = pl->x_rows; ta.out_rows = pl->x_rows;
-        if (pl->split_x && pl->variant != 2) rc = launch_x_split2(pl, 1, d_in, x_out, st);
+        if (pl->split4_x && pl->variant != 2) rc = launch_x_split4(pl, 1, d_in, x_out, st);
+        else if (pl->split_x && pl->variant != 2) rc = launch_x_split2(pl, 1, d_in, x_out, st);
         else rc = launch_tma(kx->tma_fn[TMA_X_INV], kx->tma_threads_x, kx->tma_smem_x, pl->num_sms, mi, mi2, mo, ta, st);
         rec.mark(slot++);
         // packed column 0 of the result: x-transform of the side buffer, written over the (meaningless)
@@ -1051,7 +1105,7 @@ int fft3d_c2r_host(fft3d_plan_t* pl, const void* h_in, void* h_out) {
 
 int fft3d_destroy(fft3d_plan_t* pl) {
     if (pl == nullptr) return FFT3D_OK;
-    cudaFree(pl->tw_zb); cudaFree(pl->tw_zc); cudaFree(pl->tw_y2); cudaFree(pl->tw_x2); cudaFree(pl->tw_z); cudaFree(pl->tw_y); cudaFree(pl->tw_x); cudaFree(pl->twz);
+    cudaFree(pl->tw_zb); cudaFree(pl->tw_zc); cudaFree(pl->tw_y2); cudaFree(pl->tw_x2); cudaFree(pl->tw_x4); cudaFree(pl->tw_z); cudaFree(pl->tw_y); cudaFree(pl->tw_x); cudaFree(pl->twz);
     cudaFree(pl->h_real); cudaFree(pl->h_cplx); cudaFree(pl->h_work);
     if (pl->h_stream) cudaStreamDestroy(pl->h_stream);
     timing_free(pl);

@@ -80,6 +80,34 @@ static void add_split2(KernelSet& k) {
     }
 }
 
+// X passes of length N as four N/4-point quarter tiles (where neither the whole nor the half tile pipelines)
+template <typename T, int N>
+static void add_split4(KernelSet& k) {
+    if constexpr (N >= 1024 && N % 4 == 0) {
+        using C = cx<T>;
+        using Cfg = typename CfgFor<T, N>::type;
+        using HCfg = typename CfgFor<T, N / 2>::type;
+        using QCfg = typename CfgFor<T, N / 4>::type;
+        constexpr int TTC = tma_tile_cols(Cfg::N, Cfg::S, (int)sizeof(C));
+        constexpr int QTC = tma_tile_cols(QCfg::N, QCfg::S, (int)sizeof(C));
+        if constexpr (TTC > 0 && QTC == TTC) {
+            using TXW = TmaTile<Cfg, TTC, T, true>;
+            using THW = TmaTile<HCfg, TTC, T, true>;
+            using TQW = TmaTile<QCfg, TTC, T, true>;
+            constexpr int NS = 5;
+            if constexpr (TXW::max_stages() <= 1 && THW::max_stages() < 3 && TQW::smem_bytes(NS) <= 227 * 1024) {
+                k.x4_fn[0] = (const void*)fft_x_split4_kernel<QCfg, TTC, TMA_X_FWD, T, NS>;
+                k.x4_fn[1] = (const void*)fft_x_split4_kernel<QCfg, TTC, TMA_X_INV, T, NS>;
+                k.x4_threads = TQW::NCONS + 32;
+                k.x4_smem = (size_t)TQW::smem_bytes(NS);
+                k.x4_nst = QCfg::NST;
+                for (int s = 0; s < 5; ++s) k.x4_radix[s] = s < QCfg::NST ? QCfg::radix(s) : 1;
+                k.x4_twn = QCfg::TWN;
+            }
+        }
+    }
+}
+
 // fused z+y kernels of C2C plans with Nz == Ny == N
 template <typename T, int N>
 static void add_fused_c2c(KernelSet& k) {
@@ -224,6 +252,7 @@ static KernelSet make_set(int dtype) {
     add_fused<T, FFT3D_N>(k);
     add_fused_c2c<T, FFT3D_N>(k);
     add_split2<T, FFT3D_N>(k);
+    add_split4<T, FFT3D_N>(k);
     return k;
 }
 

@@ -47,6 +47,9 @@ struct KernelSet {
     const void* x2_fn[2];      // the same for the X passes with shifted windows: [0 = X_FWD, 1 = X_INV]
     int x2_threads;
     size_t x2_smem;
+    const void* x4_fn[2];      // X passes as four quarter tiles + a radix-4 combine
+    int x4_threads, x4_nst, x4_radix[5], x4_twn;   // x4_nst.. = the factorisation of the N/4-point transform
+    size_t x4_smem;
     // C2C row kernels (z pass of the 3D C2C transform): the bulk-pipelined kernel without the Hermitian step
     const void* zc_fn[2];      // [0 = forward, 1 = inverse (scaled)]
     int zc_rpt, zc_nst, zc_radix[5], zc_twn, zc_threads;

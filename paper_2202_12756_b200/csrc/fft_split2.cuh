@@ -286,4 +286,168 @@ fft_x_split2_kernel(const __grid_constant__ TensorMapBlob ld_even, const __grid_
     }
 }
 
+// ---------------------------------------------------------------------------------------------
+// Two decimation-in-time steps taken out of the tile: the X passes of Nx = 2048 fp32, whose odd-row half
+// tiles land 80 KiB (three slots do not fit) but whose QUARTER tiles land 40 KiB (five slots do).  Rows
+// x = 4k + m, m = 0..3, are four independent Nx/4-point transforms Q_m; when the fourth is done
+//     X[k + j Nx/4] = sum_m (-+i)^(j m) w^(m k) Q_m[k],   w = exp(-+2 pi i / Nx),
+// element by element (a radix-4 butterfly on the thread's own elements, no barrier), and the four slots hold
+// output rows [j Nx/4, (j+1) Nx/4).  Loads: ld[wide][m] = rows x = m (mod 4) of the loading side, plain / wide.
+// ---------------------------------------------------------------------------------------------
+struct Split4Maps { TensorMapBlob ld[2][4]; };
+
+template <class QCfg, int DIR, typename T, class Lay, int MM = 0>
+__device__ __forceinline__ void combine_quarters(cx<T> (&v)[QCfg::P], cx<T>* q0, cx<T>* q1, cx<T>* q2, cx<T>* q3,
+                                                 const cx<T> (&wt)[3], int t, const Lay& lay, cx<T>* thin_p, long long rstride,
+                                                 bool thin) {
+    if constexpr (MM < QCfg::P) {
+        constexpr int P = QCfg::P, S = QCfg::S, H4 = QCfg::N;
+        const int k = t + MM * S, idx = lay.at(k);
+        cx<T> a[4];
+        a[0] = q0[idx];
+        a[1] = cmul(mul_root<MM, 4 * P, DIR, T>(wt[0]), q1[idx]);
+        a[2] = cmul(mul_root<2 * MM, 4 * P, DIR, T>(wt[1]), q2[idx]);
+        a[3] = cmul(mul_root<3 * MM, 4 * P, DIR, T>(wt[2]), v[MM]);
+        dft<4, DIR, T>(a);
+        if (thin) {
+            if (thin_p != nullptr) {
+#pragma unroll
+                for (int j = 0; j < 4; ++j) thin_p[(long long)(k + j * H4) * rstride] = a[j];
+            }
+        } else {
+            q0[idx] = a[0]; q1[idx] = a[1]; q2[idx] = a[2]; q3[idx] = a[3];
+        }
+        combine_quarters<QCfg, DIR, T, Lay, MM + 1>(v, q0, q1, q2, q3, wt, t, lay, thin_p, rstride, thin);
+    }
+}
+
+template <class QCfg, int TC, int PASS, typename T, int NSTAGE>
+__global__ void __launch_bounds__(QCfg::S * TC + 32, 1)
+fft_x_split4_kernel(const __grid_constant__ Split4Maps maps, const __grid_constant__ TensorMapBlob out_map, const TmaArgs a) {
+    using C = cx<T>;
+    using TT = TmaTile<QCfg, TC, T, true>;
+    constexpr int P = QCfg::P, W = TT::W, NCONS = TT::NCONS, H4 = QCfg::N;
+    constexpr int DIR = (PASS == TMA_X_FWD) ? -1 : +1;
+    static_assert(PASS == TMA_X_FWD || PASS == TMA_X_INV, "X passes only");
+    static_assert(NSTAGE >= 5, "four quarter tiles plus one in flight");
+    extern __shared__ __align__(1024) unsigned char smem_dyn[];
+    C* tw = reinterpret_cast<C*>(smem_dyn);
+    unsigned char* stages = smem_dyn + TT::TW_BYTES;
+    unsigned long long* full = reinterpret_cast<unsigned long long*>(stages + NSTAGE * TT::STAGE_BYTES);
+    unsigned long long* done = full + NSTAGE;
+
+    const int tid = threadIdx.x;
+    const bool is_producer = tid >= NCONS;
+    if (tid == NCONS) {
+        for (int s = 0; s < NSTAGE; ++s) { tma::mbar_init(&full[s], 1); tma::mbar_init(&done[s], NCONS / 32); }
+        tma::fence_mbar_init();
+    }
+    if (!is_producer) load_twiddles<DIR, T>(tw, reinterpret_cast<const C*>(a.tw), QCfg::TWN, tid, NCONS);
+    __syncthreads();
+
+    const long long first = blockIdx.x, stride = gridDim.x;
+    const long long n_tiles = first < a.ntiles ? (a.ntiles - first + stride - 1) / stride : 0;
+    const long long n_items = 4 * n_tiles;               // item i = (tile i/4, quarter i&3)
+
+    if (is_producer) {
+        if (tid != NCONS) return;
+        const unsigned long long pol_keep = tma::make_policy_evict_last();
+        auto issue_load = [=, &maps](long long i) {
+            const XTile xt = decode_xtile<PASS, true>(first + (i >> 2) * stride, a, TC);
+            const int m = (int)(i & 3), s = (int)(i % NSTAGE);
+            unsigned char* dst = stages + s * TT::STAGE_BYTES;
+            const int rowb = xt.odd ? TT::ROW_BYTES_WIDE : TT::ROW_BYTES;
+            const TensorMapBlob* map = &maps.ld[xt.odd][m];
+            const int nb = H4 / a.in_rows;
+            tma::mbar_expect_tx(&full[s], (unsigned)(H4 * rowb));
+            for (int b = 0; b < nb; ++b) {
+                void* d = dst + (size_t)b * a.in_rows * rowb;
+                const int r0 = b * a.in_rows;
+                if constexpr (PASS == TMA_X_FWD)
+                    tma::load4(d, map, &full[s], (xt.k0 - xt.odd) * W, xt.l, r0, xt.q);
+                else
+                    tma::load3(d, map, &full[s], (xt.l * a.Mp1 + xt.w * TC - xt.odd) * W, r0, xt.q);
+            }
+        };
+        auto issue_store = [=, &out_map](long long i) {
+            const XTile xt = decode_xtile<PASS, true>(first + (i >> 2) * stride, a, TC);
+            if (xt.thin) return;
+            const int j = (int)(i & 3), s = (int)(i % NSTAGE);
+            const unsigned char* src = stages + s * TT::STAGE_BYTES;
+            const int nb = H4 / a.out_rows;
+            for (int b = 0; b < nb; ++b) {
+                const void* d = src + (size_t)b * a.out_rows * TT::ROW_BYTES;
+                const int r0 = j * H4 + b * a.out_rows;
+                if constexpr (PASS == TMA_X_FWD)
+                    tma::store3_hint(&out_map, d, (xt.l * a.Mp1 + xt.k0) * W, r0, xt.q, pol_keep);
+                else
+                    tma::store4(&out_map, d, xt.w * TC * W, xt.l, r0, xt.q);
+            }
+        };
+        long long stored_tiles = 0;
+        auto ensure_stored = [&](long long j) {
+            const long long tl = j >> 2;
+            if (tl < stored_tiles) return;
+            for (long long k = 4 * tl; k < 4 * tl + 4; ++k)
+                tma::mbar_wait(&done[k % NSTAGE], (unsigned)((k / NSTAGE) & 1));
+            for (long long k = 4 * tl; k < 4 * tl + 4; ++k) issue_store(k);
+            tma::store_commit();
+            tma::store_wait_read0();
+            stored_tiles = tl + 1;
+        };
+        for (long long i = 0; i < n_items; ++i) {
+            if (i >= NSTAGE) ensure_stored(i - NSTAGE);
+            issue_load(i);
+        }
+        for (long long tl = stored_tiles; tl < n_tiles; ++tl) ensure_stored(4 * tl);
+        tma::store_wait_all();
+        return;
+    }
+
+    // ---------------- consumers ----------------
+    const int c = tid % TC, t = tid / TC;
+    const SmLayout<TC, 0> dense{c};
+    const SmLayout<TC + 2, 0> dense_wide{c + 1};
+    const SmLayout<TC, TT::PADR> padded{c};
+    const NamedSync<1, NCONS> sync{};
+    C wt[3];                                             // w^(j t), j = 1..3, w = exp(DIR 2 pi i / N), N = 4 H4
+#pragma unroll
+    for (int j = 1; j <= 3; ++j) {
+        double ws, wc;
+        sincospi((double)DIR * (double)(j * t) / (double)(2 * H4), &ws, &wc);
+        wt[j - 1] = mk<T>((T)wc, (T)ws);
+    }
+    for (long long i = 0; i < n_items; ++i) {
+        const XTile xt = decode_xtile<PASS, true>(first + (i >> 2) * stride, a, TC);
+        const int s = (int)(i % NSTAGE);
+        C* buf = reinterpret_cast<C*>(stages + s * TT::STAGE_BYTES);
+        tma::mbar_wait(&full[s], (unsigned)((i / NSTAGE) & 1));
+        C v[P];
+        if (xt.odd) read_own<QCfg, T>(v, buf, t, dense_wide);
+        else read_own<QCfg, T>(v, buf, t, dense);
+        if constexpr (QCfg::NST > 1) sync();
+        fft_stages<QCfg, 0, DIR, T>(v, buf, tw, t, padded, sync);
+        if constexpr (QCfg::NST > 1) sync();
+        if ((i & 3) != 3) {
+            write_own<QCfg, T>(v, buf, t, dense);
+        } else {
+            C* q0 = reinterpret_cast<C*>(stages + (int)((i - 3) % NSTAGE) * TT::STAGE_BYTES);
+            C* q1 = reinterpret_cast<C*>(stages + (int)((i - 2) % NSTAGE) * TT::STAGE_BYTES);
+            C* q2 = reinterpret_cast<C*>(stages + (int)((i - 1) % NSTAGE) * TT::STAGE_BYTES);
+            const bool thin = PASS == TMA_X_FWD && xt.thin;
+            const long long rstride = (long long)a.L * a.Mp1;
+            C* thin_p = nullptr;
+            if (thin && c >= xt.c_lo && c < xt.c_hi)
+                thin_p = reinterpret_cast<C*>(a.user_out) + (((long long)xt.q * a.Nx * a.L + xt.l) * a.Mp1 + (xt.k0 + c));
+            combine_quarters<QCfg, DIR, T>(v, q0, q1, q2, buf, wt, t, dense, thin_p, rstride, thin);
+            tma::fence_proxy_async();
+            __syncwarp();
+            if ((tid & 31) == 0) {
+#pragma unroll
+                for (int j = 0; j < 4; ++j) tma::mbar_arrive(&done[(i - 3 + j) % NSTAGE]);
+            }
+        }
+    }
+}
+
 }  // namespace fft3d
