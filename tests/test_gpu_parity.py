@@ -62,6 +62,7 @@ SMALL = [
     ((384, 192, 48), 12),       # 3*2^a lengths through the TMA path
     ((1536, 8, 32), 4),         # Nx = 1536: x passes as two 768-point half tiles with the shifted windows of odd rows
     ((1536, 32, 64), 16),
+    ((64, 192, 64), 32),        # L = 6: the two-class shifted windows (four classes need L % 4 == 0)
     ((2048, 8, 32), 2),         # Nx = 2048: inverse x pass as four 512-point quarter tiles + a radix-4 combine
     ((2048, 16, 64), 4),
     ((8, 2048, 16), 4),         # Ny = 2048: y passes as two half tiles + a radix-2 combine (fft_split2.cuh)
