@@ -217,7 +217,14 @@ static KernelSet make_set(int dtype) {
     using ZCfg = typename ZCfgFor<T, FFT3D_N>::type;
     if constexpr (ZCfg::S >= 8 && ZCfg::S <= 32 && (ZCfg::S & (ZCfg::S - 1)) == 0 && ZCfg::P % 2 == 0 &&
                   ZCfg::N * sizeof(C) >= 1024) {
-        constexpr int RPT = 256 / ZCfg::S;
+        // fp64: 128 threads per tile (two groups + producer = 288 threads, 224 registers each: with 256-thread groups
+        // the 120-register cap made the fp64 C2R kernel spill 184 bytes per thread)
+#ifdef FFT3D_ZB64_OLD
+        constexpr int GRP = 256;
+#else
+        constexpr int GRP = sizeof(T) == 8 && ZCfg::S <= 16 * 8 && 128 % ZCfg::S == 0 ? 128 : 256;
+#endif
+        constexpr int RPT = GRP / ZCfg::S;
         using ZT = ZTile<ZCfg, RPT, T>;
         constexpr int NG = ZT::max_stages(2) >= 3 ? 2 : 1;
         constexpr int NS = ZT::max_stages(NG) > 4 ? 4 : ZT::max_stages(NG);
