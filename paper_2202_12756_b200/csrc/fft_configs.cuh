@@ -69,6 +69,9 @@ template <typename T, int N> struct ZCfgFor { using type = typename CfgFor<T, N>
 template <> struct ZCfgFor<float, 512> { using type = FftCfg<512, 32, 32, 16>; };
 template <> struct ZCfgFor<float, 256> { using type = FftCfg<256, 16, 16, 16>; };
 template <> struct ZCfgFor<double, 512> { using type = FftCfg<512, 16, 16, 16, 2>; };
+// 768 = 48*16: one exchange instead of two (the z passes are shared-memory bound: 0.73 wavefronts per cycle per SM);
+// 48 points per thread need one 256-thread group with 224 registers instead of two with 120
+template <> struct ZCfgFor<float, 768> { using type = FftCfg<768, 48, 48, 16>; };
 
 // Tile width (columns) of the strided passes: 128-byte rows while the tile stays small,
 // 64-byte rows up to N = 2048, 32-byte rows beyond.

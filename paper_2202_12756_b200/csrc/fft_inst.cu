@@ -226,7 +226,7 @@ static KernelSet make_set(int dtype) {
 #endif
         constexpr int RPT = GRP / ZCfg::S;
         using ZT = ZTile<ZCfg, RPT, T>;
-        constexpr int NG = ZT::max_stages(2) >= 3 ? 2 : 1;
+        constexpr int NG = (ZT::max_stages(2) >= 3 && ZCfg::P <= 32) ? 2 : 1;      // P > 32: one group, 224 registers
         constexpr int NS = ZT::max_stages(NG) > 4 ? 4 : ZT::max_stages(NG);
         if constexpr (NS >= 2) {
             k.zb_fn[0] = (const void*)fft_z_bulk_kernel<ZCfg, RPT, -1, T, NS, NG>;
