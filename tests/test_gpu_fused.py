@@ -34,7 +34,7 @@ def fft():
 
 CASES = [
     # shape (Ny == Nz), p
-    ((128, 128, 128), 4),
+    ((128, 128, 128), 4),       # no bulk z kernel for 64-point rows: skipped (the plan falls back to the unfused passes)
     ((64, 256, 256), 8),        # fewer planes than CTAs per role; ring deeper than a role's lead
     ((256, 256, 256), 8),       # BASELINE.json configs[1] shape
     ((96, 384, 384), 12),       # 3*2^a lengths (radix 3) through the fused kernels
