@@ -17,9 +17,13 @@
  *            (the non-Hermitian part of the planes kz=0 and kz=Nz/2) are ignored exactly as
  *            that definition ignores them (reading R8).
  *
- * Pipeline (P:69-77 steps 1-5; inverse = reverse order), each line ONE kernel pass:
+ * Pipeline (P:69-77 steps 1-5; inverse = reverse order), each arrow-separated item ONE pass
+ * over the array:
  *   forward : z-axis R2C  ->  y-axis C2C + global transpose X (steps 2+3+4)  ->  x-axis C2C
  *   inverse : x-axis C2C  ->  inverse transpose + y-axis C2C  ->  z-axis C2R * 1/(NxNyNz)
+ * For large cubic-like fp32 plans the z and y passes of an x-plane run inside one kernel and
+ * exchange the plane through an L2-resident ring (two passes per direction; D:5.6).  A 3D
+ * complex-to-complex transform over the same layouts is declared further down (D:5.7).
  *
  * LAYOUTS (all dense, row-major, no padding; complex = interleaved (re, im)):
  *   real     f[jx][jy][jz]                    z fastest, x slowest
