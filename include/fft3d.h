@@ -128,6 +128,9 @@ int fft3d_plan_c2c(fft3d_plan_t **plan_out, long long Nx, long long Ny, long lon
 int fft3d_c2c(const fft3d_plan_t *plan, const void *d_cplx_in, void *d_cplx_out,
               void *d_work, int direction, void *cuda_stream);
 
+/* Host-buffer variant of fft3d_c2c (as fft3d_r2c_host below): H2D copy, transform, D2H copy, synchronous. */
+int fft3d_c2c_host(fft3d_plan_t *plan, const void *h_cplx_in, void *h_cplx_out, int direction);
+
 /* Host-buffer variants: H2D copy, transform, D2H copy, synchronous.  The plan lazily
  * allocates real + complex + workspace device buffers (fft3d_real_bytes + fft3d_complex_bytes
  * + fft3d_workspace_bytes) and keeps them until fft3d_destroy. */

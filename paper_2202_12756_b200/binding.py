@@ -19,7 +19,7 @@ EXPORTS = (
     "fft3d_plan", "fft3d_supported_length", "fft3d_workspace_bytes", "fft3d_real_bytes",
     "fft3d_complex_bytes", "fft3d_index", "fft3d_r2c", "fft3d_c2r", "fft3d_r2c_host",
     "fft3d_c2r_host", "fft3d_launches", "fft3d_launch_name", "fft3d_set_variant", "fft3d_destroy", "fft3d_strerror",
-    "fft3d_timing_enable", "fft3d_timing_read", "fft3d_plan_c2c", "fft3d_c2c",
+    "fft3d_timing_enable", "fft3d_timing_read", "fft3d_plan_c2c", "fft3d_c2c", "fft3d_c2c_host",
 )
 
 _lib = None
@@ -48,6 +48,8 @@ def load_library() -> ctypes.CDLL:
     lib.fft3d_plan_c2c.restype = i
     lib.fft3d_c2c.argtypes = [vp, vp, vp, vp, i, vp]
     lib.fft3d_c2c.restype = i
+    lib.fft3d_c2c_host.argtypes = [vp, vp, vp, i]
+    lib.fft3d_c2c_host.restype = i
     lib.fft3d_supported_length.argtypes = [ll]
     lib.fft3d_supported_length.restype = i
     for nm in ("fft3d_workspace_bytes", "fft3d_real_bytes", "fft3d_complex_bytes"):
@@ -259,6 +261,13 @@ class PlanC2C(Plan):
                                  ctypes.c_void_p(s.cuda_stream))
         if rc != 0:
             raise Fft3dError(rc, "fft3d_c2c")
+        return cplx_out
+
+    def c2c_host(self, cplx_in: torch.Tensor, cplx_out: torch.Tensor, direction: int):
+        assert not cplx_in.is_cuda and not cplx_out.is_cuda and cplx_in.is_contiguous() and cplx_out.is_contiguous()
+        rc = self._lib.fft3d_c2c_host(self._h, cplx_in.data_ptr(), cplx_out.data_ptr(), int(direction))
+        if rc != 0:
+            raise Fft3dError(rc, "fft3d_c2c_host")
         return cplx_out
 
     def to_natural(self, cplx_flat: torch.Tensor) -> torch.Tensor:

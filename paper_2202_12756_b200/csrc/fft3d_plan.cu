@@ -1054,7 +1054,7 @@ static int ensure_host_buffers(fft3d_plan_t* pl) {
         cudaGetLastError();
         return FFT3D_ECUDA;
     }
-    if (cudaMalloc(&pl->h_real, fft3d_real_bytes(pl)) != cudaSuccess ||
+    if (cudaMalloc(&pl->h_real, pl->kind == 0 ? fft3d_real_bytes(pl) : fft3d_complex_bytes(pl)) != cudaSuccess ||
         cudaMalloc(&pl->h_cplx, fft3d_complex_bytes(pl)) != cudaSuccess ||
         cudaMalloc(&pl->h_work, fft3d_workspace_bytes(pl)) != cudaSuccess) {
         cudaGetLastError();
@@ -1096,6 +1096,27 @@ int fft3d_c2r_host(fft3d_plan_t* pl, const void* h_in, void* h_out) {
     rc = fft3d_c2r(pl, pl->h_cplx, pl->h_real, pl->h_work, st);
     if (rc != FFT3D_OK) return rc;
     if (cudaMemcpyAsync(h_out, pl->h_real, fft3d_real_bytes(pl), cudaMemcpyDeviceToHost, st) != cudaSuccess ||
+        cudaStreamSynchronize(st) != cudaSuccess) {
+        cudaGetLastError();
+        return FFT3D_ECUDA;
+    }
+    return FFT3D_OK;
+}
+
+int fft3d_c2c_host(fft3d_plan_t* pl, const void* h_in, void* h_out, int direction) {
+    if (pl == nullptr || pl->kind != 1 || h_in == nullptr || h_out == nullptr) return FFT3D_EINVAL;
+    if (direction != -1 && direction != 1) return FFT3D_EINVAL;
+    int rc = ensure_host_buffers(pl);
+    if (rc != FFT3D_OK) return rc;
+    cudaStream_t st = pl->h_stream;
+    const size_t cb = fft3d_complex_bytes(pl);
+    if (cudaMemcpyAsync(pl->h_real, h_in, cb, cudaMemcpyHostToDevice, st) != cudaSuccess) {
+        cudaGetLastError();
+        return FFT3D_ECUDA;
+    }
+    rc = fft3d_c2c(pl, pl->h_real, pl->h_cplx, pl->h_work, direction, st);
+    if (rc != FFT3D_OK) return rc;
+    if (cudaMemcpyAsync(h_out, pl->h_cplx, cb, cudaMemcpyDeviceToHost, st) != cudaSuccess ||
         cudaStreamSynchronize(st) != cudaSuccess) {
         cudaGetLastError();
         return FFT3D_ECUDA;

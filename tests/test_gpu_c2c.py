@@ -156,3 +156,18 @@ def test_c2c_512_full_oracle_and_1024_properties(fft, oracle_mod):
     err = max((back[i] - f[i]).abs().max().item() for i in range(n))
     assert err <= tol(shape, torch.float32) * 2.6
     plan.close()
+
+
+def test_c2c_host_entry_point(fft, oracle_mod):
+    from paper_2202_12756_b200 import inputs
+    shape, p = (32, 64, 256), 4
+    plan = fft.PlanC2C(*shape, dtype=torch.float64, virtual_slabs=p)
+    f = inputs.complex_grid(shape, torch.complex128, seed=31)
+    out = torch.empty(plan.n_complex, dtype=torch.complex128)
+    plan.c2c_host(f.reshape(-1).contiguous(), out, -1)
+    F_ref = oracle_mod.c2c(f.numpy(), -1)
+    assert rel_l2(plan.to_natural(out).numpy(), F_ref) <= tol(shape, torch.float64)
+    back = torch.empty_like(out)
+    plan.c2c_host(out, back, +1)
+    assert (back.reshape(shape) - f).abs().max().item() <= tol(shape, torch.float64) * 2
+    plan.close()
