@@ -8,7 +8,8 @@
 
 #define FFT3D_FOREACH_N(X) \
     X(4) X(8) X(16) X(32) X(64) X(128) X(256) X(512) X(1024) X(2048) X(4096) \
-    X(6) X(12) X(24) X(48) X(96) X(192) X(384) X(768) X(1536) X(3072)
+    X(6) X(12) X(24) X(48) X(96) X(192) X(384) X(768) X(1536) X(3072) \
+    X(20) X(40) X(80) X(160) X(320) X(640) X(1280)
 
 namespace fft3d {
 
@@ -40,6 +41,15 @@ FFT3D_CFG(float, 768, 24, 24, 8, 4)
 FFT3D_CFG(float, 1536, 24, 24, 8, 8)
 FFT3D_CFG(float, 3072, 24, 24, 8, 8, 2)
 
+// 5*2^a (radix-5 leaf in fft_radix.cuh)
+FFT3D_CFG(float, 20, 20, 20)
+FFT3D_CFG(float, 40, 20, 20, 2)
+FFT3D_CFG(float, 80, 20, 20, 4)
+FFT3D_CFG(float, 160, 20, 20, 4, 2)
+FFT3D_CFG(float, 320, 20, 20, 4, 4)
+FFT3D_CFG(float, 640, 20, 20, 4, 4, 2)
+FFT3D_CFG(float, 1280, 20, 20, 4, 4, 4)
+
 // fp64: registers are twice as wide, so fewer points per thread
 FFT3D_CFG(double, 4, 4, 4)
 FFT3D_CFG(double, 8, 8, 8)
@@ -62,6 +72,14 @@ FFT3D_CFG(double, 384, 12, 12, 4, 4, 2)
 FFT3D_CFG(double, 768, 12, 12, 4, 4, 4)
 FFT3D_CFG(double, 1536, 12, 12, 4, 4, 4, 2)
 FFT3D_CFG(double, 3072, 12, 12, 4, 4, 4, 4)
+
+FFT3D_CFG(double, 20, 20, 20)
+FFT3D_CFG(double, 40, 20, 20, 2)
+FFT3D_CFG(double, 80, 20, 20, 4)
+FFT3D_CFG(double, 160, 20, 20, 4, 2)
+FFT3D_CFG(double, 320, 20, 20, 4, 4)
+FFT3D_CFG(double, 640, 20, 20, 4, 4, 2)
+FFT3D_CFG(double, 1280, 20, 20, 4, 4, 4)
 
 // Factorisation used by the bulk-pipelined z kernels (fft_zpass.cuh): the strided-pass one unless
 // a shape with fewer exchanges fits a row's threads inside one warp.

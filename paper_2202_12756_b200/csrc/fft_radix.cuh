@@ -142,10 +142,27 @@ __device__ __forceinline__ void dft(cx<T> (&v)[R]) {
         v[2] = csub(t0, t2);
         v[1] = cadd(t1, id);
         v[3] = csub(t1, id);
+    } else if constexpr (R == 5) {
+        // X_k = x0 + sum_{j=1..4} x_j w^(jk), w = exp(DIR 2 pi i/5): with s1 = x1+x4, s2 = x2+x3, d1 = x1-x4, d2 = x2-x3,
+        // X_{1,4} = x0 + c1 s1 + c2 s2 +- DIR i (k1 d1 + k2 d2),  X_{2,3} = x0 + c2 s1 + c1 s2 +- DIR i (k2 d1 - k1 d2)
+        constexpr T c1 = (T)0.30901699437494742410229341718281906;    // cos(2 pi/5)
+        constexpr T c2 = (T)-0.80901699437494742410229341718281906;   // cos(4 pi/5)
+        constexpr T k1 = (T)0.95105651629515357211643933337938214;    // sin(2 pi/5)
+        constexpr T k2 = (T)0.58778525229247312916870595463907277;    // sin(4 pi/5)
+        const C s1 = cadd(v[1], v[4]), s2 = cadd(v[2], v[3]), d1 = csub(v[1], v[4]), d2 = csub(v[2], v[3]);
+        const C a1 = mk<T>(v[0].x + c1 * s1.x + c2 * s2.x, v[0].y + c1 * s1.y + c2 * s2.y);
+        const C a2 = mk<T>(v[0].x + c2 * s1.x + c1 * s2.x, v[0].y + c2 * s1.y + c1 * s2.y);
+        const C b1 = cmul_i<DIR>(mk<T>(k1 * d1.x + k2 * d2.x, k1 * d1.y + k2 * d2.y));
+        const C b2 = cmul_i<DIR>(mk<T>(k2 * d1.x - k1 * d2.x, k2 * d1.y - k1 * d2.y));
+        v[0] = mk<T>(v[0].x + s1.x + s2.x, v[0].y + s1.y + s2.y);
+        v[1] = cadd(a1, b1);
+        v[4] = csub(a1, b1);
+        v[2] = cadd(a2, b2);
+        v[3] = csub(a2, b2);
     } else {
-        constexpr int R1 = (R % 4 == 0) ? 4 : ((R % 2 == 0) ? 2 : 3);
+        constexpr int R1 = (R % 4 == 0) ? 4 : ((R % 2 == 0) ? 2 : ((R % 3 == 0) ? 3 : 5));
         constexpr int R2 = R / R1;
-        static_assert(R1 * R2 == R, "radix must be 2^a 3^b");
+        static_assert(R1 * R2 == R, "radix must be 2^a 3^b 5^c");
         C sub[R1][R2];
 #pragma unroll
         for (int q = 0; q < R1; ++q)

@@ -62,6 +62,10 @@ SMALL = [
     ((384, 192, 48), 12),       # 3*2^a lengths through the TMA path
     ((1536, 8, 32), 4),         # Nx = 1536: x passes as two 768-point half tiles with the shifted windows of odd rows
     ((1536, 32, 64), 16),
+    ((40, 80, 160), 4),         # 5*2^a lengths on every axis (radix-5 leaf; z half: 80)
+    ((20, 20, 40), 1),
+    ((320, 160, 80), 8),
+    ((80, 40, 1280), 4),        # 640-point rows through the bulk z kernel
     ((64, 192, 64), 32),        # L = 6: the two-class shifted windows (four classes need L % 4 == 0)
     ((2048, 8, 32), 2),         # Nx = 2048: inverse x pass as four 512-point quarter tiles + a radix-4 combine
     ((2048, 16, 64), 4),
@@ -201,7 +205,7 @@ def test_argument_errors(fft):
         fft.Plan(64, 64, 64, virtual_slabs=3)
     assert e.value.status == 1
     with pytest.raises(fft.Fft3dError) as e:
-        fft.Plan(40, 64, 64)
+        fft.Plan(56, 64, 64)                       # 56 = 7*8: no radix 7
     assert e.value.status == 2
     plan = fft.Plan(16, 16, 16, dtype=torch.float32)
     x = plan.empty_real()
