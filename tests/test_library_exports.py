@@ -51,7 +51,7 @@ def test_plan_validation_needs_no_gpu(lib):
     assert lib.fft3d_plan(ctypes.byref(h), 64, 64, 64, 0, 3) == 1        # p does not divide
     assert lib.fft3d_plan(ctypes.byref(h), 64, 64, 64, 5, 1) == 1        # bad dtype
     assert lib.fft3d_plan(ctypes.byref(h), 1, 64, 64, 0, 1) == 1         # extent < 2
-    assert lib.fft3d_plan(ctypes.byref(h), 40, 64, 64, 0, 1) == 2        # 40 = 5*8 unsupported
+    assert lib.fft3d_plan(ctypes.byref(h), 56, 64, 64, 0, 1) == 2        # 56 = 7*8 unsupported (no radix 7)
     assert lib.fft3d_plan(None, 64, 64, 64, 0, 1) == 1
 
 
