@@ -148,6 +148,14 @@ int fft3d_c2r_host(fft3d_plan_t *plan, const void *h_cplx_in, void *h_real_out);
 int fft3d_launches(const fft3d_plan_t *plan, int which);
 const char *fft3d_launch_name(const fft3d_plan_t *plan, int which, int i);
 
+/* Which implementation launch i runs with the plan's current variant (a static string; NULL if i is out of
+ * range): "fused_ring" (z+y passes of a plane in one persistent kernel, D:5.6), "bulk" (z rows streamed by 1-D
+ * bulk copies, D:5.3), "tma" (strided pass on whole tiles through a TMA ring, D:5.2), "tma_split2" /
+ * "tma_split4" (the same on half / quarter tiles plus a radix-2 / radix-4 combine), "plain" (plain loads and
+ * stores: any extent), "fixup" (the plane-sized Nyquist pack / unpack kernels, D:5.4).  Tests use it to make
+ * sure a shape really exercises the kernel it is meant to. */
+const char *fft3d_launch_impl(const fft3d_plan_t *plan, int which, int i);
+
 /* Per-kernel timing for roofline reports.  After fft3d_timing_enable(plan, max_calls) every
  * fft3d_r2c / fft3d_c2r call on this plan records CUDA events between its kernel launches on the
  * caller's stream (until max_calls calls per direction have been recorded; later calls run

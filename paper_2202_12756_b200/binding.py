@@ -20,6 +20,7 @@ EXPORTS = (
     "fft3d_complex_bytes", "fft3d_index", "fft3d_r2c", "fft3d_c2r", "fft3d_r2c_host",
     "fft3d_c2r_host", "fft3d_launches", "fft3d_launch_name", "fft3d_set_variant", "fft3d_destroy", "fft3d_strerror",
     "fft3d_timing_enable", "fft3d_timing_read", "fft3d_plan_c2c", "fft3d_c2c", "fft3d_c2c_host",
+    "fft3d_launch_impl",
 )
 
 _lib = None
@@ -67,6 +68,8 @@ def load_library() -> ctypes.CDLL:
     lib.fft3d_launches.restype = i
     lib.fft3d_launch_name.argtypes = [vp, i, i]
     lib.fft3d_launch_name.restype = ctypes.c_char_p
+    lib.fft3d_launch_impl.argtypes = [vp, i, i]
+    lib.fft3d_launch_impl.restype = ctypes.c_char_p
     lib.fft3d_set_variant.argtypes = [vp, i]
     lib.fft3d_set_variant.restype = i
     lib.fft3d_timing_enable.argtypes = [vp, i]
@@ -96,15 +99,17 @@ _CPLX = {F32: torch.complex64, F64: torch.complex128}
 class Plan:
     """fft3d_plan(Nx, Ny, Nz, dtype, virtual_slabs) with torch tensors as buffers."""
 
+    _PLAN_FN = "fft3d_plan"
+
     def __init__(self, Nx: int, Ny: int, Nz: int, dtype=torch.float32, virtual_slabs: int = 1):
         lib = load_library()
         self.dtype_code = {torch.float32: F32, torch.float64: F64}[dtype]
         self.shape = (int(Nx), int(Ny), int(Nz))
         self.p = int(virtual_slabs)
         h = ctypes.c_void_p()
-        rc = lib.fft3d_plan(ctypes.byref(h), Nx, Ny, Nz, self.dtype_code, self.p)
+        rc = getattr(lib, self._PLAN_FN)(ctypes.byref(h), Nx, Ny, Nz, self.dtype_code, self.p)
         if rc != 0:
-            raise Fft3dError(rc, "fft3d_plan(%d,%d,%d,p=%d)" % (Nx, Ny, Nz, self.p))
+            raise Fft3dError(rc, "%s(%d,%d,%d,p=%d)" % (self._PLAN_FN, Nx, Ny, Nz, self.p))
         self._h = h
         self._lib = lib
         self.real_dtype = _REAL[self.dtype_code]
@@ -112,7 +117,7 @@ class Plan:
         self.real_bytes = lib.fft3d_real_bytes(h)
         self.complex_bytes = lib.fft3d_complex_bytes(h)
         self.workspace_bytes = lib.fft3d_workspace_bytes(h)
-        self.n_complex = Nx * Ny * (Nz // 2 + 1)
+        self.n_complex = self.complex_bytes // (2 * (4 if self.dtype_code == F32 else 8))
 
     # ---- buffers -------------------------------------------------------------------------
     def empty_real(self, device="cuda"):
@@ -139,6 +144,10 @@ class Plan:
     def launch_names(self, which: int):
         return tuple(self._lib.fft3d_launch_name(self._h, which, k).decode() for k in range(self.launches(which)))
 
+    def launch_impls(self, which: int):
+        """Implementation of each launch ("tma", "fused_ring", "plain", ...), aligned with launch_names."""
+        return tuple(self._lib.fft3d_launch_impl(self._h, which, k).decode() for k in range(self.launches(which)))
+
     def timing_enable(self, max_calls: int):
         rc = self._lib.fft3d_timing_enable(self._h, int(max_calls))
         if rc != 0:
@@ -160,14 +169,37 @@ class Plan:
         if not (t.is_cuda and t.is_contiguous() and t.dtype == dtype and t.numel() * t.element_size() == nbytes):
             raise ValueError("%s must be a contiguous CUDA tensor of dtype %s and %d bytes" % (name, dtype, nbytes))
 
+    def _check_work(self, work: torch.Tensor, ref: torch.Tensor):
+        # the C side cannot see the size of a bare pointer: an undersized workspace would be an out-of-bounds write
+        if not (work.is_cuda and work.is_contiguous() and work.device == ref.device and
+                work.numel() * work.element_size() >= self.workspace_bytes):
+            raise ValueError("work must be a contiguous CUDA tensor on %s of at least %d bytes"
+                             % (ref.device, self.workspace_bytes))
+
+    def _check_host(self, t: torch.Tensor, dtype, nbytes: int, name: str):
+        if t.is_cuda or not t.is_contiguous() or t.dtype != dtype or t.numel() * t.element_size() != nbytes:
+            raise ValueError("%s must be a contiguous host tensor of dtype %s and %d bytes" % (name, dtype, nbytes))
+
+    def _stream(self, stream, ref: torch.Tensor, temporaries):
+        """The stream to launch on; buffers allocated inside the call are tied to it so that the caching
+        allocator does not hand them out again while the kernels are still queued."""
+        s = stream if stream is not None else torch.cuda.current_stream(ref.device)
+        for t in temporaries:
+            t.record_stream(s)
+        return s
+
     def r2c(self, real_in, cplx_out=None, work=None, stream=None):
         self._check(real_in, self.real_dtype, self.real_bytes, "real_in")
+        tmp = []
         if cplx_out is None:
             cplx_out = self.empty_complex(real_in.device)
+            tmp.append(cplx_out)
         if work is None:
             work = self.empty_workspace(real_in.device)
+            tmp.append(work)
         self._check(cplx_out, self.complex_dtype, self.complex_bytes, "cplx_out")
-        s = stream if stream is not None else torch.cuda.current_stream(real_in.device)
+        self._check_work(work, real_in)
+        s = self._stream(stream, real_in, tmp)
         rc = self._lib.fft3d_r2c(self._h, real_in.data_ptr(), cplx_out.data_ptr(), work.data_ptr(),
                                  ctypes.c_void_p(s.cuda_stream))
         if rc != 0:
@@ -176,12 +208,16 @@ class Plan:
 
     def c2r(self, cplx_in, real_out=None, work=None, stream=None):
         self._check(cplx_in, self.complex_dtype, self.complex_bytes, "cplx_in")
+        tmp = []
         if real_out is None:
             real_out = self.empty_real(cplx_in.device)
+            tmp.append(real_out)
         if work is None:
             work = self.empty_workspace(cplx_in.device)
+            tmp.append(work)
         self._check(real_out, self.real_dtype, self.real_bytes, "real_out")
-        s = stream if stream is not None else torch.cuda.current_stream(cplx_in.device)
+        self._check_work(work, cplx_in)
+        s = self._stream(stream, cplx_in, tmp)
         rc = self._lib.fft3d_c2r(self._h, cplx_in.data_ptr(), real_out.data_ptr(), work.data_ptr(),
                                  ctypes.c_void_p(s.cuda_stream))
         if rc != 0:
@@ -190,14 +226,16 @@ class Plan:
 
     # ---- host entry points (host tensors, copies inside the call) --------------------------
     def r2c_host(self, real_in: torch.Tensor, cplx_out: torch.Tensor):
-        assert not real_in.is_cuda and not cplx_out.is_cuda and real_in.is_contiguous() and cplx_out.is_contiguous()
+        self._check_host(real_in, self.real_dtype, self.real_bytes, "real_in")
+        self._check_host(cplx_out, self.complex_dtype, self.complex_bytes, "cplx_out")
         rc = self._lib.fft3d_r2c_host(self._h, real_in.data_ptr(), cplx_out.data_ptr())
         if rc != 0:
             raise Fft3dError(rc, "fft3d_r2c_host")
         return cplx_out
 
     def c2r_host(self, cplx_in: torch.Tensor, real_out: torch.Tensor):
-        assert not cplx_in.is_cuda and not real_out.is_cuda and cplx_in.is_contiguous() and real_out.is_contiguous()
+        self._check_host(cplx_in, self.complex_dtype, self.complex_bytes, "cplx_in")
+        self._check_host(real_out, self.real_dtype, self.real_bytes, "real_out")
         rc = self._lib.fft3d_c2r_host(self._h, cplx_in.data_ptr(), real_out.data_ptr())
         if rc != 0:
             raise Fft3dError(rc, "fft3d_c2r_host")
@@ -231,32 +269,20 @@ class PlanC2C(Plan):
     """fft3d_plan_c2c(Nx, Ny, Nz, dtype, virtual_slabs): 3D complex-to-complex transform (argument marshalling
     only).  Forward output / inverse input are flat complex buffers in the slab layout [p][Nx][Ny/p][Nz]."""
 
-    def __init__(self, Nx: int, Ny: int, Nz: int, dtype=torch.float32, virtual_slabs: int = 1):
-        lib = load_library()
-        self.dtype_code = {torch.float32: F32, torch.float64: F64}[dtype]
-        self.shape = (int(Nx), int(Ny), int(Nz))
-        self.p = int(virtual_slabs)
-        h = ctypes.c_void_p()
-        rc = lib.fft3d_plan_c2c(ctypes.byref(h), Nx, Ny, Nz, self.dtype_code, self.p)
-        if rc != 0:
-            raise Fft3dError(rc, "fft3d_plan_c2c(%d,%d,%d,p=%d)" % (Nx, Ny, Nz, self.p))
-        self._h = h
-        self._lib = lib
-        self.real_dtype = _REAL[self.dtype_code]
-        self.complex_dtype = _CPLX[self.dtype_code]
-        self.real_bytes = lib.fft3d_real_bytes(h)
-        self.complex_bytes = lib.fft3d_complex_bytes(h)
-        self.workspace_bytes = lib.fft3d_workspace_bytes(h)
-        self.n_complex = Nx * Ny * Nz
+    _PLAN_FN = "fft3d_plan_c2c"
 
     def c2c(self, cplx_in, direction: int, cplx_out=None, work=None, stream=None):
         self._check(cplx_in, self.complex_dtype, self.complex_bytes, "cplx_in")
+        tmp = []
         if cplx_out is None:
             cplx_out = self.empty_complex(cplx_in.device)
+            tmp.append(cplx_out)
         if work is None:
             work = self.empty_workspace(cplx_in.device)
+            tmp.append(work)
         self._check(cplx_out, self.complex_dtype, self.complex_bytes, "cplx_out")
-        s = stream if stream is not None else torch.cuda.current_stream(cplx_in.device)
+        self._check_work(work, cplx_in)
+        s = self._stream(stream, cplx_in, tmp)
         rc = self._lib.fft3d_c2c(self._h, cplx_in.data_ptr(), cplx_out.data_ptr(), work.data_ptr(), int(direction),
                                  ctypes.c_void_p(s.cuda_stream))
         if rc != 0:
@@ -264,7 +290,8 @@ class PlanC2C(Plan):
         return cplx_out
 
     def c2c_host(self, cplx_in: torch.Tensor, cplx_out: torch.Tensor, direction: int):
-        assert not cplx_in.is_cuda and not cplx_out.is_cuda and cplx_in.is_contiguous() and cplx_out.is_contiguous()
+        self._check_host(cplx_in, self.complex_dtype, self.complex_bytes, "cplx_in")
+        self._check_host(cplx_out, self.complex_dtype, self.complex_bytes, "cplx_out")
         rc = self._lib.fft3d_c2c_host(self._h, cplx_in.data_ptr(), cplx_out.data_ptr(), int(direction))
         if rc != 0:
             raise Fft3dError(rc, "fft3d_c2c_host")

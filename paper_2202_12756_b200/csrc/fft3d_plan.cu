@@ -657,6 +657,24 @@ static bool use_fused(const fft3d_plan_t* pl) {
 }
 static bool use_tma(const fft3d_plan_t* pl) { return pl->variant != 1; }
 
+// Which implementation each pass of an R2C/C2R plan runs with the current variant (one place: the launch
+// code below and fft3d_launch_impl both ask these).
+enum PassImpl { IMPL_PLAIN = 0, IMPL_TMA, IMPL_TMA_SPLIT2, IMPL_TMA_SPLIT4, IMPL_BULK, IMPL_FUSED, IMPL_FIXUP };
+static PassImpl z_impl(const fft3d_plan_t* pl) { return use_tma(pl) && pl->bulk_z ? IMPL_BULK : IMPL_PLAIN; }
+static PassImpl y_impl(const fft3d_plan_t* pl) {
+    if (use_tma(pl) && pl->split_y && pl->variant != 2) return IMPL_TMA_SPLIT2;
+    return use_tma(pl) && pl->tma_y ? IMPL_TMA : IMPL_PLAIN;
+}
+static PassImpl x_impl(const fft3d_plan_t* pl, int d) {
+    if (pl->kind == 1) return use_tma(pl) && pl->tma_xc ? IMPL_TMA : IMPL_PLAIN;
+    if (!(use_tma(pl) && pl->tma_x)) return IMPL_PLAIN;
+    // (the quarter-tile kernel is used for the inverse only: measured at 2048^3, F3 25.1 ms against 23.4 ms whole
+    // tiles -- its thin tiles cost four loads each -- but I1 20.0 against 22.8)
+    if (d == 1 && pl->split4_x && pl->variant != 2) return IMPL_TMA_SPLIT4;
+    if (pl->split_x && pl->variant != 2) return IMPL_TMA_SPLIT2;
+    return IMPL_TMA;
+}
+
 int fft3d_launches(const fft3d_plan_t* pl, int which) {
     if (pl == nullptr || which < 0 || which > 1) return 0;
     if (pl->kind == 1) return use_fused(pl) ? 2 : 3;
@@ -692,6 +710,19 @@ const char* fft3d_launch_name(const fft3d_plan_t* pl, int which, int i) {
     return seq[i];
 }
 
+const char* fft3d_launch_impl(const fft3d_plan_t* pl, int which, int i) {
+    const char* nm = fft3d_launch_name(pl, which, i);
+    if (nm == nullptr) return nullptr;
+    static const char* const names[] = {"plain", "tma", "tma_split2", "tma_split4", "bulk", "fused_ring", "fixup"};
+    PassImpl im = IMPL_FIXUP;
+    if (std::strstr(nm, "fused") != nullptr) im = IMPL_FUSED;
+    else if (std::strcmp(nm, "x_c2c_inv_col0") == 0) im = IMPL_PLAIN;
+    else if (nm[0] == 'z') im = pl->kind == 1 ? IMPL_BULK : z_impl(pl);
+    else if (nm[0] == 'y') im = y_impl(pl);
+    else if (nm[0] == 'x') im = x_impl(pl, which);
+    return names[im];
+}
+
 int fft3d_set_variant(fft3d_plan_t* pl, int variant) {
     // 0 = the fastest known path (fused z+y passes where they win, TMA-pipelined passes elsewhere),
     // 1 = plain-load kernels only, 2 = unfused TMA-pipelined passes (six array passes per pair),
@@ -713,7 +744,7 @@ int fft3d_r2c(const fft3d_plan_t* pl, const void* d_in, void* d_out, void* d_wor
     Recorder rec(pl, 0, st);
     int slot = 0;
     rec.mark(slot++);
-    const bool tma_on = use_tma(pl), fz = use_fused(pl);
+    const bool fz = use_fused(pl);
     int rc;
     if (fz) {
         // F1+F2 fused: real -> (ring in L2) -> slab array in the workspace
@@ -725,7 +756,7 @@ int fft3d_r2c(const fft3d_plan_t* pl, const void* d_in, void* d_out, void* d_wor
     ZArgs z{};
     z.in = d_in; z.out = d_out; z.tw = pl->tw_z; z.twz = pl->twz; z.nrows = Nx * Ny; z.scale = 1.0;
     const KernelSet* kz = pl->kz;
-    if (tma_on && pl->bulk_z) rc = launch_zbulk(pl, 0, d_in, d_out, 1.0, st);
+    if (z_impl(pl) == IMPL_BULK) rc = launch_zbulk(pl, 0, d_in, d_out, 1.0, st);
     else rc = launch(kz->z_fn[0], (z.nrows + kz->z_rpb - 1) / kz->z_rpb, pl->grid_z[0], kz->z_threads, kz->z_smem, &z, st);
     if (rc != FFT3D_OK) return rc;
     rec.mark(slot++);
@@ -738,9 +769,9 @@ int fft3d_r2c(const fft3d_plan_t* pl, const void* d_in, void* d_out, void* d_wor
     a.ntiles = Nx * a.ntz;
     a.in_hi = Ny * M; a.in_lo = 0; a.in_rq = 0; a.in_rl = M;
     a.out_hi = L * M; a.out_lo = 0; a.out_rq = Nx * L * M; a.out_rl = M;
-    if (tma_on && pl->split_y && pl->variant != 2) {
+    if (y_impl(pl) == IMPL_TMA_SPLIT2) {
         rc = launch_y_split2(pl, 0, d_out, d_work, st);
-    } else if (tma_on && pl->tma_y) {
+    } else if (y_impl(pl) == IMPL_TMA) {
         TensorMapBlob mi, mo;
         if (!map_natural(pl, &mi, d_out, ky->tma_tc, pl->y_rows_nat) ||
             !map_slab_y(pl, &mo, d_work, ky->tma_tc, pl->y_rows_slab)) return FFT3D_ECUDA;
@@ -763,11 +794,9 @@ int fft3d_r2c(const fft3d_plan_t* pl, const void* d_in, void* d_out, void* d_wor
     b.ntiles = (long long)p * L * b.ntz;
     b.in_hi = Nx * L * M; b.in_lo = M; b.in_rq = 0; b.in_rl = L * M;
     b.out_hi = Nx * L * (M + 1); b.out_lo = M + 1; b.out_rq = 0; b.out_rl = L * (M + 1);
-    // (the quarter-tile kernel is used for the inverse only: measured at 2048^3, F3 25.1 ms against 23.4 ms whole
-    // tiles -- its thin tiles cost four loads each -- but I1 20.0 against 22.8)
-    if (tma_on && pl->split_x && pl->variant != 2) {
+    if (x_impl(pl, 0) == IMPL_TMA_SPLIT2) {
         rc = launch_x_split2(pl, 0, d_work, d_out, st);
-    } else if (tma_on && pl->tma_x) {
+    } else if (x_impl(pl, 0) == IMPL_TMA) {
         TensorMapBlob mi, mo;
         TensorMapBlob mi2;
         const int tc = kx->tma_tc_x, of = kx->tma_oddfix;
@@ -809,7 +838,7 @@ int fft3d_c2r(const fft3d_plan_t* pl, const void* d_in, void* d_out, void* d_wor
     Recorder rec(pl, 1, st);
     int slot = 0;
     rec.mark(slot++);
-    const bool tma_on = use_tma(pl), fz = use_fused(pl);
+    const bool fz = use_fused(pl);
     // fused: I1 writes the slab array in the workspace and I2+I3 go from there to d_out, so the side
     // buffer sits behind the ring; unfused: I1 -> d_out (scratch) -> I2 -> workspace -> I3 -> d_out
     void* side = fz ? (void*)(reinterpret_cast<unsigned char*>(d_work) + pl->slab_bytes + pl->ring_bytes) : d_work;
@@ -829,7 +858,7 @@ int fft3d_c2r(const fft3d_plan_t* pl, const void* d_in, void* d_out, void* d_wor
     b.c0_hi = Nx * L; b.c0_lo = 1; b.c0_rl = L;
     b.out_hi = Nx * L * M; b.out_lo = M; b.out_rq = 0; b.out_rl = L * M;
     int rc;
-    if (tma_on && pl->tma_x) {
+    if (x_impl(pl, 1) != IMPL_PLAIN) {
         TensorMapBlob mi, mo;
         TensorMapBlob mi2;
         const int tc = kx->tma_tc_x, of = kx->tma_oddfix;
@@ -839,8 +868,8 @@ int fft3d_c2r(const fft3d_plan_t* pl, const void* d_in, void* d_out, void* d_wor
         ta.tw = pl->tw_x; ta.ntz = (int)(M / tc);
         ta.ntiles = of ? (long long)p * (L / 2) * (2 * ta.ntz) : (long long)p * L * ta.ntz;
         ta.L = (int)L; ta.Nx = (int)Nx; ta.Mp1 = (int)(M + 1); ta.in_rows = pl->x_rows; ta.out_rows = pl->x_rows;
-        if (pl->split4_x && pl->variant != 2) rc = launch_x_split4(pl, 1, d_in, x_out, st);
-        else if (pl->split_x && pl->variant != 2) rc = launch_x_split2(pl, 1, d_in, x_out, st);
+        if (x_impl(pl, 1) == IMPL_TMA_SPLIT4) rc = launch_x_split4(pl, 1, d_in, x_out, st);
+        else if (x_impl(pl, 1) == IMPL_TMA_SPLIT2) rc = launch_x_split2(pl, 1, d_in, x_out, st);
         else rc = launch_tma(kx->tma_fn[TMA_X_INV], kx->tma_threads_x, kx->tma_smem_x, pl->num_sms, mi, mi2, mo, ta, st);
         rec.mark(slot++);
         // packed column 0 of the result: x-transform of the side buffer, written over the (meaningless)
@@ -875,9 +904,9 @@ int fft3d_c2r(const fft3d_plan_t* pl, const void* d_in, void* d_out, void* d_wor
     a.ntiles = Nx * a.ntz;
     a.in_hi = L * M; a.in_lo = 0; a.in_rq = Nx * L * M; a.in_rl = M;
     a.out_hi = Ny * M; a.out_lo = 0; a.out_rq = 0; a.out_rl = M;
-    if (tma_on && pl->split_y && pl->variant != 2) {
+    if (y_impl(pl) == IMPL_TMA_SPLIT2) {
         rc = launch_y_split2(pl, 1, d_out, d_work, st);
-    } else if (tma_on && pl->tma_y) {
+    } else if (y_impl(pl) == IMPL_TMA) {
         TensorMapBlob mi, mo;
         if (!map_slab_y(pl, &mi, d_out, ky->tma_tc, pl->y_rows_slab) ||
             !map_natural(pl, &mo, d_work, ky->tma_tc, pl->y_rows_nat)) return FFT3D_ECUDA;
@@ -896,7 +925,7 @@ int fft3d_c2r(const fft3d_plan_t* pl, const void* d_in, void* d_out, void* d_wor
     ZArgs z{};
     z.in = d_work; z.out = d_out; z.tw = pl->tw_z; z.twz = pl->twz; z.nrows = Nx * Ny;
     z.scale = 1.0 / ((double)Nx * (double)Ny * (double)Nz);
-    if (tma_on && pl->bulk_z) rc = launch_zbulk(pl, 1, d_work, d_out, z.scale, st);
+    if (z_impl(pl) == IMPL_BULK) rc = launch_zbulk(pl, 1, d_work, d_out, z.scale, st);
     else rc = launch(kz->z_fn[1], (z.nrows + kz->z_rpb - 1) / kz->z_rpb, pl->grid_z[1], kz->z_threads, kz->z_smem, &z, st);
     rec.mark(slot++);
     return rc;
@@ -916,7 +945,6 @@ int fft3d_c2c(const fft3d_plan_t* pl, const void* d_in, void* d_out, void* d_wor
     const long long Nx = pl->Nx, Ny = pl->Ny, M = pl->M, L = pl->L, p = pl->p;
     const KernelSet *kz = pl->kz, *ky = pl->ky, *kx = pl->kx;
     const int d = direction < 0 ? 0 : 1;
-    const bool tma_on = use_tma(pl);
     Recorder rec(pl, d, st);
     int slot = 0, rc = FFT3D_OK;
     rec.mark(slot++);
@@ -933,8 +961,8 @@ int fft3d_c2c(const fft3d_plan_t* pl, const void* d_in, void* d_out, void* d_wor
         return FFT3D_OK;
     };
     auto y_pass = [&](const void* in, void* out) -> int {       // forward: natural -> slab; inverse: slab -> natural
-        if (tma_on && pl->split_y && pl->variant != 2) return launch_y_split2(pl, d, in, out, st);
-        if (tma_on && pl->tma_y) {
+        if (y_impl(pl) == IMPL_TMA_SPLIT2) return launch_y_split2(pl, d, in, out, st);
+        if (y_impl(pl) == IMPL_TMA) {
             TensorMapBlob mi, mo;
             bool ok = d == 0 ? (map_natural(pl, &mi, in, ky->tma_tc, pl->y_rows_nat) && map_slab_y(pl, &mo, out, ky->tma_tc, pl->y_rows_slab))
                              : (map_slab_y(pl, &mi, in, ky->tma_tc, pl->y_rows_slab) && map_natural(pl, &mo, out, ky->tma_tc, pl->y_rows_nat));
@@ -959,7 +987,7 @@ int fft3d_c2c(const fft3d_plan_t* pl, const void* d_in, void* d_out, void* d_wor
         return launch(ky->s_fn[1][KIND_SLAB_LIN], a.ntiles, pl->grid_y[1], ky->s_threads, ky->s_smem, &a, st);
     };
     auto x_pass = [&](const void* in, void* out) -> int {       // lines along x inside every virtual slab, pitch M
-        if (tma_on && pl->tma_xc) {
+        if (x_impl(pl, d) == IMPL_TMA) {
             // X_FWD reads the 4-D slab view and writes the flattened one, X_INV the other way round; with one
             // pitch M on both sides the two views describe the same layout
             TensorMapBlob mi, mo;

@@ -109,11 +109,17 @@ __device__ __forceinline__ void write_own(const cx<T> (&v)[Cfg::P], cx<T>* __res
     }
 }
 
-// One stage (and, recursively, the following ones).
-template <class Cfg, int SI, int DIR, typename T, class Lay, class Sync>
+struct NoHook {
+    __device__ __forceinline__ void operator()() const {}
+};
+
+// One stage (and, recursively, the following ones).  `before_scatter` runs once, after the first butterfly of
+// stage 0 has been computed in registers and before anything is written to `sm` (transforms with more than one
+// stage only): kernels whose exchange buffer may still be busy wait for it there, behind the arithmetic.
+template <class Cfg, int SI, int DIR, typename T, class Lay, class Sync, class Hook = NoHook>
 __device__ __forceinline__ void fft_stages(cx<T> (&v)[Cfg::P], cx<T>* __restrict__ sm,
                                            const cx<T>* __restrict__ tw, int t, const Lay& lay,
-                                           const Sync& sync) {
+                                           const Sync& sync, const Hook& before_scatter = Hook{}) {
     using C = cx<T>;
     constexpr int r = Cfg::radix(SI), Ns = Cfg::ns(SI), P = Cfg::P, S = Cfg::S, B = P / r;
     constexpr bool last = (SI == Cfg::NST - 1);
@@ -150,6 +156,9 @@ __device__ __forceinline__ void fft_stages(cx<T> (&v)[Cfg::P], cx<T>* __restrict
             }
         }
         dft<r, DIR, T>(a);
+        if constexpr (SI == 0 && !last) {
+            if (u == 0) before_scatter();
+        }
         if constexpr (last) {
 #pragma unroll
             for (int i = 0; i < r; ++i) v[u + i * B] = a[i];

@@ -39,6 +39,9 @@ CASES = [
     ((256, 256, 256), 8),       # BASELINE.json configs[1] shape
     ((96, 384, 384), 12),       # 3*2^a lengths (radix 3) through the fused kernels
     ((16, 512, 512), 2),        # Nx barely above the ring depth
+    # the 512/1024 instantiation bench.py times at 1024^3 (default there), ring of 8 planes, on a thin slab
+    ((16, 1024, 1024), 8),
+    ((24, 1024, 1024), 1),
 ]
 
 
@@ -53,6 +56,7 @@ def test_fused_matches_oracle(fft, oracle_mod, shape, p, dtype):
         pytest.skip("fused kernels are not compiled for %s %s" % (shape, dtype))
     assert "yz_c2r_fused" in plan.launch_names(1)
     assert "z_r2c" not in plan.launch_names(0) and "z_c2r" not in plan.launch_names(1)
+    assert plan.launch_impls(0)[0] == "fused_ring" and plan.launch_impls(1)[-1] == "fused_ring"
     d_in = f.cuda()
     keep = d_in.clone()
     work = plan.empty_workspace("cuda")

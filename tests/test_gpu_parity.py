@@ -74,6 +74,60 @@ SMALL = [
 ]
 
 
+# Thin slabs that run the very FFT-1024 kernel instantiations bench.py times at 1024^3 (full oracle, < 1 s each):
+# shape, p, variant, {launch name: implementation that must be selected}
+BENCH_KERNELS = [
+    # F3 with four row classes l % 4 and every thin tile (columns M-2, M-1 / M-1 / 0), I1 + the col0 launch
+    ((1024, 16, 32), 4, 0, {"x_c2c_fwd": "tma", "x_c2c_inv": "tma", "x_c2c_inv_col0": "plain"}),
+    ((1024, 32, 64), 2, 0, {"x_c2c_fwd": "tma", "x_c2c_inv": "tma"}),
+    ((1024, 8, 32), 4, 0, {"x_c2c_fwd": "tma", "x_c2c_inv": "tma"}),       # L = 2: the two-class windows
+    # FFT-1024 Y passes: slab boxes inside one slab (L = 1024) and spanning several (L = 64)
+    ((16, 1024, 32), 1, 0, {"y_c2c_fwd": "tma", "y_c2c_inv": "tma"}),
+    ((16, 1024, 32), 16, 0, {"y_c2c_fwd": "tma", "y_c2c_inv": "tma"}),
+    # 512-point rows through the bulk z kernel next to 1024-point y lines, unfused
+    ((8, 1024, 1024), 8, 2, {"z_r2c": "bulk", "y_c2c_fwd": "tma", "z_c2r": "bulk", "y_c2c_inv": "tma"}),
+    # 1536 / 2048 on x and y at bench-like row lengths
+    # (fp32 implementation, fp64 implementation) where they differ: fp64 whole tiles still leave room for a ring
+    ((1536, 16, 32), 4, 0, {"x_c2c_fwd": ("tma_split2", "tma"), "x_c2c_inv": ("tma_split2", "tma")}),
+    ((2048, 16, 32), 4, 0, {"x_c2c_inv": ("tma_split4", "tma")}),
+    ((8, 2048, 32), 8, 0, {"y_c2c_fwd": "tma_split2", "y_c2c_inv": "tma_split2"}),
+    ((16, 1536, 32), 16, 0, {"y_c2c_fwd": "tma", "y_c2c_inv": "tma"}),
+]
+
+
+@pytest.mark.parametrize("shape,p,variant,impls", BENCH_KERNELS)
+@pytest.mark.parametrize("dtype", [torch.float32, torch.float64])
+def test_bench_kernel_instantiations_match_full_oracle(fft, oracle_mod, shape, p, variant, impls, dtype):
+    """Element-wise parity, against the FULL oracle, of the kernels that make up bench.py's step; the plan must
+    select the implementation named (fft3d_launch_impl), so a silent fallback fails the test."""
+    from paper_2202_12756_b200 import inputs
+    f = inputs.uniform_grid(shape, dtype, seed=11)
+    plan = fft.Plan(*shape, dtype=dtype, virtual_slabs=p)
+    plan.set_variant(variant)
+    got = dict(zip(plan.launch_names(0) + plan.launch_names(1), plan.launch_impls(0) + plan.launch_impls(1)))
+    for name, impl in impls.items():
+        if isinstance(impl, tuple):
+            impl = impl[0] if dtype == torch.float32 else impl[1]
+        assert got.get(name) == impl, (name, impl, got)
+    d_in = f.cuda()
+    d_out = plan.r2c(d_in)
+    F_gpu = plan.to_natural(d_out).cpu().numpy().astype(np.complex128)
+    F_ref = oracle_mod.r2c(f.double().numpy())
+    assert rel_l2(F_gpu, F_ref) <= tol(shape, dtype)
+    # worst single entry, relative to the rms of the spectrum (white-noise input: every entry is O(rms))
+    rms = np.sqrt(np.mean(np.abs(F_ref) ** 2))
+    assert np.abs(F_gpu - F_ref).max() <= 8 * tol(shape, dtype) * rms
+    S = inputs.random_spectrum(shape, plan.complex_dtype, seed=12)
+    f_ref = oracle_mod.c2r(S.to(torch.complex128).numpy(), shape[2])
+    f_gpu = plan.c2r(plan.from_natural(S.cuda())).cpu().double().numpy()
+    assert rel_l2(f_gpu, f_ref) <= tol(shape, dtype)
+    assert np.abs(f_gpu - f_ref).max() <= 8 * tol(shape, dtype) * np.sqrt(np.mean(f_ref ** 2))
+    back = plan.c2r(d_out)
+    err = (back.cpu().double() - f.double()).abs().max().item() / f.double().abs().max().item()
+    assert err <= tol(shape, dtype)
+    plan.close()
+
+
 @pytest.mark.parametrize("shape,p", SMALL)
 @pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
 @pytest.mark.parametrize("variant", [0, 1])     # 0: TMA-pipelined strided passes where possible, 1: plain-load kernels
