@@ -181,6 +181,15 @@ int fft3d_timing_read(fft3d_plan_t *plan, int which, float *ms_sum, int *calls);
  * this plan.  The workspace size does not depend on the variant. */
 int fft3d_set_variant(fft3d_plan_t *plan, int variant);
 
+/* Tunables of the fused z+y pipeline (D:5.6); the defaults are the measured best on B200.  Like
+ * fft3d_set_variant these change the plan: call them while no transform on this plan is being enqueued.
+ * Results do not depend on them (bit-identical).  Returns FFT3D_EINVAL for an unknown option or a value out
+ * of range.
+ *   FUSED_Z_SMS_FWD / _INV   SMs [0, value) run the z tiles, the others the y tiles (even; 0 = alternate CTA pairs)
+ *   FUSED_RING_PLANES        yz-planes in the L2 ring (2 .. the number the workspace was sized for) */
+enum { FFT3D_OPT_FUSED_Z_SMS_FWD = 1, FFT3D_OPT_FUSED_Z_SMS_INV = 2, FFT3D_OPT_FUSED_RING_PLANES = 3 };
+int fft3d_set_option(fft3d_plan_t *plan, int option, long long value);
+
 int fft3d_destroy(fft3d_plan_t *plan);          /* NULL is accepted */
 
 const char *fft3d_strerror(int status);         /* static string, never NULL */

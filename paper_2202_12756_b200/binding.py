@@ -12,6 +12,7 @@ import os
 import torch
 
 F32, F64 = 0, 1
+OPT_FUSED_Z_SMS_FWD, OPT_FUSED_Z_SMS_INV, OPT_FUSED_RING_PLANES = 1, 2, 3
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libfft3d.so")
 
@@ -20,7 +21,7 @@ EXPORTS = (
     "fft3d_complex_bytes", "fft3d_index", "fft3d_r2c", "fft3d_c2r", "fft3d_r2c_host",
     "fft3d_c2r_host", "fft3d_launches", "fft3d_launch_name", "fft3d_set_variant", "fft3d_destroy", "fft3d_strerror",
     "fft3d_timing_enable", "fft3d_timing_read", "fft3d_plan_c2c", "fft3d_c2c", "fft3d_c2c_host",
-    "fft3d_launch_impl",
+    "fft3d_launch_impl", "fft3d_set_option",
 )
 
 _lib = None
@@ -72,6 +73,8 @@ def load_library() -> ctypes.CDLL:
     lib.fft3d_launch_impl.restype = ctypes.c_char_p
     lib.fft3d_set_variant.argtypes = [vp, i]
     lib.fft3d_set_variant.restype = i
+    lib.fft3d_set_option.argtypes = [vp, i, ll]
+    lib.fft3d_set_option.restype = i
     lib.fft3d_timing_enable.argtypes = [vp, i]
     lib.fft3d_timing_enable.restype = i
     lib.fft3d_timing_read.argtypes = [vp, i, ctypes.POINTER(ctypes.c_float), ctypes.POINTER(i)]
@@ -140,6 +143,11 @@ class Plan:
         rc = self._lib.fft3d_set_variant(self._h, int(v))
         if rc != 0:
             raise Fft3dError(rc, "fft3d_set_variant")
+
+    def set_option(self, option: int, value: int):
+        rc = self._lib.fft3d_set_option(self._h, int(option), int(value))
+        if rc != 0:
+            raise Fft3dError(rc, "fft3d_set_option(%d, %d)" % (option, value))
 
     def launch_names(self, which: int):
         return tuple(self._lib.fft3d_launch_name(self._h, which, k).decode() for k in range(self.launches(which)))

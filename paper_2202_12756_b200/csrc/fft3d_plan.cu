@@ -94,6 +94,7 @@ struct fft3d_plan_s {
     bool fused_default;        // ... and expected to win (variant 0 uses them)
     int fz_R;                  // ring depth (planes)
     int fz_kz[2];              // [fwd, inv] SMs [0, kz) run the z tiles, the others the y tiles (0: split by CTA pairs)
+    int fz_R_max;              // ring planes the workspace was sized for
     size_t slab_bytes, ring_bytes, side_bytes, flags_bytes;
 };
 
@@ -288,9 +289,6 @@ int launch_fused(const fft3d_plan_s* pl, int d, const void* in, void* out, void*
     a.Nx = (int)pl->Nx; a.Ny = (int)pl->Ny; a.L = (int)pl->L; a.R = pl->fz_R; a.kz = pl->fz_kz[d];
     a.rows_slab = pl->y_rows_slab;
     a.scale = 1.0 / ((double)pl->Nx * (double)pl->Ny * (double)pl->Nz);
-#ifdef FFT3D_TUNING
-    if (const char* e = getenv("FFT3D_FZ_KZ")) a.kz = atoi(e);
-#endif
     void* argv[3] = {(void*)&ring_map, (void*)&slab_map, (void*)&a};
     cudaError_t e = cudaLaunchCooperativeKernel(fn, dim3((unsigned)pl->num_sms), dim3((unsigned)f_threads), argv, f_smem, st);
     if (e != cudaSuccess) { cudaGetLastError(); return FFT3D_ECUDA; }
@@ -299,9 +297,6 @@ int launch_fused(const fft3d_plan_s* pl, int d, const void* in, void* out, void*
 
 // fp32 X_FWD: four row classes l % 4 put every user-side window on a 32-byte sector (fft_kernels.cuh, XTile)
 bool x_fwd_cls4(const fft3d_plan_s* pl) {
-#ifdef FFT3D_TUNING
-    if (const char* e = getenv("FFT3D_CLS4")) return atoi(e) != 0 && pl->esize == 4 && pl->L % 4 == 0 && pl->M % 4 == 0;
-#endif
     return pl->esize == 4 && pl->L % 4 == 0 && pl->M % 4 == 0;
 }
 
@@ -572,9 +567,6 @@ static int plan_create(fft3d_plan_t** out, long long Nx, long long Ny, long long
         const size_t plane = (size_t)Ny * pl->M * 2 * pl->esize;
         int R = (int)(((size_t)48 << 20) / plane);
         if (R > 8) R = 8;
-#ifdef FFT3D_TUNING
-        if (const char* e = getenv("FFT3D_FZ_R")) R = atoi(e);
-#endif
         int coop = 0;
         cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
         if (R >= 2 && Nx >= R && coop) {
@@ -583,8 +575,9 @@ static int plan_create(fft3d_plan_t** out, long long Nx, long long Ny, long long
                 int g = 0;
                 ok = prepare_kernel(ky->fz_fn[d], ky->fz_threads, ky->fz_smem, sms, &g) == FFT3D_OK && g >= sms;
             }
+
             if (ok) {
-                pl->fused = true; pl->fz_R = R;
+                pl->fused = true; pl->fz_R = pl->fz_R_max = R;
                 // a z tile costs ~1.2x the instructions of a y tile: 54 % of the SMs (80 of 148: best of a
                 // sweep 70..84 in both directions), rounded to whole TPCs
                 pl->fz_kz[0] = pl->fz_kz[1] = (int)(sms * 0.54 + 1.0) & ~1;
@@ -594,7 +587,7 @@ static int plan_create(fft3d_plan_t** out, long long Nx, long long Ny, long long
                 pl->fused_default = ky->fz_ng >= 2 && ky->fz_nstage >= 3 && pl->slab_bytes >= ((size_t)2 << 30);
                 pl->ring_bytes = plane * R;
                 pl->side_bytes = ((size_t)Nx * Ny * 2 * pl->esize + 255) & ~(size_t)255;
-                pl->flags_bytes = ((size_t)2 * Nx * sizeof(unsigned) + 255) & ~(size_t)255;
+                pl->flags_bytes = (((size_t)2 * Nx + FZ_CTL_WORDS) * sizeof(unsigned) + 255) & ~(size_t)255;
             }
         }
     }
@@ -612,12 +605,13 @@ static int plan_create(fft3d_plan_t** out, long long Nx, long long Ny, long long
                 int g = 0;
                 ok = prepare_kernel(ky->fc_fn[d], ky->fc_threads, ky->fc_smem, sms, &g) == FFT3D_OK && g >= sms;
             }
+
             if (ok) {
-                pl->fused = true; pl->fz_R = R;
+                pl->fused = true; pl->fz_R = pl->fz_R_max = R;
                 pl->fz_kz[0] = pl->fz_kz[1] = (sms / 2 + 1) & ~1;      // z and y tiles cost about the same here
                 pl->fused_default = pl->slab_bytes >= ((size_t)2 << 30);
                 pl->ring_bytes = plane * R;
-                pl->flags_bytes = ((size_t)2 * Nx * sizeof(unsigned) + 255) & ~(size_t)255;
+                pl->flags_bytes = (((size_t)2 * Nx + FZ_CTL_WORDS) * sizeof(unsigned) + 255) & ~(size_t)255;
             }
         }
     }
@@ -721,6 +715,23 @@ const char* fft3d_launch_impl(const fft3d_plan_t* pl, int which, int i) {
     else if (nm[0] == 'y') im = y_impl(pl);
     else if (nm[0] == 'x') im = x_impl(pl, which);
     return names[im];
+}
+
+int fft3d_set_option(fft3d_plan_t* pl, int option, long long value) {
+    if (pl == nullptr) return FFT3D_EINVAL;
+    switch (option) {
+        case FFT3D_OPT_FUSED_Z_SMS_FWD:
+        case FFT3D_OPT_FUSED_Z_SMS_INV:
+            if (value < 0 || value >= pl->num_sms || (value & 1)) return FFT3D_EINVAL;   // whole TPCs; 0 = split by CTA pairs
+            pl->fz_kz[option == FFT3D_OPT_FUSED_Z_SMS_FWD ? 0 : 1] = (int)value;
+            return FFT3D_OK;
+        case FFT3D_OPT_FUSED_RING_PLANES:
+            if (!pl->fused || value < 2 || value > pl->fz_R_max || value > pl->Nx) return FFT3D_EINVAL;
+            pl->fz_R = (int)value;
+            return FFT3D_OK;
+        default:
+            return FFT3D_EINVAL;
+    }
 }
 
 int fft3d_set_variant(fft3d_plan_t* pl, int variant) {

@@ -1,8 +1,9 @@
 // fft_configs.cuh -- which FFT lengths this build has kernels for, and how each is factored.
 //
 // CfgFor<T, N>::type = FftCfg<N, P, r0, r1, ...>: P points per thread, stage radices r_i (each
-// dividing P).  Lengths are 2^a (4..4096) and 3*2^a (6..3072): every extent in BASELINE.json's
-// configs (64, 256, 1024, 1536 = 3*2^9, 2048) and their halves for the z pass.
+// dividing P).  Lengths are 2^a (4..4096), 3*2^a (6..3072) and 5*2^a (20..1280): every extent in
+// BASELINE.json's configs (64, 256, 1024, 1536 = 3*2^9, 2048) and their halves for the z pass, plus the radix-5
+// family of SURVEY.md 8(f)-4.
 #pragma once
 #include "fft_core.cuh"
 

@@ -27,7 +27,8 @@
 //
 // Why roles: the two tile bodies are ~35 KB of straight-line code each and the two SMs of a TPC
 // share an instruction cache; with both bodies alive in one TPC 60 % of the issue stalls in the
-// FFT code were instruction fetches (ncu, profiles/).  Roles follow %smid so that a TPC never mixes.
+// FFT code were instruction fetches (ncu, profiles/).  Roles follow %smid so that a TPC never mixes; ranks inside a
+// role come from an atomic ticket (no assumption about the ids), and every spin on a global counter is bounded.
 //
 // Ordering between CTAs uses two counters per plane in global memory (zeroed before the launch):
 //   p1_done[x]    += 1 when a phase-1 tile of plane x has been stored (store complete, released at once)
@@ -43,7 +44,6 @@
 // exactly the z-tile and y-tile code of fft_zpass.cuh / fft_kernels.cuh.
 #pragma once
 #include <cstdint>
-#include <cstdio>
 
 #include "fft_core.cuh"
 #include "fft_kernels.cuh"
@@ -105,30 +105,14 @@ __device__ __forceinline__ unsigned ld_acquire(const unsigned* p) {
 __device__ __forceinline__ void red_release_add(unsigned* p, unsigned v) {
     asm volatile("red.release.gpu.global.add.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
 }
+// Spin on a global counter, bounded: ~1 us per poll, 2^24 polls > 10 s.  A pipeline that cannot make progress
+// traps -- the host then sees a launch failure and the API returns FFT3D_ECUDA -- instead of hanging the device.
 __device__ __forceinline__ void wait_count(const unsigned* p, unsigned target) {
-#ifdef FFT3D_WATCHDOG
-    long long t0 = clock64();
+    unsigned polls = 0;
     while (ld_acquire(p) < target) {
         __nanosleep(64);
-        if (clock64() - t0 > 4000000000LL) { printf("wait_count stuck: blk %d tid %d have %u want %u\n", blockIdx.x, threadIdx.x, ld_acquire(p), target); __trap(); }
+        if (++polls > (1u << 24)) __trap();
     }
-#else
-    while (ld_acquire(p) < target) __nanosleep(64);
-#endif
-}
-// mbarrier wait with a watchdog (debug builds)
-__device__ __forceinline__ void mbar_wait_dbg(unsigned long long* bar, unsigned parity, int what) {
-#ifdef FFT3D_WATCHDOG
-    long long t0 = clock64();
-    unsigned ok = 0;
-    while (!ok) {
-        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
-                     : "=r"(ok) : "r"(smem_u32(bar)), "r"(parity) : "memory");
-        if (!ok && clock64() - t0 > 4000000000LL) { printf("mbar stuck: what %d blk %d tid %d parity %u\n", what, blockIdx.x, threadIdx.x, parity); __trap(); }
-    }
-#else
-    mbar_wait(bar, parity);
-#endif
 }
 }  // namespace tma
 
@@ -152,6 +136,9 @@ struct FusedTile {
     }
     static constexpr int THREADS = threads(max_stages());
 };
+
+// words of the control block that follows the 2*Nx plane counters in the flags area (zeroed before the launch)
+enum { FZ_CTL_NZ = 0, FZ_CTL_NY = 1, FZ_CTL_ARRIVED = 2, FZ_CTL_WORDS = 8 };
 
 struct FItem { int p1, x, j; };
 
@@ -182,6 +169,7 @@ fft_zy_fused_kernel(const __grid_constant__ TensorMapBlob ring_map, const __grid
     // the groups in turn (NSTAGE need not be a multiple of NG) and a parity wait is only meaningful
     // within one phase of the barrier's current one, so a group polls seen[s] before it waits for ITS phase.
     volatile int* seen = reinterpret_cast<volatile int*>(empty + NSTAGE);
+    volatile int* role_s = seen + NSTAGE;                // [role_z, rank, nrole] broadcast from thread 0
 
     const int tid = threadIdx.x;
     if (tid == NCONS) {
@@ -199,24 +187,33 @@ fft_zy_fused_kernel(const __grid_constant__ TensorMapBlob ring_map, const __grid
 
     const int n_z = a.Ny / RPT, n_y = M / TC;            // z tiles / y tiles per plane
     const int n1 = FWD ? n_z : n_y, n2 = FWD ? n_y : n_z;
-    // Role of this CTA: z tiles or y tiles, never both -- the two bodies are ~35 KB of straight-line
-    // code each, and the SMs of a TPC share an instruction cache, so both SMs of a TPC get the same role.
-    //   kz > 0 and one CTA per SM (grid == %nsmid): SMs [0, kz) take the z tiles, the rest the y tiles
-    //   otherwise: CTA pairs (4k, 4k+1) -> z, (4k+2, 4k+3) -> y
-    unsigned smid, nsmid;
-    asm("mov.u32 %0, %%smid;" : "=r"(smid));
-    asm("mov.u32 %0, %%nsmid;" : "=r"(nsmid));
-    int role_z, rank, nrole;
-    if (a.kz > 0 && nsmid == gridDim.x && a.kz < (int)gridDim.x) {
-        role_z = (int)smid < a.kz;
-        rank = role_z ? (int)smid : (int)smid - a.kz;
-        nrole = role_z ? a.kz : (int)gridDim.x - a.kz;
-    } else {
-        const int b = blockIdx.x, g4 = gridDim.x / 4 * 4;
-        if (b < g4) { role_z = !((b >> 1) & 1); rank = ((b >> 2) << 1) | (b & 1); nrole = g4 / 2; }
-        else { role_z = !(b & 1); rank = g4 / 2 + ((b - g4) >> 1); nrole = g4 / 2; }
-        nrole += role_z ? ((int)gridDim.x - g4 + 1) / 2 : ((int)gridDim.x - g4) / 2;
+    // Role of this CTA: z tiles or y tiles, never both -- the two bodies are ~35 KB of straight-line code each,
+    // and the SMs of a TPC share an instruction cache, so both SMs of a TPC get the same role: SMs [0, kz) take
+    // the z tiles (kz even), the rest the y tiles; kz = 0: CTA pairs (4k, 4k+1) -> z, (4k+2, 4k+3) -> y.
+    // Nothing is assumed about %smid being dense or about one CTA per SM: every CTA draws its rank inside its
+    // role from an atomic ticket and learns the role sizes after a grid-wide arrival counter (cooperative launch:
+    // all CTAs are co-resident).  If a role came out empty, all CTAs fall back to alternating by blockIdx.
+    unsigned* ctl = a.flags + 2 * a.Nx;
+    if (tid == 0) {
+        unsigned smid;
+        asm("mov.u32 %0, %%smid;" : "=r"(smid));
+        const int b = blockIdx.x, G = gridDim.x;
+        int rz = (a.kz > 0 && a.kz < G) ? ((int)smid < a.kz) : !((b >> 1) & 1);
+        int rk = (int)atomicAdd(&ctl[rz ? FZ_CTL_NZ : FZ_CTL_NY], 1u);
+        __threadfence();
+        tma::red_release_add(&ctl[FZ_CTL_ARRIVED], 1u);
+        tma::wait_count(&ctl[FZ_CTL_ARRIVED], (unsigned)G);
+        const int nz = (int)tma::ld_acquire(&ctl[FZ_CTL_NZ]), ny = (int)tma::ld_acquire(&ctl[FZ_CTL_NY]);
+        int nr = rz ? nz : ny;
+        if (nz == 0 || ny == 0) {
+            rz = !(b & 1);
+            rk = b >> 1;
+            nr = rz ? (G + 1) / 2 : G / 2;
+        }
+        role_s[0] = rz; role_s[1] = rk; role_s[2] = nr;
     }
+    __syncthreads();
+    const int role_z = role_s[0], rank = role_s[1], nrole = role_s[2];
     const int my_p1 = FWD ? role_z : !role_z;            // this CTA's tiles are the phase-1 tiles
     const int nper = role_z ? n_z : n_y;                 // tiles per plane of this role
     const int total = a.Nx * nper;
@@ -233,7 +230,7 @@ fft_zy_fused_kernel(const __grid_constant__ TensorMapBlob ring_map, const __grid
                 FItem it; it.p1 = my_p1; it.x = g / nper; it.j = g - it.x * nper;
                 const int s = i % NSTAGE, n = i / NSTAGE;
                 unsigned char* dst = stages + s * FT::STAGE_BYTES;
-                if (n > 0) tma::mbar_wait_dbg(&empty[s], (unsigned)((n - 1) & 1), 0);
+                if (n > 0) tma::mbar_wait(&empty[s], (unsigned)((n - 1) & 1));
                 if (!it.p1 && it.x > ready) {
                     tma::wait_count(&p1_done[it.x], (unsigned)n1);
                     tma::fence_proxy_async_all();
@@ -245,7 +242,7 @@ fft_zy_fused_kernel(const __grid_constant__ TensorMapBlob ring_map, const __grid
                     if constexpr (FWD) {                 // rows of the real input (HBM stream)
                         const unsigned char* src = reinterpret_cast<const unsigned char*>(a.in) + (long long)it.x * plane_bytes +
                                                    (long long)it.j * ZT::TILE_BYTES;
-                        constexpr int CHUNK = 16384;
+                        constexpr int CHUNK = 65536;
                         for (int o = 0; o < ZT::TILE_BYTES; o += CHUNK)
                             tma::bulk_load_h(dst + o, src + o, ZT::TILE_BYTES - o < CHUNK ? ZT::TILE_BYTES - o : CHUNK, &full[s], pol_stream);
                     } else {                             // RPT rows gathered from the column-tiled ring: one box
@@ -256,7 +253,7 @@ fft_zy_fused_kernel(const __grid_constant__ TensorMapBlob ring_map, const __grid
                     if constexpr (FWD) {                 // column tile j of the ring plane: one contiguous block
                         const unsigned char* src = reinterpret_cast<const unsigned char*>(a.ring) +
                                                    (long long)(it.x % a.R) * plane_bytes + (long long)it.j * YT::TILE_BYTES;
-                        constexpr int CHUNK = 16384;
+                        constexpr int CHUNK = 65536;
                         for (int o = 0; o < YT::TILE_BYTES; o += CHUNK)
                             tma::bulk_load_h(dst + o, src + o, YT::TILE_BYTES - o < CHUNK ? YT::TILE_BYTES - o : CHUNK, &full[s], pol_keep);
                     } else {                             // columns of plane x gathered from the slab layout
@@ -280,7 +277,7 @@ fft_zy_fused_kernel(const __grid_constant__ TensorMapBlob ring_map, const __grid
                 const int s = i % NSTAGE, n = i / NSTAGE;
                 if (s != my_s) { ++i; continue; }
                 const unsigned char* src = stages + s * FT::STAGE_BYTES;
-                tma::mbar_wait_dbg(&done[s], (unsigned)(n & 1), 1);
+                tma::mbar_wait(&done[s], (unsigned)(n & 1));
                 if (it.p1 && it.x >= a.R && it.x - a.R > freed) {          // ring slot must have been read out
                     tma::wait_count(&p2_loaded[it.x - a.R], (unsigned)n2);
                     freed = it.x - a.R;
@@ -292,7 +289,7 @@ fft_zy_fused_kernel(const __grid_constant__ TensorMapBlob ring_map, const __grid
                     } else {                             // rows of the real output (HBM stream)
                         unsigned char* dst = reinterpret_cast<unsigned char*>(a.out) + (long long)it.x * plane_bytes +
                                              (long long)it.j * ZT::TILE_BYTES;
-                        constexpr int CHUNK = 16384;
+                        constexpr int CHUNK = 65536;
                         for (int o = 0; o < ZT::TILE_BYTES; o += CHUNK)
                             tma::bulk_store_h(dst + o, src + o, ZT::TILE_BYTES - o < CHUNK ? ZT::TILE_BYTES - o : CHUNK, pol_stream);
                     }
@@ -307,7 +304,7 @@ fft_zy_fused_kernel(const __grid_constant__ TensorMapBlob ring_map, const __grid
                     } else {                             // column tile j of the ring plane: one contiguous block
                         unsigned char* dst = reinterpret_cast<unsigned char*>(a.ring) +
                                              (long long)(it.x % a.R) * plane_bytes + (long long)it.j * YT::TILE_BYTES;
-                        constexpr int CHUNK = 16384;
+                        constexpr int CHUNK = 65536;
                         for (int o = 0; o < YT::TILE_BYTES; o += CHUNK)
                             tma::bulk_store_h(dst + o, src + o, YT::TILE_BYTES - o < CHUNK ? YT::TILE_BYTES - o : CHUNK, pol_keep);
                     }
@@ -357,15 +354,10 @@ fft_zy_fused_kernel(const __grid_constant__ TensorMapBlob ring_map, const __grid
         if (!mine) continue;
         C* buf = reinterpret_cast<C*>(stages + s * FT::STAGE_BYTES);
         while (seen[s] < n) { }                          // the previous phase of this slot has been observed
-        tma::mbar_wait_dbg(&full[s], (unsigned)(n & 1), 2);
+        tma::mbar_wait(&full[s], (unsigned)(n & 1));
         if (gt == 0) seen[s] = n + 1;
         if (!it.p1 && gt == 0) tma::red_release_add(&p2_loaded[it.x], 1u);   // the ring tile has been read
         const bool isz = FWD ? it.p1 : !it.p1;
-#ifdef FFT3D_COPY_ONLY_FUSED   // experiment: data movement without the transforms (wrong results by design)
-        tma::fence_proxy_async(); __syncwarp();
-        if ((tid & 31) == 0) tma::mbar_arrive(&done[s]);
-        continue;
-#endif
         if (isz) {
             constexpr int P = ZCfg::P;
             C v[P];

@@ -7,9 +7,6 @@
 #include "fft_configs.cuh"
 #include "fft_registry.h"
 
-#ifndef FFT3D_PREFETCH
-#define FFT3D_PREFETCH true
-#endif
 #ifndef FFT3D_N
 #error "compile with -DFFT3D_N=<length>"
 #endif
@@ -142,7 +139,7 @@ static KernelSet make_set(int dtype) {
     constexpr size_t S_SMEM = TWB + (size_t)TP::ROWS * TC * sizeof(C);
     constexpr int S_THREADS = Cfg::S * TC;
     // the second register set of the prefetching variant must fit the register file
-    constexpr bool S_PF = FFT3D_PREFETCH && (S_THREADS * (4 * Cfg::P * (int)sizeof(T) / 4 + 48) <= 65536);
+    constexpr bool S_PF = (S_THREADS * (4 * Cfg::P * (int)sizeof(T) / 4 + 48) <= 65536);
     constexpr int S_MINB = S_PF ? 1 : min_blocks(S_THREADS, Cfg::P, (int)sizeof(T), S_SMEM);
     constexpr int RPB = rows_per_block(Cfg::S);
     constexpr size_t Z_SMEM = TWB + (size_t)Cfg::N * sizeof(C) + (size_t)RPB * RowPad<Cfg>::PITCH * sizeof(C);
@@ -175,11 +172,7 @@ static KernelSet make_set(int dtype) {
         // complex fp32 rows of the user's spectrum (M+1 entries) start on 8-byte boundaries for odd l:
         // the X passes shift those tiles' windows (ODDFIX, see fft_kernels.cuh)
         // (fp64: the same shift puts the 64-byte windows of odd rows on 32-byte sectors of the user array)
-#ifdef FFT3D_NO_OF64
-        constexpr bool OF = sizeof(C) % 16 != 0;
-#else
         constexpr bool OF = true;
-#endif
         using TY = TmaTile<Cfg, TTC, T, false>;
         // X passes: same tile width (48-byte rows were tried to get a second ring stage back at
         // N = 1536 where the shifted windows land TC+2 columns: rows that are not a multiple of the
@@ -219,11 +212,7 @@ static KernelSet make_set(int dtype) {
                   ZCfg::N * sizeof(C) >= 1024) {
         // fp64: 128 threads per tile (two groups + producer = 288 threads, 224 registers each: with 256-thread groups
         // the 120-register cap made the fp64 C2R kernel spill 184 bytes per thread)
-#ifdef FFT3D_ZB64_OLD
-        constexpr int GRP = 256;
-#else
         constexpr int GRP = sizeof(T) == 8 && ZCfg::S <= 16 * 8 && 128 % ZCfg::S == 0 ? 128 : 256;
-#endif
         constexpr int RPT = GRP / ZCfg::S;
         using ZT = ZTile<ZCfg, RPT, T>;
         constexpr int NG = (ZT::max_stages(2) >= 3 && ZCfg::P <= 32) ? 2 : 1;      // P > 32: one group, 224 registers

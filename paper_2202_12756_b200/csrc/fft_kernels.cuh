@@ -447,11 +447,6 @@ fft_strided_tma_kernel(const __grid_constant__ TensorMapBlob in_map, const __gri
         XTile xt{};
         if constexpr (XPASS) xt = decode_xtile<PASS, ODDFIX>(first + i * stride, a, TC);
         tma::mbar_wait(&full[s], (unsigned)((i / NSTAGE) & 1));
-#ifdef FFT3D_COPY_ONLY   // experiment: data movement without the transform (wrong results by design)
-        tma::fence_proxy_async(); __syncwarp();
-        if ((tid & 31) == 0) tma::mbar_arrive(&done[s]);
-        continue;
-#endif
         C v[P];
         if (ODDFIX && xt.odd) read_own<Cfg, T>(v, buf, t, dense_wide);
         else read_own<Cfg, T>(v, buf, t, dense);

@@ -1,5 +1,5 @@
 // fft_radix.cuh -- register-level building blocks: complex helpers, compile-time twiddles and a
-// fully unrolled in-register DFT of any length R = 2^a * 3^b (R <= 32 used).
+// fully unrolled in-register DFT of any length R = 2^a * 3^b * 5^c (R <= 48 used).
 //
 // The transform implemented is the 1D DFT of Eq. (1)/(2) of the paper:
 //   X[k] = sum_j x[j] exp(DIR * 2 pi i j k / R),  DIR = -1 forward, +1 inverse (unnormalised).

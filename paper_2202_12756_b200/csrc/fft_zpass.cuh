@@ -235,11 +235,6 @@ __global__ void __launch_bounds__(Cfg::S * RPT * NG + 32, 1) fft_z_bulk_kernel(c
         while (seen[s] < n) { }
         tma::mbar_wait(&full[s], (unsigned)(n & 1));
         if (gt == 0) seen[s] = n + 1;
-#ifdef FFT3D_COPY_ONLY_Z   // experiment: data movement without the transform (wrong results by design)
-        tma::fence_proxy_async(); __syncwarp();
-        if ((tid & 31) == 0) tma::mbar_arrive(&done[s]);
-        continue;
-#endif
         C v[P];
         read_own<Cfg, T>(v, buf, t, dense);
         if constexpr (DIR > 0 && !C2C) {
