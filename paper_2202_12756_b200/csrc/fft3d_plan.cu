@@ -96,6 +96,13 @@ struct fft3d_plan_s {
     int fz_kz[2];              // [fwd, inv] SMs [0, kz) run the z tiles, the others the y tiles (0: split by CTA pairs)
     int fz_R_max;              // ring planes the workspace was sized for
     size_t slab_bytes, ring_bytes, side_bytes, flags_bytes;
+    // Sub-ranges the passes work on.  A plain plan covers the whole problem; the stage entry points of a
+    // distributed plan (fft3d_dist_*) run the same launch code on a copy of the plan with these narrowed.
+    long long xpn;             // yz-planes handled by the z and y passes (Nx)
+    long long xp0;             // index along x, in the slab array, of the first of them (0)
+    long long sNx;             // x extent of one virtual-slab block of the slab array: its q stride is sNx*L*M (Nx)
+    int qn;                    // virtual slabs handled by the x passes, pointers already at the first one (p)
+    int dist_G, dist_rank;     // distributed plans: number of ranks and this rank (0, 0 otherwise)
 };
 
 namespace {
@@ -218,25 +225,27 @@ bool make_map(const fft3d_plan_s* pl, TensorMapBlob* out, const void* base, int 
 // The four array views of the strided passes (sz = bytes per complex, W = sz/8 words).
 bool map_natural(const fft3d_plan_s* pl, TensorMapBlob* m, const void* base, int tc, int rows) {   // [Nx][Ny][M]
     const long long sz = 2 * pl->esize, W = sz / 8;
-    long long d[3] = {pl->M * W, pl->Ny, pl->Nx}, st[2] = {pl->M * sz, pl->Ny * pl->M * sz};
+    long long d[3] = {pl->M * W, pl->Ny, pl->xpn}, st[2] = {pl->M * sz, pl->Ny * pl->M * sz};
     int b[3] = {(int)(tc * W), rows, 1};
     return make_map(pl, m, base, 3, d, st, b);
 }
-bool map_slab_y(const fft3d_plan_s* pl, TensorMapBlob* m, const void* base, int tc, int rows) {    // [p][Nx][L][M], rows along (q,l)
+bool map_slab_y(const fft3d_plan_s* pl, TensorMapBlob* m, const void* base, int tc, int rows) {    // [p][sNx][L][M], rows along (q,l)
     const long long sz = 2 * pl->esize, W = sz / 8, L = pl->L;
-    long long d[4] = {pl->M * W, L, pl->Nx, pl->p}, st[3] = {pl->M * sz, L * pl->M * sz, pl->Nx * L * pl->M * sz};
+    // planes [xp0, xp0 + xpn) of every virtual slab: the plane coordinate of the kernels starts at 0
+    const unsigned char* b0 = reinterpret_cast<const unsigned char*>(base) + (size_t)pl->xp0 * L * pl->M * sz;
+    long long d[4] = {pl->M * W, L, pl->xpn, pl->p}, st[3] = {pl->M * sz, L * pl->M * sz, pl->sNx * L * pl->M * sz};
     int b[4] = {(int)(tc * W), (int)(rows < L ? rows : L), 1, (int)(rows < L ? 1 : rows / L)};
-    return make_map(pl, m, base, 4, d, st, b);
+    return make_map(pl, m, b0, 4, d, st, b);
 }
 bool map_slab_x(const fft3d_plan_s* pl, TensorMapBlob* m, const void* base, int tc, int rows) {    // [p][Nx][L][M], rows along x; tc = box columns
     const long long sz = 2 * pl->esize, W = sz / 8, L = pl->L;
-    long long d[4] = {pl->M * W, L, pl->Nx, pl->p}, st[3] = {pl->M * sz, L * pl->M * sz, pl->Nx * L * pl->M * sz};
+    long long d[4] = {pl->M * W, L, pl->Nx, pl->qn}, st[3] = {pl->M * sz, L * pl->M * sz, pl->Nx * L * pl->M * sz};
     int b[4] = {(int)(tc * W), 1, rows, 1};
     return make_map(pl, m, base, 4, d, st, b);
 }
 bool map_user_x(const fft3d_plan_s* pl, TensorMapBlob* m, const void* base, int tc, int rows, long long pitch = 0) {    // [p][Nx][L*pitch], rows along x
     const long long sz = 2 * pl->esize, W = sz / 8, L = pl->L, Mp1 = pitch > 0 ? pitch : pl->M + 1;
-    long long d[3] = {L * Mp1 * W, pl->Nx, pl->p}, st[2] = {L * Mp1 * sz, pl->Nx * L * Mp1 * sz};
+    long long d[3] = {L * Mp1 * W, pl->Nx, pl->qn}, st[2] = {L * Mp1 * sz, pl->Nx * L * Mp1 * sz};
     int b[3] = {(int)(tc * W), rows, 1};
     return make_map(pl, m, base, 3, d, st, b);
 }
@@ -255,7 +264,7 @@ int launch_zbulk(const fft3d_plan_s* pl, int d, const void* in, void* out, doubl
     const KernelSet* kz = pl->kz;
     ZBulkArgs z{};
     z.in = in; z.out = out; z.tw = pl->tw_zb; z.twz = pl->twz;
-    z.ntiles = pl->Nx * pl->Ny / kz->zb_rpt; z.scale = scale;
+    z.ntiles = pl->xpn * pl->Ny / kz->zb_rpt; z.scale = scale;
     long long g = z.ntiles < pl->num_sms ? z.ntiles : pl->num_sms;
     void* argv[1] = {&z};
     cudaError_t e = cudaLaunchKernel(kz->zb_fn[d], dim3((unsigned)g), dim3((unsigned)kz->zb_threads), argv, kz->zb_smem, st);
@@ -264,16 +273,13 @@ int launch_zbulk(const fft3d_plan_s* pl, int d, const void* in, void* out, doubl
 }
 
 // F1+F2 (d = 0: real `in` -> slab array) or I2+I3 (d = 1: slab array -> real `out`) as one cooperative launch
-int launch_fused(const fft3d_plan_s* pl, int d, const void* in, void* out, void* slab, void* d_work, cudaStream_t st) {
+int launch_fused(const fft3d_plan_s* pl, int d, const void* in, void* out, void* slab, void* ring, unsigned* flags, cudaStream_t st) {
     const KernelSet* ky = pl->ky;
     const bool c2c = pl->kind == 1;
     const void* fn = c2c ? ky->fc_fn[d] : ky->fz_fn[d];
     const int f_tc = c2c ? ky->fc_tc : ky->fz_tc, f_rpt = c2c ? ky->fc_rpt : ky->fz_rpt;
     const int f_threads = c2c ? ky->fc_threads : ky->fz_threads;
     const size_t f_smem = c2c ? ky->fc_smem : ky->fz_smem;
-    unsigned char* w = reinterpret_cast<unsigned char*>(d_work);
-    void* ring = w + pl->slab_bytes;
-    unsigned* flags = reinterpret_cast<unsigned*>(w + pl->slab_bytes + pl->ring_bytes + pl->side_bytes);
     if (cudaMemsetAsync(flags, 0, pl->flags_bytes, st) != cudaSuccess) { cudaGetLastError(); return FFT3D_ECUDA; }
     TensorMapBlob ring_map, slab_map;
     {   // the ring as [R][M/TC][Ny][TC]; a z tile is the box (TC, M/TC, RPT, 1)
@@ -286,7 +292,7 @@ int launch_fused(const fft3d_plan_s* pl, int d, const void* in, void* out, void*
     if (!map_slab_y(pl, &slab_map, slab, f_tc, pl->y_rows_slab)) return FFT3D_ECUDA;
     FusedArgs a{};
     a.in = in; a.out = out; a.ring = ring; a.tw_z = c2c ? pl->tw_zc : pl->tw_zb; a.twz = pl->twz; a.tw_y = pl->tw_y; a.flags = flags;
-    a.Nx = (int)pl->Nx; a.Ny = (int)pl->Ny; a.L = (int)pl->L; a.R = pl->fz_R; a.kz = pl->fz_kz[d];
+    a.Nx = (int)pl->xpn; a.Ny = (int)pl->Ny; a.L = (int)pl->L; a.R = pl->fz_R; a.kz = pl->fz_kz[d];
     a.rows_slab = pl->y_rows_slab;
     a.scale = 1.0 / ((double)pl->Nx * (double)pl->Ny * (double)pl->Nz);
     void* argv[3] = {(void*)&ring_map, (void*)&slab_map, (void*)&a};
@@ -303,11 +309,12 @@ bool x_fwd_cls4(const fft3d_plan_s* pl) {
 // Y pass as two half tiles (fft_split2.cuh): d = 0 natural `in` -> slab `out`, d = 1 slab `in` -> natural `out`
 int launch_y_split2(const fft3d_plan_s* pl, int d, const void* in, void* out, cudaStream_t st) {
     const KernelSet* ky = pl->ky;
-    const long long sz = 2 * pl->esize, W = sz / 8, M = pl->M, L = pl->L, Ny = pl->Ny, Nx = pl->Nx;
+    const long long sz = 2 * pl->esize, W = sz / 8, M = pl->M, L = pl->L, Ny = pl->Ny, Nx = pl->xpn;
     const int tc = ky->tma_tc;
     TensorMapBlob ev, od, mo;
     for (int h = 0; h < 2; ++h) {
-        const unsigned char* base = reinterpret_cast<const unsigned char*>(in) + (size_t)h * M * sz;
+        const unsigned char* base = reinterpret_cast<const unsigned char*>(in) + (size_t)h * M * sz +
+                                    (d == 1 ? (size_t)pl->xp0 * L * M * sz : 0);
         bool ok;
         if (d == 0) {       // even / odd rows of [Nx][Ny][M]
             long long dm[3] = {M * W, Ny / 2, Nx}, sb[2] = {2 * M * sz, Ny * M * sz};
@@ -315,7 +322,7 @@ int launch_y_split2(const fft3d_plan_s* pl, int d, const void* in, void* out, cu
             ok = make_map(pl, h ? &od : &ev, base, 3, dm, sb, bx);
         } else {            // even / odd rows l of [p][Nx][L][M]
             const long long Lh = L / 2;
-            long long dm[4] = {M * W, Lh, Nx, pl->p}, sb[3] = {2 * M * sz, L * M * sz, Nx * L * M * sz};
+            long long dm[4] = {M * W, Lh, Nx, pl->p}, sb[3] = {2 * M * sz, L * M * sz, pl->sNx * L * M * sz};
             const int rows = pl->y2_rows_slab;
             int bx[4] = {(int)(tc * W), (int)(rows < Lh ? rows : Lh), 1, (int)(rows < Lh ? 1 : rows / Lh)};
             ok = make_map(pl, h ? &od : &ev, base, 4, dm, sb, bx);
@@ -325,7 +332,7 @@ int launch_y_split2(const fft3d_plan_s* pl, int d, const void* in, void* out, cu
     if (!(d == 0 ? map_slab_y(pl, &mo, out, tc, pl->y_rows_slab) : map_natural(pl, &mo, out, tc, pl->y_rows_nat))) return FFT3D_ECUDA;
     TmaArgs ta{};
     ta.tw = pl->tw_y2; ta.ntz = (int)(M / tc); ta.ntiles = Nx * ta.ntz;
-    ta.L = (int)L; ta.Nx = (int)Nx; ta.Mp1 = (int)(M + 1);
+    ta.L = (int)L; ta.Nx = (int)pl->Nx; ta.Mp1 = (int)(M + 1);
     ta.in_rows = d == 0 ? pl->y2_rows_nat : pl->y2_rows_slab;
     ta.out_rows = d == 0 ? pl->y_rows_slab : pl->y_rows_nat;
     return launch_tma(ky->y2_fn[d], ky->y2_threads, ky->y2_smem, pl->num_sms, ev, od, mo, ta, st);
@@ -334,7 +341,7 @@ int launch_y_split2(const fft3d_plan_s* pl, int d, const void* in, void* out, cu
 // X pass as two half tiles (fft_split2.cuh): d = 0 packed slab `in` -> user spectrum `out`, d = 1 the reverse
 int launch_x_split2(const fft3d_plan_s* pl, int d, const void* in, void* out, cudaStream_t st) {
     const KernelSet* kx = pl->kx;
-    const long long sz = 2 * pl->esize, W = sz / 8, M = pl->M, L = pl->L, Nx = pl->Nx, p = pl->p, Mp1 = M + 1;
+    const long long sz = 2 * pl->esize, W = sz / 8, M = pl->M, L = pl->L, Nx = pl->Nx, p = pl->qn, Mp1 = M + 1;
     const int tc = kx->tma_tc_x, rows = pl->x2_rows;
     TensorMapBlob ld[2][2], mo;          // [wide][odd x rows]
     for (int wide = 0; wide < 2; ++wide)
@@ -372,7 +379,7 @@ int launch_x_split2(const fft3d_plan_s* pl, int d, const void* in, void* out, cu
 // X pass as four quarter tiles (fft_split2.cuh, fft_x_split4_kernel): d = 0 packed slab -> user spectrum, d = 1 reverse
 int launch_x_split4(const fft3d_plan_s* pl, int d, const void* in, void* out, cudaStream_t st) {
     const KernelSet* kx = pl->kx;
-    const long long sz = 2 * pl->esize, W = sz / 8, M = pl->M, L = pl->L, Nx = pl->Nx, p = pl->p, Mp1 = M + 1;
+    const long long sz = 2 * pl->esize, W = sz / 8, M = pl->M, L = pl->L, Nx = pl->Nx, p = pl->qn, Mp1 = M + 1;
     const int tc = kx->tma_tc_x, rows = pl->x4_rows;
     Split4Maps maps;
     TensorMapBlob mo;
@@ -460,6 +467,7 @@ static int plan_create(fft3d_plan_t** out, long long Nx, long long Ny, long long
     std::memset(pl, 0, sizeof(*pl));
     pl->Nx = Nx; pl->Ny = Ny; pl->Nz = Nz; pl->M = Mcols; pl->kind = kind; pl->p = virtual_slabs; pl->L = Ny / virtual_slabs;
     pl->dtype = dtype; pl->esize = dtype == FFT3D_F32 ? 4 : 8;
+    pl->xpn = Nx; pl->xp0 = 0; pl->sNx = Nx; pl->qn = virtual_slabs;
     pl->kz = kz; pl->ky = ky; pl->kx = kx; pl->num_sms = sms;
 
     int rc = upload_stage_twiddles(kz->nst, kz->radix, kz->twn, pl->esize, &pl->tw_z);
@@ -743,75 +751,66 @@ int fft3d_set_variant(fft3d_plan_t* pl, int variant) {
     return FFT3D_OK;
 }
 
-int fft3d_r2c(const fft3d_plan_t* pl, const void* d_in, void* d_out, void* d_work, void* stream) {
-    if (pl == nullptr || pl->kind != 0 || d_in == nullptr || d_out == nullptr || d_work == nullptr) return FFT3D_EINVAL;
-    const size_t rb = fft3d_real_bytes(pl), cb = fft3d_complex_bytes(pl), wb = fft3d_workspace_bytes(pl);
-    if (((uintptr_t)d_in | (uintptr_t)d_out | (uintptr_t)d_work) & 15) return FFT3D_EINVAL;
-    if (overlap(d_in, rb, d_out, cb) || overlap(d_in, rb, d_work, wb) || overlap(d_out, cb, d_work, wb))
-        return FFT3D_EINVAL;
-    cudaStream_t st = (cudaStream_t)stream;
-    const long long Nx = pl->Nx, Ny = pl->Ny, M = pl->M, L = pl->L, p = pl->p;
+// ---- the stages of the R2C / C2R pipelines, on the plan's sub-ranges (whole problem for a plain plan) ----
 
-    Recorder rec(pl, 0, st);
-    int slot = 0;
-    rec.mark(slot++);
-    const bool fz = use_fused(pl);
+// F1 + F2 (paper step 1 and steps 2-4) of planes [xp0, xp0 + xpn): real `d_in` -> slab array.
+// Fused: through `ring` (L2) with the plane counters in `flags`; unfused: through `scratch` [xpn][Ny][M].
+static int stage_fwd_zy(const fft3d_plan_t* pl, const void* d_in, void* scratch, void* slab, void* ring, unsigned* flags,
+                        cudaStream_t st, Recorder& rec, int& slot) {
+    const long long Nxp = pl->xpn, Ny = pl->Ny, M = pl->M, L = pl->L;
     int rc;
-    if (fz) {
-        // F1+F2 fused: real -> (ring in L2) -> slab array in the workspace
-        rc = launch_fused(pl, 0, d_in, nullptr, d_work, d_work, st);
-        if (rc != FFT3D_OK) return rc;
+    if (use_fused(pl)) {
+        rc = launch_fused(pl, 0, d_in, nullptr, slab, ring, flags, st);
         rec.mark(slot++);
-    } else {
-    // F1: real [Nx*Ny rows][Nz] -> packed complex [Nx][Ny][M] in d_out (scratch use)
-    ZArgs z{};
-    z.in = d_in; z.out = d_out; z.tw = pl->tw_z; z.twz = pl->twz; z.nrows = Nx * Ny; z.scale = 1.0;
+        return rc;
+    }
+    // F1: real [xpn*Ny rows][Nz] -> packed complex [xpn][Ny][M] in the scratch
     const KernelSet* kz = pl->kz;
-    if (z_impl(pl) == IMPL_BULK) rc = launch_zbulk(pl, 0, d_in, d_out, 1.0, st);
+    ZArgs z{};
+    z.in = d_in; z.out = scratch; z.tw = pl->tw_z; z.twz = pl->twz; z.nrows = Nxp * Ny; z.scale = 1.0;
+    if (z_impl(pl) == IMPL_BULK) rc = launch_zbulk(pl, 0, d_in, scratch, 1.0, st);
     else rc = launch(kz->z_fn[0], (z.nrows + kz->z_rpb - 1) / kz->z_rpb, pl->grid_z[0], kz->z_threads, kz->z_smem, &z, st);
     if (rc != FFT3D_OK) return rc;
     rec.mark(slot++);
 
-    // F2: y-axis FFT of d_out [x][y][M]; row ky goes to work[q][x][ky_l][M]  (steps 2-4 folded in)
+    // F2: y-axis FFT of the scratch [x][y][M]; row ky goes to slab[q][xp0 + x][ky_l][M]  (steps 2-4 folded in)
     const KernelSet* ky = pl->ky;
-    StridedArgs a{};
-    a.in = d_out; a.out = d_work; a.col0 = nullptr; a.tw = pl->tw_y;
-    a.ntz = (int)((M + ky->tc - 1) / ky->tc); a.ncols = (int)M; a.a_lo = 1; a.L = (int)L;
-    a.ntiles = Nx * a.ntz;
-    a.in_hi = Ny * M; a.in_lo = 0; a.in_rq = 0; a.in_rl = M;
-    a.out_hi = L * M; a.out_lo = 0; a.out_rq = Nx * L * M; a.out_rl = M;
     if (y_impl(pl) == IMPL_TMA_SPLIT2) {
-        rc = launch_y_split2(pl, 0, d_out, d_work, st);
+        rc = launch_y_split2(pl, 0, scratch, slab, st);
     } else if (y_impl(pl) == IMPL_TMA) {
         TensorMapBlob mi, mo;
-        if (!map_natural(pl, &mi, d_out, ky->tma_tc, pl->y_rows_nat) ||
-            !map_slab_y(pl, &mo, d_work, ky->tma_tc, pl->y_rows_slab)) return FFT3D_ECUDA;
+        if (!map_natural(pl, &mi, scratch, ky->tma_tc, pl->y_rows_nat) ||
+            !map_slab_y(pl, &mo, slab, ky->tma_tc, pl->y_rows_slab)) return FFT3D_ECUDA;
         TmaArgs ta{};
-        ta.tw = pl->tw_y; ta.ntz = (int)(M / ky->tma_tc); ta.ntiles = Nx * ta.ntz;
-        ta.L = (int)L; ta.Nx = (int)Nx; ta.Mp1 = (int)(M + 1); ta.in_rows = pl->y_rows_nat; ta.out_rows = pl->y_rows_slab;
+        ta.tw = pl->tw_y; ta.ntz = (int)(M / ky->tma_tc); ta.ntiles = Nxp * ta.ntz;
+        ta.L = (int)L; ta.Nx = (int)pl->Nx; ta.Mp1 = (int)(M + 1); ta.in_rows = pl->y_rows_nat; ta.out_rows = pl->y_rows_slab;
         rc = launch_tma(ky->tma_fn[TMA_Y_FWD], ky->tma_threads, ky->tma_smem_y, pl->num_sms, mi, mi, mo, ta, st);
     } else {
+        StridedArgs a{};
+        a.in = scratch; a.col0 = nullptr; a.tw = pl->tw_y;
+        a.out = reinterpret_cast<unsigned char*>(slab) + (size_t)pl->xp0 * L * M * 2 * pl->esize;
+        a.ntz = (int)((M + ky->tc - 1) / ky->tc); a.ncols = (int)M; a.a_lo = 1; a.L = (int)L;
+        a.ntiles = Nxp * a.ntz;
+        a.in_hi = Ny * M; a.in_lo = 0; a.in_rq = 0; a.in_rl = M;
+        a.out_hi = L * M; a.out_lo = 0; a.out_rq = pl->sNx * L * M; a.out_rl = M;
         rc = launch(ky->s_fn[0][KIND_LIN_SLAB], a.ntiles, pl->grid_y[0], ky->s_threads, ky->s_smem, &a, st);
     }
-    if (rc != FFT3D_OK) return rc;
     rec.mark(slot++);
-    }
+    return rc;
+}
 
-    // F3: x-axis FFT per virtual slab q and row ky_l: work (pitch M) -> d_out (pitch M+1)
+// F3 (paper step 5): x-axis FFT inside each of the qn virtual slabs: slab (pitch M) -> spectrum (pitch M+1).
+static int stage_fwd_x(const fft3d_plan_t* pl, const void* slab, void* d_out, cudaStream_t st, Recorder& rec, int& slot) {
+    const long long Nx = pl->Nx, M = pl->M, L = pl->L, p = pl->qn;
     const KernelSet* kx = pl->kx;
-    StridedArgs b{};
-    b.in = d_work; b.out = d_out; b.col0 = nullptr; b.tw = pl->tw_x;
-    b.ntz = (int)((M + kx->tc - 1) / kx->tc); b.ncols = (int)M; b.a_lo = (int)L; b.L = (int)Nx;
-    b.ntiles = (long long)p * L * b.ntz;
-    b.in_hi = Nx * L * M; b.in_lo = M; b.in_rq = 0; b.in_rl = L * M;
-    b.out_hi = Nx * L * (M + 1); b.out_lo = M + 1; b.out_rq = 0; b.out_rl = L * (M + 1);
+    int rc;
     if (x_impl(pl, 0) == IMPL_TMA_SPLIT2) {
-        rc = launch_x_split2(pl, 0, d_work, d_out, st);
+        rc = launch_x_split2(pl, 0, slab, d_out, st);
     } else if (x_impl(pl, 0) == IMPL_TMA) {
         TensorMapBlob mi, mo;
         TensorMapBlob mi2;
         const int tc = kx->tma_tc_x, of = kx->tma_oddfix;
-        if (!map_slab_x(pl, &mi, d_work, tc, pl->x_rows) || !map_slab_x(pl, &mi2, d_work, tc + 2, pl->x_rows) ||
+        if (!map_slab_x(pl, &mi, slab, tc, pl->x_rows) || !map_slab_x(pl, &mi2, slab, tc + 2, pl->x_rows) ||
             !map_user_x(pl, &mo, d_out, tc, pl->x_rows)) return FFT3D_ECUDA;
         TmaArgs ta{};
         ta.user_out = d_out;
@@ -821,73 +820,44 @@ int fft3d_r2c(const fft3d_plan_t* pl, const void* d_in, void* d_out, void* d_wor
         ta.L = (int)L; ta.Nx = (int)Nx; ta.Mp1 = (int)(M + 1); ta.in_rows = pl->x_rows; ta.out_rows = pl->x_rows;
         rc = launch_tma(kx->tma_fn[TMA_X_FWD], kx->tma_threads_x, kx->tma_smem_x, pl->num_sms, mi, mi2, mo, ta, st);
     } else {
+        StridedArgs b{};
+        b.in = slab; b.out = d_out; b.col0 = nullptr; b.tw = pl->tw_x;
+        b.ntz = (int)((M + kx->tc - 1) / kx->tc); b.ncols = (int)M; b.a_lo = (int)L; b.L = (int)Nx;
+        b.ntiles = (long long)p * L * b.ntz;
+        b.in_hi = Nx * L * M; b.in_lo = M; b.in_rq = 0; b.in_rl = L * M;
+        b.out_hi = Nx * L * (M + 1); b.out_lo = M + 1; b.out_rq = 0; b.out_rl = L * (M + 1);
         rc = launch(kx->s_fn[0][KIND_LIN_LIN], b.ntiles, pl->grid_x[0], kx->s_threads, kx->s_smem, &b, st);
     }
-    if (rc != FFT3D_OK) return rc;
     rec.mark(slot++);
-
-    // column 0 holds A + iB (planes kz = 0 and kz = Nz/2): separate them in place
-    PlaneArgs f{};
-    f.src = nullptr; f.dst = d_out; f.Nx = (int)Nx; f.Ny = (int)Ny; f.L = (int)L; f.M = (int)M;
-    if (launch_unpack_nyquist(pl->dtype, f, st) != cudaSuccess) { cudaGetLastError(); return FFT3D_ECUDA; }
-    rec.mark(slot++);
-    return FFT3D_OK;
+    return rc;
 }
 
-int fft3d_c2r(const fft3d_plan_t* pl, const void* d_in, void* d_out, void* d_work, void* stream) {
-    if (pl == nullptr || pl->kind != 0 || d_in == nullptr || d_out == nullptr || d_work == nullptr) return FFT3D_EINVAL;
-    const size_t rb = fft3d_real_bytes(pl), cb = fft3d_complex_bytes(pl), wb = fft3d_workspace_bytes(pl);
-    if (((uintptr_t)d_in | (uintptr_t)d_out | (uintptr_t)d_work) & 15) return FFT3D_EINVAL;
-    if (overlap(d_in, cb, d_out, rb) || overlap(d_in, cb, d_work, wb) || overlap(d_out, rb, d_work, wb))
-        return FFT3D_EINVAL;
-    cudaStream_t st = (cudaStream_t)stream;
-    const long long Nx = pl->Nx, Ny = pl->Ny, Nz = pl->Nz, M = pl->M, L = pl->L, p = pl->p;
-
-    // pre-pack: side[q][kx][ky_l] = sym(plane kz=0) + i sym(plane kz=Nz/2), kept at the start of
-    // the workspace until I1 has consumed it (reading R8: only the Hermitian part of the two
-    // self-conjugate planes enters Eq. (2)+(3)).
-    Recorder rec(pl, 1, st);
-    int slot = 0;
-    rec.mark(slot++);
-    const bool fz = use_fused(pl);
-    // fused: I1 writes the slab array in the workspace and I2+I3 go from there to d_out, so the side
-    // buffer sits behind the ring; unfused: I1 -> d_out (scratch) -> I2 -> workspace -> I3 -> d_out
-    void* side = fz ? (void*)(reinterpret_cast<unsigned char*>(d_work) + pl->slab_bytes + pl->ring_bytes) : d_work;
-    void* x_out = fz ? d_work : d_out;
-    PlaneArgs f{};
-    f.src = d_in; f.dst = side; f.Nx = (int)Nx; f.Ny = (int)Ny; f.L = (int)L; f.M = (int)M;
-    if (launch_pack_nyquist(pl->dtype, f, st) != cudaSuccess) { cudaGetLastError(); return FFT3D_ECUDA; }
-    rec.mark(slot++);
-
-    // I1: x-axis inverse FFT: d_in (pitch M+1, column 0 from the side buffer) -> d_out scratch (pitch M)
+// I1 (step 5 reversed): x-axis inverse FFT inside each of the qn virtual slabs: spectrum (pitch M+1, its
+// column 0 replaced by the packed `side` [qn][Nx][L]) -> slab (pitch M).
+static int stage_inv_x(const fft3d_plan_t* pl, const void* d_in, const void* side, void* slab, cudaStream_t st,
+                       Recorder& rec, int& slot) {
+    const long long Nx = pl->Nx, M = pl->M, L = pl->L, p = pl->qn;
     const KernelSet* kx = pl->kx;
-    StridedArgs b{};
-    b.in = d_in; b.out = x_out; b.col0 = side; b.tw = pl->tw_x;
-    b.ntz = (int)((M + kx->tc - 1) / kx->tc); b.ncols = (int)M; b.a_lo = (int)L; b.L = (int)Nx;
-    b.ntiles = (long long)p * L * b.ntz;
-    b.in_hi = Nx * L * (M + 1); b.in_lo = M + 1; b.in_rq = 0; b.in_rl = L * (M + 1);
-    b.c0_hi = Nx * L; b.c0_lo = 1; b.c0_rl = L;
-    b.out_hi = Nx * L * M; b.out_lo = M; b.out_rq = 0; b.out_rl = L * M;
     int rc;
     if (x_impl(pl, 1) != IMPL_PLAIN) {
         TensorMapBlob mi, mo;
         TensorMapBlob mi2;
         const int tc = kx->tma_tc_x, of = kx->tma_oddfix;
         if (!map_user_x(pl, &mi, d_in, tc, pl->x_rows) || !map_user_x(pl, &mi2, d_in, tc + 2, pl->x_rows) ||
-            !map_slab_x(pl, &mo, x_out, tc, pl->x_rows)) return FFT3D_ECUDA;
+            !map_slab_x(pl, &mo, slab, tc, pl->x_rows)) return FFT3D_ECUDA;
         TmaArgs ta{};
         ta.tw = pl->tw_x; ta.ntz = (int)(M / tc);
         ta.ntiles = of ? (long long)p * (L / 2) * (2 * ta.ntz) : (long long)p * L * ta.ntz;
         ta.L = (int)L; ta.Nx = (int)Nx; ta.Mp1 = (int)(M + 1); ta.in_rows = pl->x_rows; ta.out_rows = pl->x_rows;
-        if (x_impl(pl, 1) == IMPL_TMA_SPLIT4) rc = launch_x_split4(pl, 1, d_in, x_out, st);
-        else if (x_impl(pl, 1) == IMPL_TMA_SPLIT2) rc = launch_x_split2(pl, 1, d_in, x_out, st);
+        if (x_impl(pl, 1) == IMPL_TMA_SPLIT4) rc = launch_x_split4(pl, 1, d_in, slab, st);
+        else if (x_impl(pl, 1) == IMPL_TMA_SPLIT2) rc = launch_x_split2(pl, 1, d_in, slab, st);
         else rc = launch_tma(kx->tma_fn[TMA_X_INV], kx->tma_threads_x, kx->tma_smem_x, pl->num_sms, mi, mi2, mo, ta, st);
         rec.mark(slot++);
         // packed column 0 of the result: x-transform of the side buffer, written over the (meaningless)
         // column the tiles produced from the user's raw kz = 0 plane
         if (rc == FFT3D_OK) {
             StridedArgs c0{};
-            c0.in = side; c0.out = x_out; c0.col0 = nullptr; c0.tw = pl->tw_x;
+            c0.in = side; c0.out = slab; c0.col0 = nullptr; c0.tw = pl->tw_x;
             c0.ntz = (int)((L + kx->tc - 1) / kx->tc); c0.ncols = (int)L; c0.a_lo = 1; c0.L = (int)Nx;
             c0.ntiles = (long long)p * c0.ntz;
             c0.in_hi = Nx * L; c0.in_lo = 0; c0.in_rq = 0; c0.in_rl = L;
@@ -895,51 +865,120 @@ int fft3d_c2r(const fft3d_plan_t* pl, const void* d_in, void* d_out, void* d_wor
             rc = launch(kx->s_fn[1][KIND_LIN_LIN], c0.ntiles, pl->grid_x[1], kx->s_threads, kx->s_smem, &c0, st);
         }
     } else {
+        StridedArgs b{};
+        b.in = d_in; b.out = slab; b.col0 = side; b.tw = pl->tw_x;
+        b.ntz = (int)((M + kx->tc - 1) / kx->tc); b.ncols = (int)M; b.a_lo = (int)L; b.L = (int)Nx;
+        b.ntiles = (long long)p * L * b.ntz;
+        b.in_hi = Nx * L * (M + 1); b.in_lo = M + 1; b.in_rq = 0; b.in_rl = L * (M + 1);
+        b.c0_hi = Nx * L; b.c0_lo = 1; b.c0_rl = L;
+        b.out_hi = Nx * L * M; b.out_lo = M; b.out_rq = 0; b.out_rl = L * M;
         rc = launch(kx->s_fn[1][KIND_LIN_LIN], b.ntiles, pl->grid_x[1], kx->s_threads, kx->s_smem, &b, st);
     }
-    if (rc != FFT3D_OK) return rc;
     rec.mark(slot++);
+    return rc;
+}
 
-    if (fz) {
-        // I2+I3 fused: slab array -> (ring in L2) -> real output, normalisation included
-        rc = launch_fused(pl, 1, nullptr, d_out, d_work, d_work, st);
+// I2 + I3 (steps 4..1 reversed, with the 1/(NxNyNz) normalisation) of planes [xp0, xp0 + xpn):
+// slab array -> real `d_out`.  Fused: through `ring`; unfused: through `scratch` [xpn][Ny][M].
+static int stage_inv_yz(const fft3d_plan_t* pl, const void* slab, void* scratch, void* d_out, void* ring, unsigned* flags,
+                        cudaStream_t st, Recorder& rec, int& slot) {
+    const long long Nxp = pl->xpn, Ny = pl->Ny, M = pl->M, L = pl->L;
+    int rc;
+    if (use_fused(pl)) {
+        rc = launch_fused(pl, 1, nullptr, d_out, const_cast<void*>(slab), ring, flags, st);
         rec.mark(slot++);
         return rc;
     }
-
-    // I2: y-axis inverse FFT gathering rows from the slab layout: d_out scratch -> work [x][y][M]
+    // I2: y-axis inverse FFT gathering rows from the slab layout: slab -> scratch [x][y][M]
     const KernelSet* ky = pl->ky;
-    StridedArgs a{};
-    a.in = d_out; a.out = d_work; a.col0 = nullptr; a.tw = pl->tw_y;
-    a.ntz = (int)((M + ky->tc - 1) / ky->tc); a.ncols = (int)M; a.a_lo = 1; a.L = (int)L;
-    a.ntiles = Nx * a.ntz;
-    a.in_hi = L * M; a.in_lo = 0; a.in_rq = Nx * L * M; a.in_rl = M;
-    a.out_hi = Ny * M; a.out_lo = 0; a.out_rq = 0; a.out_rl = M;
     if (y_impl(pl) == IMPL_TMA_SPLIT2) {
-        rc = launch_y_split2(pl, 1, d_out, d_work, st);
+        rc = launch_y_split2(pl, 1, slab, scratch, st);
     } else if (y_impl(pl) == IMPL_TMA) {
         TensorMapBlob mi, mo;
-        if (!map_slab_y(pl, &mi, d_out, ky->tma_tc, pl->y_rows_slab) ||
-            !map_natural(pl, &mo, d_work, ky->tma_tc, pl->y_rows_nat)) return FFT3D_ECUDA;
+        if (!map_slab_y(pl, &mi, slab, ky->tma_tc, pl->y_rows_slab) ||
+            !map_natural(pl, &mo, scratch, ky->tma_tc, pl->y_rows_nat)) return FFT3D_ECUDA;
         TmaArgs ta{};
-        ta.tw = pl->tw_y; ta.ntz = (int)(M / ky->tma_tc); ta.ntiles = Nx * ta.ntz;
-        ta.L = (int)L; ta.Nx = (int)Nx; ta.Mp1 = (int)(M + 1); ta.in_rows = pl->y_rows_slab; ta.out_rows = pl->y_rows_nat;
+        ta.tw = pl->tw_y; ta.ntz = (int)(M / ky->tma_tc); ta.ntiles = Nxp * ta.ntz;
+        ta.L = (int)L; ta.Nx = (int)pl->Nx; ta.Mp1 = (int)(M + 1); ta.in_rows = pl->y_rows_slab; ta.out_rows = pl->y_rows_nat;
         rc = launch_tma(ky->tma_fn[TMA_Y_INV], ky->tma_threads, ky->tma_smem_y, pl->num_sms, mi, mi, mo, ta, st);
     } else {
+        StridedArgs a{};
+        a.in = reinterpret_cast<const unsigned char*>(slab) + (size_t)pl->xp0 * L * M * 2 * pl->esize;
+        a.out = scratch; a.col0 = nullptr; a.tw = pl->tw_y;
+        a.ntz = (int)((M + ky->tc - 1) / ky->tc); a.ncols = (int)M; a.a_lo = 1; a.L = (int)L;
+        a.ntiles = Nxp * a.ntz;
+        a.in_hi = L * M; a.in_lo = 0; a.in_rq = pl->sNx * L * M; a.in_rl = M;
+        a.out_hi = Ny * M; a.out_lo = 0; a.out_rq = 0; a.out_rl = M;
         rc = launch(ky->s_fn[1][KIND_SLAB_LIN], a.ntiles, pl->grid_y[1], ky->s_threads, ky->s_smem, &a, st);
     }
     if (rc != FFT3D_OK) return rc;
     rec.mark(slot++);
 
-    // I3: z-axis C2R with the 1/(NxNyNz) normalisation: work -> d_out
+    // I3: z-axis C2R with the 1/(NxNyNz) normalisation: scratch -> d_out
     const KernelSet* kz = pl->kz;
     ZArgs z{};
-    z.in = d_work; z.out = d_out; z.tw = pl->tw_z; z.twz = pl->twz; z.nrows = Nx * Ny;
-    z.scale = 1.0 / ((double)Nx * (double)Ny * (double)Nz);
-    if (z_impl(pl) == IMPL_BULK) rc = launch_zbulk(pl, 1, d_work, d_out, z.scale, st);
+    z.in = scratch; z.out = d_out; z.tw = pl->tw_z; z.twz = pl->twz; z.nrows = Nxp * Ny;
+    z.scale = 1.0 / ((double)pl->Nx * (double)Ny * (double)pl->Nz);
+    if (z_impl(pl) == IMPL_BULK) rc = launch_zbulk(pl, 1, scratch, d_out, z.scale, st);
     else rc = launch(kz->z_fn[1], (z.nrows + kz->z_rpb - 1) / kz->z_rpb, pl->grid_z[1], kz->z_threads, kz->z_smem, &z, st);
     rec.mark(slot++);
     return rc;
+}
+
+// where a plain plan keeps the pieces of its fused pipeline in the workspace: [slab array | ring | side | flags]
+static void* ws_ring(const fft3d_plan_t* pl, void* d_work) { return reinterpret_cast<unsigned char*>(d_work) + pl->slab_bytes; }
+static void* ws_side(const fft3d_plan_t* pl, void* d_work) { return reinterpret_cast<unsigned char*>(d_work) + pl->slab_bytes + pl->ring_bytes; }
+static unsigned* ws_flags(const fft3d_plan_t* pl, void* d_work) {
+    return reinterpret_cast<unsigned*>(reinterpret_cast<unsigned char*>(d_work) + pl->slab_bytes + pl->ring_bytes + pl->side_bytes);
+}
+
+int fft3d_r2c(const fft3d_plan_t* pl, const void* d_in, void* d_out, void* d_work, void* stream) {
+    if (pl == nullptr || pl->kind != 0 || pl->dist_G != 0 || d_in == nullptr || d_out == nullptr || d_work == nullptr) return FFT3D_EINVAL;
+    const size_t rb = fft3d_real_bytes(pl), cb = fft3d_complex_bytes(pl), wb = fft3d_workspace_bytes(pl);
+    if (((uintptr_t)d_in | (uintptr_t)d_out | (uintptr_t)d_work) & 15) return FFT3D_EINVAL;
+    if (overlap(d_in, rb, d_out, cb) || overlap(d_in, rb, d_work, wb) || overlap(d_out, cb, d_work, wb))
+        return FFT3D_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    Recorder rec(pl, 0, st);
+    int slot = 0;
+    rec.mark(slot++);
+    // fused: real -> (ring in L2) -> slab array in the workspace; unfused: real -> d_out (scratch use) -> workspace
+    int rc = stage_fwd_zy(pl, d_in, d_out, d_work, ws_ring(pl, d_work), ws_flags(pl, d_work), st, rec, slot);
+    if (rc != FFT3D_OK) return rc;
+    rc = stage_fwd_x(pl, d_work, d_out, st, rec, slot);
+    if (rc != FFT3D_OK) return rc;
+    // column 0 holds A + iB (planes kz = 0 and kz = Nz/2): separate them in place
+    PlaneArgs f{};
+    f.src = nullptr; f.dst = d_out; f.Nx = (int)pl->Nx; f.Ny = (int)pl->Ny; f.L = (int)pl->L; f.M = (int)pl->M;
+    if (launch_unpack_nyquist(pl->dtype, f, st) != cudaSuccess) { cudaGetLastError(); return FFT3D_ECUDA; }
+    rec.mark(slot++);
+    return FFT3D_OK;
+}
+
+int fft3d_c2r(const fft3d_plan_t* pl, const void* d_in, void* d_out, void* d_work, void* stream) {
+    if (pl == nullptr || pl->kind != 0 || pl->dist_G != 0 || d_in == nullptr || d_out == nullptr || d_work == nullptr) return FFT3D_EINVAL;
+    const size_t rb = fft3d_real_bytes(pl), cb = fft3d_complex_bytes(pl), wb = fft3d_workspace_bytes(pl);
+    if (((uintptr_t)d_in | (uintptr_t)d_out | (uintptr_t)d_work) & 15) return FFT3D_EINVAL;
+    if (overlap(d_in, cb, d_out, rb) || overlap(d_in, cb, d_work, wb) || overlap(d_out, rb, d_work, wb))
+        return FFT3D_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    Recorder rec(pl, 1, st);
+    int slot = 0;
+    rec.mark(slot++);
+    const bool fz = use_fused(pl);
+    // pre-pack: side[q][kx][ky_l] = sym(plane kz=0) + i sym(plane kz=Nz/2) (reading R8: only the Hermitian part of
+    // the two self-conjugate planes enters Eq. (2)+(3)).  Fused: I1 writes the slab array in the workspace and I2+I3
+    // go from there to d_out, so the side buffer sits behind the ring; unfused: the side buffer sits at the start
+    // of the workspace until I1 has consumed it, I1 -> d_out (scratch use) -> I2 -> workspace -> I3 -> d_out.
+    void* side = fz ? ws_side(pl, d_work) : d_work;
+    void* slab = fz ? d_work : d_out;
+    PlaneArgs f{};
+    f.src = d_in; f.dst = side; f.Nx = (int)pl->Nx; f.Ny = (int)pl->Ny; f.L = (int)pl->L; f.M = (int)pl->M;
+    if (launch_pack_nyquist(pl->dtype, f, st) != cudaSuccess) { cudaGetLastError(); return FFT3D_ECUDA; }
+    rec.mark(slot++);
+    int rc = stage_inv_x(pl, d_in, side, slab, st, rec, slot);
+    if (rc != FFT3D_OK) return rc;
+    return stage_inv_yz(pl, slab, d_work, d_out, ws_ring(pl, d_work), ws_flags(pl, d_work), st, rec, slot);
 }
 
 // 3D C2C (the paper's R2C, C2C and C2R share one workspace).  direction -1: forward,
@@ -1022,11 +1061,11 @@ int fft3d_c2c(const fft3d_plan_t* pl, const void* d_in, void* d_out, void* d_wor
 
     if (use_fused(pl)) {
         if (d == 0) {
-            rc = launch_fused(pl, 0, d_in, nullptr, d_work, d_work, st);   rec.mark(slot++); if (rc != FFT3D_OK) return rc;
+            rc = launch_fused(pl, 0, d_in, nullptr, d_work, ws_ring(pl, d_work), ws_flags(pl, d_work), st);   rec.mark(slot++); if (rc != FFT3D_OK) return rc;
             rc = x_pass(d_work, d_out);                                    rec.mark(slot++);
         } else {
             rc = x_pass(d_in, d_work);                                     rec.mark(slot++); if (rc != FFT3D_OK) return rc;
-            rc = launch_fused(pl, 1, nullptr, d_out, d_work, d_work, st);  rec.mark(slot++);
+            rc = launch_fused(pl, 1, nullptr, d_out, d_work, ws_ring(pl, d_work), ws_flags(pl, d_work), st);  rec.mark(slot++);
         }
         return rc;
     }
