@@ -128,6 +128,70 @@ int fft3d_plan_c2c(fft3d_plan_t **plan_out, long long Nx, long long Ny, long lon
 int fft3d_c2c(const fft3d_plan_t *plan, const void *d_cplx_in, void *d_cplx_out,
               void *d_work, int direction, void *cuda_stream);
 
+/* ---- Slab decomposition over G GPUs, one process and one plan per GPU -------------------------
+ * This is the paper's method itself (P:54 slabs along x; P:67-77 steps 1-5; P:86 inverse), with its exchange fused
+ * into the y pass.  Rank r of G owns
+ *     real slab     f[x_l][jy][jz],            x = r*Nx/G + x_l          [Nx/G][Ny][Nz]
+ *     spectrum part F[kx][ky_l][kz],           ky = r*Ny/G + ky_l        [Nx][Ny/G][Nz/2+1]    (Fig. 1(f))
+ * i.e. part r of the layout [G][Nx][Ny/G][Nz/2+1] that a single-GPU plan with virtual_slabs = G produces; results
+ * are bit-identical to that plan's.  The stages, each asynchronous on the caller's stream; "==" marks a point
+ * where every rank must have finished the previous stage (a barrier, or the collective itself):
+ *   forward  fft3d_dist_fwd_local   steps 1-3: z R2C + y C2C of the own planes; row ky of plane x is stored straight
+ *                                   to its place in the exchange array (the local transpose, the all-to-all and the
+ *                                   chunk transpose, as addressing of the y pass's stores)
+ *            ==  [CHUNKS layout: all-to-all of the G chunks]
+ *            fft3d_dist_fwd_x       step 5: x C2C on the own y-slab -> own spectrum part
+ *            fft3d_dist_fwd_col0    publish the packed column 0 of the own rows as a dense [Nx][Ny/G] plane part
+ *            ==  [all-gather of the plane parts, or peer pointers]
+ *            fft3d_dist_fwd_unpack  planes kz = 0 and kz = Nz/2 of the own rows (needs C(-kx,-ky): another rank's)
+ *   inverse  fft3d_dist_inv_planes  publish the planes kz = 0, Nz/2 of the own rows, [2][Nx][Ny/G]
+ *            ==  [all-gather / peer pointers]
+ *            fft3d_dist_inv_pack    Hermitian part of the two planes (reading R8) -> packed column, in d_work
+ *            fft3d_dist_inv_x       x C2C inverse on the own y-slab -> own part of the exchange array
+ *            ==  [CHUNKS layout: all-to-all]
+ *            fft3d_dist_inv_local   y C2C inverse + z C2R with 1/(NxNyNz) of the own planes -> own real slab
+ * Exchange array, two layouts:
+ *   FFT3D_XCHG_UNIFIED  one array [G][Nx][Ny/G][Nz/2] (packed complex) whose part q lives in rank q's memory: the
+ *                       forward y pass PUSHES rows into the peers' parts over NVLink (device to device, the
+ *                       self chunk like any other), the inverse y pass PULLS them.  d_xchg is the base of the whole
+ *                       array as mapped in this process (fft3d_vmm_* maps the peers' allocations into one virtual
+ *                       range; on one GPU it is simply one buffer, which is how the tests emulate G ranks).
+ *   FFT3D_XCHG_CHUNKS   a local array [G][Nx/G][Ny/G][Nz/2]: chunk q is the message for rank q; the caller
+ *                       runs the all-to-all (NCCL ncclSend/ncclRecv pairs) between the stages; after it the G received
+ *                       chunks, in source-rank order, ARE the part [Nx][Ny/G][Nz/2] (forward), and vice versa.
+ * fft3d_dist_fwd_x / fft3d_dist_inv_x take the own part [Nx][Ny/G][Nz/2] (UNIFIED: d_xchg + rank*FFT3D_DIST_SLAB bytes).
+ * Buffer sizes: fft3d_dist_bytes(plan, FFT3D_DIST_REAL | _SLAB (one part of the exchange array) | _SPEC | _PLANES
+ * (a plane part, [2][Nx][Ny/G] complex) | _WORK).  d_plane_parts: HOST array of G device pointers, entry q = rank
+ * q's plane part as addressable from this device.  G <= 16; G | Nx and G | Ny; all pointers 16-byte
+ * aligned device pointers.  fft3d_r2c / fft3d_c2r reject a distributed plan and vice versa (FFT3D_EINVAL). */
+enum { FFT3D_DIST_REAL = 0, FFT3D_DIST_SLAB = 1, FFT3D_DIST_SPEC = 2, FFT3D_DIST_PLANES = 3, FFT3D_DIST_WORK = 4 };
+enum { FFT3D_XCHG_UNIFIED = 0, FFT3D_XCHG_CHUNKS = 1 };
+int fft3d_plan_dist(fft3d_plan_t **plan_out, long long Nx, long long Ny, long long Nz, int dtype, int G, int rank);
+size_t fft3d_dist_bytes(const fft3d_plan_t *plan, int which);
+int fft3d_dist_fwd_local(const fft3d_plan_t *plan, const void *d_real_slab, void *d_xchg, int layout, void *d_work,
+                         void *cuda_stream);
+int fft3d_dist_fwd_x(const fft3d_plan_t *plan, const void *d_slab_part, void *d_spec_part, void *cuda_stream);
+int fft3d_dist_fwd_col0(const fft3d_plan_t *plan, const void *d_spec_part, void *d_plane_part, void *cuda_stream);
+int fft3d_dist_fwd_unpack(const fft3d_plan_t *plan, void *d_spec_part, const void *const *d_plane_parts, void *cuda_stream);
+int fft3d_dist_inv_planes(const fft3d_plan_t *plan, const void *d_spec_part, void *d_plane_part, void *cuda_stream);
+int fft3d_dist_inv_pack(const fft3d_plan_t *plan, const void *const *d_plane_parts, void *d_work, void *cuda_stream);
+int fft3d_dist_inv_x(const fft3d_plan_t *plan, const void *d_spec_part, void *d_slab_part, void *d_work, void *cuda_stream);
+int fft3d_dist_inv_local(const fft3d_plan_t *plan, const void *d_xchg, int layout, void *d_real_slab, void *d_work,
+                         void *cuda_stream);
+
+/* One virtual address range over G device allocations (CUDA virtual memory management) for the UNIFIED exchange
+ * array: every rank creates its part (`bytes` a multiple of fft3d_vmm_granularity(); *fd_out, if asked for, is a POSIX
+ * file descriptor the owner passes to its peers and closes afterwards), imports the peers' descriptors, and maps all
+ * G handles back to back in rank order: *va_out + q*part_bytes is then rank q's memory, readable and writable from
+ * the current device (NVLink peer access; the same device in the single-GPU tests).  Handles are plain integers
+ * (CUmemGenericAllocationHandle).  Unmap before releasing; a part stays alive while any rank holds a handle. */
+size_t fft3d_vmm_granularity(void);
+int fft3d_vmm_create(size_t bytes, unsigned long long *handle_out, int *fd_out);
+int fft3d_vmm_import(int fd, unsigned long long *handle_out);
+int fft3d_vmm_map(const unsigned long long *handles, int n, size_t part_bytes, void **va_out);
+int fft3d_vmm_unmap(void *va, int n, size_t part_bytes);
+int fft3d_vmm_release(unsigned long long handle);
+
 /* Host-buffer variant of fft3d_c2c (as fft3d_r2c_host below): H2D copy, transform, D2H copy, synchronous. */
 int fft3d_c2c_host(fft3d_plan_t *plan, const void *h_cplx_in, void *h_cplx_out, int direction);
 

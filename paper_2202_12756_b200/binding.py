@@ -22,6 +22,9 @@ EXPORTS = (
     "fft3d_c2r_host", "fft3d_launches", "fft3d_launch_name", "fft3d_set_variant", "fft3d_destroy", "fft3d_strerror",
     "fft3d_timing_enable", "fft3d_timing_read", "fft3d_plan_c2c", "fft3d_c2c", "fft3d_c2c_host",
     "fft3d_launch_impl", "fft3d_set_option",
+    "fft3d_plan_dist", "fft3d_dist_bytes", "fft3d_dist_fwd_local", "fft3d_dist_fwd_x", "fft3d_dist_fwd_col0",
+    "fft3d_dist_fwd_unpack", "fft3d_dist_inv_planes", "fft3d_dist_inv_pack", "fft3d_dist_inv_x", "fft3d_dist_inv_local",
+    "fft3d_vmm_granularity", "fft3d_vmm_create", "fft3d_vmm_import", "fft3d_vmm_map", "fft3d_vmm_unmap", "fft3d_vmm_release",
 )
 
 _lib = None
@@ -73,6 +76,31 @@ def load_library() -> ctypes.CDLL:
     lib.fft3d_launch_impl.restype = ctypes.c_char_p
     lib.fft3d_set_variant.argtypes = [vp, i]
     lib.fft3d_set_variant.restype = i
+    ull = ctypes.c_ulonglong
+    lib.fft3d_plan_dist.argtypes = [ctypes.POINTER(vp), ll, ll, ll, i, i, i]
+    lib.fft3d_plan_dist.restype = i
+    lib.fft3d_dist_bytes.argtypes = [vp, i]
+    lib.fft3d_dist_bytes.restype = sz
+    lib.fft3d_dist_fwd_local.argtypes = [vp, vp, vp, i, vp, vp]
+    lib.fft3d_dist_inv_local.argtypes = [vp, vp, i, vp, vp, vp]
+    lib.fft3d_dist_fwd_x.argtypes = [vp, vp, vp, vp]
+    lib.fft3d_dist_inv_x.argtypes = [vp, vp, vp, vp, vp]
+    lib.fft3d_dist_fwd_col0.argtypes = [vp, vp, vp, vp]
+    lib.fft3d_dist_inv_planes.argtypes = [vp, vp, vp, vp]
+    lib.fft3d_dist_fwd_unpack.argtypes = [vp, vp, ctypes.POINTER(vp), vp]
+    lib.fft3d_dist_inv_pack.argtypes = [vp, ctypes.POINTER(vp), vp, vp]
+    for nm in ("fft3d_dist_fwd_local", "fft3d_dist_inv_local", "fft3d_dist_fwd_x", "fft3d_dist_inv_x", "fft3d_dist_fwd_col0",
+               "fft3d_dist_inv_planes", "fft3d_dist_fwd_unpack", "fft3d_dist_inv_pack"):
+        getattr(lib, nm).restype = i
+    lib.fft3d_vmm_granularity.argtypes = []
+    lib.fft3d_vmm_granularity.restype = sz
+    lib.fft3d_vmm_create.argtypes = [sz, ctypes.POINTER(ull), ctypes.POINTER(i)]
+    lib.fft3d_vmm_import.argtypes = [i, ctypes.POINTER(ull)]
+    lib.fft3d_vmm_map.argtypes = [ctypes.POINTER(ull), i, sz, ctypes.POINTER(vp)]
+    lib.fft3d_vmm_unmap.argtypes = [vp, i, sz]
+    lib.fft3d_vmm_release.argtypes = [ull]
+    for nm in ("fft3d_vmm_create", "fft3d_vmm_import", "fft3d_vmm_map", "fft3d_vmm_unmap", "fft3d_vmm_release"):
+        getattr(lib, nm).restype = i
     lib.fft3d_set_option.argtypes = [vp, i, ll]
     lib.fft3d_set_option.restype = i
     lib.fft3d_timing_enable.argtypes = [vp, i]

@@ -72,6 +72,91 @@ __global__ void pack_nyquist_kernel(const PlaneArgs a) {
     }
 }
 
+// ---- distributed plans (fft3d_dist_*): the packed-column bookkeeping when the spectrum is split over G ranks ----
+// Rank q owns rows ky in [q*L, (q+1)*L) of the spectrum, stored [Nx][L][M+1].  The partner C(-kx,-ky) of an own
+// entry lives on rank (-ky mod Ny)/L, so the ranks first publish the planes involved as dense [Nx][L] arrays
+// (extract_planes), exchange them (all-gather, or peer pointers over NVLink), and then every rank fixes up its own
+// rows reading the partners from those read-only copies: no rank writes another rank's memory, nothing races.
+struct DistPlaneArgs {
+    const void* spec;            // own part of the spectrum [Nx][L][M+1]              (extract: source)
+    void* spec_out;              // own part of the spectrum                              (unpack: destination)
+    void* own;                   // own plane part [ncols][Nx][L]                         (extract: destination)
+    const void* parts[16];       // every rank's plane part [ncols][Nx][L], own included  (unpack / pack: sources)
+    void* side;                  // pack: own packed side buffer [Nx][L]
+    int Nx, Ny, L, M, q, ncols;
+};
+
+// own[c][kx][l] = spec[kx][l][c ? M : 0]
+template <typename T>
+__global__ void extract_planes_kernel(const DistPlaneArgs a) {
+    using C = cx<T>;
+    const long long n = (long long)a.Nx * a.L;
+    const C* in = reinterpret_cast<const C*>(a.spec);
+    C* out = reinterpret_cast<C*>(a.own);
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n * a.ncols;
+         i += (long long)gridDim.x * blockDim.x) {
+        const int c = (int)(i / n);
+        const long long r = i - (long long)c * n;
+        out[i] = in[r * (a.M + 1) + (c ? a.M : 0)];
+    }
+}
+
+// A(k) = (C(k) + conj C(-k))/2 -> column 0, B(k) = (C(k) - conj C(-k))/(2i) -> column M of the own rows
+template <typename T>
+__global__ void dist_unpack_kernel(const DistPlaneArgs a) {
+    using C = cx<T>;
+    const long long n = (long long)a.Nx * a.L;
+    C* out = reinterpret_cast<C*>(a.spec_out);
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+        const int kx = (int)(i / a.L), l = (int)(i % a.L), ky = a.q * a.L + l;
+        const int mx = kx == 0 ? 0 : a.Nx - kx, my = ky == 0 ? 0 : a.Ny - ky;
+        const int mq = my / a.L, ml = my - mq * a.L;
+        const C c1 = reinterpret_cast<const C*>(a.parts[a.q])[i];
+        const C c2 = reinterpret_cast<const C*>(a.parts[mq])[(long long)mx * a.L + ml];
+        out[i * (a.M + 1)] = mk<T>((T)0.5 * (c1.x + c2.x), (T)0.5 * (c1.y - c2.y));
+        out[i * (a.M + 1) + a.M] = mk<T>((T)0.5 * (c1.y + c2.y), (T)-0.5 * (c1.x - c2.x));
+    }
+}
+
+// side(k) = As(k) + i Bs(k), As / Bs the Hermitian parts of the planes kz = 0 / kz = Nz/2 (reading R8)
+template <typename T>
+__global__ void dist_pack_kernel(const DistPlaneArgs a) {
+    using C = cx<T>;
+    const long long n = (long long)a.Nx * a.L;
+    C* side = reinterpret_cast<C*>(a.side);
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+        const int kx = (int)(i / a.L), l = (int)(i % a.L), ky = a.q * a.L + l;
+        const int mx = kx == 0 ? 0 : a.Nx - kx, my = ky == 0 ? 0 : a.Ny - ky;
+        const int mq = my / a.L, ml = my - mq * a.L;
+        const long long j = (long long)mx * a.L + ml;
+        const C* own = reinterpret_cast<const C*>(a.parts[a.q]);
+        const C* oth = reinterpret_cast<const C*>(a.parts[mq]);
+        const C a1 = own[i], b1 = own[n + i], a2 = oth[j], b2 = oth[n + j];
+        const C As = mk<T>((T)0.5 * (a1.x + a2.x), (T)0.5 * (a1.y - a2.y));
+        const C Bs = mk<T>((T)0.5 * (b1.x + b2.x), (T)0.5 * (b1.y - b2.y));
+        side[i] = mk<T>(As.x - Bs.y, As.y + Bs.x);
+    }
+}
+
+template <typename T>
+static cudaError_t run_dist(void (*k)(const DistPlaneArgs), const DistPlaneArgs& a, cudaStream_t st) {
+    const long long n = (long long)a.Nx * a.L * (a.ncols > 0 ? a.ncols : 1);
+    long long blocks = (n + 255) / 256;
+    if (blocks > 148 * 16) blocks = 148 * 16;
+    k<<<(unsigned)blocks, 256, 0, st>>>(a);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_dist_extract(int dtype, const DistPlaneArgs& a, cudaStream_t st) {
+    return dtype == 0 ? run_dist<float>(extract_planes_kernel<float>, a, st) : run_dist<double>(extract_planes_kernel<double>, a, st);
+}
+cudaError_t launch_dist_unpack(int dtype, const DistPlaneArgs& a, cudaStream_t st) {
+    return dtype == 0 ? run_dist<float>(dist_unpack_kernel<float>, a, st) : run_dist<double>(dist_unpack_kernel<double>, a, st);
+}
+cudaError_t launch_dist_pack(int dtype, const DistPlaneArgs& a, cudaStream_t st) {
+    return dtype == 0 ? run_dist<float>(dist_pack_kernel<float>, a, st) : run_dist<double>(dist_pack_kernel<double>, a, st);
+}
+
 template <typename T>
 static cudaError_t run(void (*k)(const PlaneArgs), const PlaneArgs& a, cudaStream_t st) {
     const long long n = (long long)a.Nx * a.Ny;

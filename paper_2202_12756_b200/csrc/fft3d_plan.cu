@@ -49,6 +49,19 @@ struct PlaneArgs {
 cudaError_t launch_unpack_nyquist(int dtype, const PlaneArgs& a, cudaStream_t st);
 cudaError_t launch_pack_nyquist(int dtype, const PlaneArgs& a, cudaStream_t st);
 
+// the same bookkeeping for distributed plans: planes published as dense copies, own rows only (fft3d_fixup.cu)
+struct DistPlaneArgs {
+    const void* spec;
+    void* spec_out;
+    void* own;
+    const void* parts[16];
+    void* side;
+    int Nx, Ny, L, M, q, ncols;
+};
+cudaError_t launch_dist_extract(int dtype, const DistPlaneArgs& a, cudaStream_t st);
+cudaError_t launch_dist_unpack(int dtype, const DistPlaneArgs& a, cudaStream_t st);
+cudaError_t launch_dist_pack(int dtype, const DistPlaneArgs& a, cudaStream_t st);
+
 }  // namespace fft3d
 
 using namespace fft3d;
@@ -981,6 +994,150 @@ int fft3d_c2r(const fft3d_plan_t* pl, const void* d_in, void* d_out, void* d_wor
     return stage_inv_yz(pl, slab, d_work, d_out, ws_ring(pl, d_work), ws_flags(pl, d_work), st, rec, slot);
 }
 
+// ---------------------------------------------------------------------------------------------------------
+// Distributed slab decomposition over G GPUs: the paper's method itself.
+// Rank r owns the x-slab [Nx/G][Ny][Nz] of the real field and the y-slab [Nx][Ny/G][Nz/2+1] of the spectrum.
+// The stages below run the SAME launch code as the single-GPU transform on a copy of the plan narrowed to the
+// rank's planes / virtual slab; what differs between the exchange back-ends is only where the slab array lives.
+// ---------------------------------------------------------------------------------------------------------
+static size_t dist_scratch_bytes(const fft3d_plan_t* pl) { return pl->slab_bytes / (size_t)pl->dist_G; }
+static size_t dist_side_bytes(const fft3d_plan_t* pl) { return (((size_t)pl->Nx * pl->L * 2 * pl->esize) + 255) & ~(size_t)255; }
+static unsigned char* dist_ring(const fft3d_plan_t* pl, void* w) { return reinterpret_cast<unsigned char*>(w) + dist_scratch_bytes(pl); }
+static unsigned char* dist_side(const fft3d_plan_t* pl, void* w) { return dist_ring(pl, w) + pl->ring_bytes; }
+static unsigned* dist_flags(const fft3d_plan_t* pl, void* w) { return reinterpret_cast<unsigned*>(dist_side(pl, w) + dist_side_bytes(pl)); }
+
+int fft3d_plan_dist(fft3d_plan_t** out, long long Nx, long long Ny, long long Nz, int dtype, int G, int rank) {
+    if (out == nullptr) return FFT3D_EINVAL;
+    *out = nullptr;
+    if (G < 1 || G > 16 || rank < 0 || rank >= G) return FFT3D_EINVAL;
+    int rc = plan_create(out, Nx, Ny, Nz, dtype, G, 0);              // p = G: checks G | Nx and G | Ny
+    if (rc != FFT3D_OK) return rc;
+    fft3d_plan_t* pl = *out;
+    pl->dist_G = G; pl->dist_rank = rank;
+    const long long Nxl = Nx / G;
+    if (pl->fused) {
+        // the ring holds planes of the local x-slab only; fusion pays once the LOCAL arrays are far larger than L2
+        if (Nxl < 2) pl->fused = pl->fused_default = false;
+        else if (pl->fz_R > Nxl) {
+            pl->fz_R = pl->fz_R_max = (int)Nxl;
+            pl->ring_bytes = (size_t)Ny * pl->M * 2 * pl->esize * (size_t)Nxl;
+        }
+        pl->fused_default = pl->fused_default && dist_scratch_bytes(pl) >= ((size_t)2 << 30);
+    }
+    if (!pl->fused) {       // size the (unused) fused pieces of the workspace for the flags only
+        pl->ring_bytes = 0;
+        pl->flags_bytes = 256;
+    }
+    return FFT3D_OK;
+}
+
+size_t fft3d_dist_bytes(const fft3d_plan_t* pl, int which) {
+    if (pl == nullptr || pl->dist_G == 0) return 0;
+    const size_t G = (size_t)pl->dist_G, csz = 2 * (size_t)pl->esize;
+    switch (which) {
+        case FFT3D_DIST_REAL: return (size_t)pl->Nx * pl->Ny * pl->Nz * pl->esize / G;
+        case FFT3D_DIST_SLAB: return pl->slab_bytes / G;
+        case FFT3D_DIST_SPEC: return (size_t)pl->Nx * pl->L * (pl->M + 1) * csz;
+        case FFT3D_DIST_PLANES: return 2 * (size_t)pl->Nx * pl->L * csz;
+        case FFT3D_DIST_WORK: return dist_scratch_bytes(pl) + pl->ring_bytes + dist_side_bytes(pl) + pl->flags_bytes;
+        default: return 0;
+    }
+}
+
+// the plan narrowed to this rank's planes of the z and y passes
+static int dist_view_zy(const fft3d_plan_t* pl, int layout, fft3d_plan_t* v) {
+    if (layout != FFT3D_XCHG_UNIFIED && layout != FFT3D_XCHG_CHUNKS) return FFT3D_EINVAL;
+    *v = *pl;
+    v->timing = nullptr;
+    v->xpn = pl->Nx / pl->dist_G;
+    if (layout == FFT3D_XCHG_UNIFIED) { v->xp0 = pl->dist_rank * v->xpn; v->sNx = pl->Nx; }   // [G][Nx][L][M], part q on rank q
+    else { v->xp0 = 0; v->sNx = v->xpn; }                                                       // [G][Nx/G][L][M], all local
+    return FFT3D_OK;
+}
+
+int fft3d_dist_fwd_local(const fft3d_plan_t* pl, const void* d_real_slab, void* d_xchg, int layout, void* d_work, void* stream) {
+    if (pl == nullptr || pl->dist_G == 0 || d_real_slab == nullptr || d_xchg == nullptr || d_work == nullptr) return FFT3D_EINVAL;
+    if (((uintptr_t)d_real_slab | (uintptr_t)d_xchg | (uintptr_t)d_work) & 15) return FFT3D_EINVAL;
+    fft3d_plan_t v;
+    int rc = dist_view_zy(pl, layout, &v);
+    if (rc != FFT3D_OK) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    Recorder rec(&v, 0, st);
+    int slot = 0;
+    return stage_fwd_zy(&v, d_real_slab, d_work, d_xchg, dist_ring(pl, d_work), dist_flags(pl, d_work), st, rec, slot);
+}
+
+int fft3d_dist_fwd_x(const fft3d_plan_t* pl, const void* d_slab_part, void* d_spec_part, void* stream) {
+    if (pl == nullptr || pl->dist_G == 0 || d_slab_part == nullptr || d_spec_part == nullptr) return FFT3D_EINVAL;
+    if (((uintptr_t)d_slab_part | (uintptr_t)d_spec_part) & 15) return FFT3D_EINVAL;
+    fft3d_plan_t v = *pl;
+    v.timing = nullptr;
+    v.qn = 1;
+    cudaStream_t st = (cudaStream_t)stream;
+    Recorder rec(&v, 0, st);
+    int slot = 0;
+    return stage_fwd_x(&v, d_slab_part, d_spec_part, st, rec, slot);
+}
+
+static int dist_planes(const fft3d_plan_t* pl, const void* d_spec_part, void* d_plane_part, int ncols, void* stream) {
+    if (pl == nullptr || pl->dist_G == 0 || d_spec_part == nullptr || d_plane_part == nullptr) return FFT3D_EINVAL;
+    DistPlaneArgs a{};
+    a.spec = d_spec_part; a.own = d_plane_part;
+    a.Nx = (int)pl->Nx; a.Ny = (int)pl->Ny; a.L = (int)pl->L; a.M = (int)pl->M; a.q = pl->dist_rank; a.ncols = ncols;
+    if (launch_dist_extract(pl->dtype, a, (cudaStream_t)stream) != cudaSuccess) { cudaGetLastError(); return FFT3D_ECUDA; }
+    return FFT3D_OK;
+}
+int fft3d_dist_fwd_col0(const fft3d_plan_t* pl, const void* d_spec_part, void* d_plane_part, void* stream) {
+    return dist_planes(pl, d_spec_part, d_plane_part, 1, stream);
+}
+int fft3d_dist_inv_planes(const fft3d_plan_t* pl, const void* d_spec_part, void* d_plane_part, void* stream) {
+    return dist_planes(pl, d_spec_part, d_plane_part, 2, stream);
+}
+
+int fft3d_dist_fwd_unpack(const fft3d_plan_t* pl, void* d_spec_part, const void* const* d_plane_parts, void* stream) {
+    if (pl == nullptr || pl->dist_G == 0 || d_spec_part == nullptr || d_plane_parts == nullptr) return FFT3D_EINVAL;
+    DistPlaneArgs a{};
+    a.spec_out = d_spec_part;
+    for (int q = 0; q < pl->dist_G; ++q) { if (d_plane_parts[q] == nullptr) return FFT3D_EINVAL; a.parts[q] = d_plane_parts[q]; }
+    a.Nx = (int)pl->Nx; a.Ny = (int)pl->Ny; a.L = (int)pl->L; a.M = (int)pl->M; a.q = pl->dist_rank; a.ncols = 1;
+    if (launch_dist_unpack(pl->dtype, a, (cudaStream_t)stream) != cudaSuccess) { cudaGetLastError(); return FFT3D_ECUDA; }
+    return FFT3D_OK;
+}
+
+int fft3d_dist_inv_pack(const fft3d_plan_t* pl, const void* const* d_plane_parts, void* d_work, void* stream) {
+    if (pl == nullptr || pl->dist_G == 0 || d_plane_parts == nullptr || d_work == nullptr) return FFT3D_EINVAL;
+    DistPlaneArgs a{};
+    a.side = dist_side(pl, d_work);
+    for (int q = 0; q < pl->dist_G; ++q) { if (d_plane_parts[q] == nullptr) return FFT3D_EINVAL; a.parts[q] = d_plane_parts[q]; }
+    a.Nx = (int)pl->Nx; a.Ny = (int)pl->Ny; a.L = (int)pl->L; a.M = (int)pl->M; a.q = pl->dist_rank; a.ncols = 1;
+    if (launch_dist_pack(pl->dtype, a, (cudaStream_t)stream) != cudaSuccess) { cudaGetLastError(); return FFT3D_ECUDA; }
+    return FFT3D_OK;
+}
+
+int fft3d_dist_inv_x(const fft3d_plan_t* pl, const void* d_spec_part, void* d_slab_part, void* d_work, void* stream) {
+    if (pl == nullptr || pl->dist_G == 0 || d_spec_part == nullptr || d_slab_part == nullptr || d_work == nullptr) return FFT3D_EINVAL;
+    if (((uintptr_t)d_slab_part | (uintptr_t)d_spec_part | (uintptr_t)d_work) & 15) return FFT3D_EINVAL;
+    fft3d_plan_t v = *pl;
+    v.timing = nullptr;
+    v.qn = 1;
+    cudaStream_t st = (cudaStream_t)stream;
+    Recorder rec(&v, 1, st);
+    int slot = 0;
+    return stage_inv_x(&v, d_spec_part, dist_side(pl, d_work), d_slab_part, st, rec, slot);
+}
+
+int fft3d_dist_inv_local(const fft3d_plan_t* pl, const void* d_xchg, int layout, void* d_real_slab, void* d_work, void* stream) {
+    if (pl == nullptr || pl->dist_G == 0 || d_real_slab == nullptr || d_xchg == nullptr || d_work == nullptr) return FFT3D_EINVAL;
+    if (((uintptr_t)d_real_slab | (uintptr_t)d_xchg | (uintptr_t)d_work) & 15) return FFT3D_EINVAL;
+    fft3d_plan_t v;
+    int rc = dist_view_zy(pl, layout, &v);
+    if (rc != FFT3D_OK) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    Recorder rec(&v, 1, st);
+    int slot = 0;
+    return stage_inv_yz(&v, d_xchg, d_work, d_real_slab, dist_ring(pl, d_work), dist_flags(pl, d_work), st, rec, slot);
+}
+
 // 3D C2C (the paper's R2C, C2C and C2R share one workspace).  direction -1: forward,
 // unnormalised (z rows, y lines with the slab permutation of steps 2-4, x lines: steps 1 and 5);
 // +1: inverse, scaled by 1/(NxNyNz), the passes in reverse order.
@@ -1090,7 +1247,7 @@ static void timing_free(fft3d_plan_t* pl) {
 }
 
 int fft3d_timing_enable(fft3d_plan_t* pl, int max_calls) {
-    if (pl == nullptr || max_calls < 0 || max_calls > 4096) return FFT3D_EINVAL;
+    if (pl == nullptr || pl->dist_G != 0 || max_calls < 0 || max_calls > 4096) return FFT3D_EINVAL;
     timing_free(pl);
     if (max_calls == 0) return FFT3D_OK;
     TimingState* t = new (std::nothrow) TimingState();

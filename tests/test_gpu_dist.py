@@ -1,0 +1,115 @@
+"""The slab decomposition over G ranks (csrc: fft3d_dist_*), proven on ONE GPU:
+all G ranks' stages run one after the other on the device (paper_2202_12756_b200/dist.py::EmulatedRanks) and must
+reproduce, bit for bit, the monolithic transform with virtual_slabs = G -- which tests/test_gpu_parity.py holds against
+the fp64 oracle -- and the oracle itself within BASELINE.json's tolerance.  Both exchange layouts (UNIFIED: the y pass
+stores straight into the owners' parts; CHUNKS: explicit all-to-all of Nx/G x Ny/G chunks), and the
+UNIFIED array as G separate allocations mapped into one virtual range (CUDA VMM), as on a real NVLink node."""
+import math
+
+import numpy as np
+import pytest
+import torch
+
+pytestmark = pytest.mark.gpu
+
+
+def tol(shape, dtype):
+    n = shape[0] * shape[1] * shape[2]
+    return (2e-6 if dtype == torch.float32 else 1e-13) * math.log2(n)
+
+
+@pytest.fixture(scope="module")
+def fft():
+    import paper_2202_12756_b200 as m
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    m.load_library()
+    return m
+
+
+CASES = [
+    # shape, G, variant
+    ((64, 64, 64), 2, 0),
+    ((64, 64, 64), 4, 0),
+    ((64, 64, 64), 8, 0),
+    ((32, 48, 24), 4, 1),          # plain-load kernels, radix 3
+    ((256, 128, 256), 8, 0),       # TMA passes, slab boxes spanning whole slabs
+    ((1024, 16, 32), 4, 0),        # FFT-1024 x passes with the four-class windows on every rank's slab
+    ((1536, 32, 64), 8, 0),        # x passes as two half tiles
+    ((16, 2048, 16), 4, 0),        # y passes as two half tiles, plane offsets in their even/odd row maps
+    ((64, 256, 256), 8, 3),        # fused z+y kernels on 8 planes per rank
+    ((128, 256, 256), 2, 3),
+]
+
+
+@pytest.mark.parametrize("shape,G,variant", CASES)
+@pytest.mark.parametrize("dtype", [torch.float32, torch.float64])
+@pytest.mark.parametrize("layout", [0, 1])
+def test_emulated_ranks_equal_monolithic_transform(fft, oracle_mod, shape, G, variant, dtype, layout):
+    from paper_2202_12756_b200 import dist, inputs
+    f = inputs.uniform_grid(shape, dtype, seed=21).cuda()
+    mono = fft.Plan(*shape, dtype=dtype, virtual_slabs=G)
+    mono.set_variant(variant)
+    ref = mono.r2c(f)
+    em = dist.EmulatedRanks(*shape, dtype, G, layout=layout, variant=variant)
+    spec = torch.empty_like(ref)
+    em.forward(f, spec)
+    torch.cuda.synchronize()
+    assert torch.equal(torch.view_as_real(spec), torch.view_as_real(ref)), "forward differs from the monolithic plan"
+    # inverse of a random, NOT Hermitian-consistent spectrum (reading R8)
+    S = mono.from_natural(inputs.random_spectrum(shape, mono.complex_dtype, seed=22).cuda())
+    ref_back = mono.c2r(S)
+    back = torch.empty_like(f)
+    em.inverse(S, back)
+    torch.cuda.synchronize()
+    assert torch.equal(back, ref_back), "inverse differs from the monolithic plan"
+    # and against the oracle directly (one layout is enough: the results are bit-identical)
+    if layout == 0 and shape[0] * shape[1] * shape[2] <= 1 << 24:
+        F_ref = oracle_mod.r2c(f.cpu().double().numpy())
+        F = mono.to_natural(spec).cpu().numpy().astype(np.complex128)
+        assert np.linalg.norm((F - F_ref).ravel()) <= tol(shape, dtype) * np.linalg.norm(F_ref.ravel())
+    em.close()
+    mono.close()
+
+
+def test_unified_array_over_vmm_mappings(fft):
+    """The UNIFIED exchange array as G separate device allocations mapped back to back (fft3d_vmm_*): TMA stores of
+    the y pass land in the right allocation, TMA loads of the inverse find them."""
+    from paper_2202_12756_b200 import dist, inputs
+    shape, G, dtype = (256, 256, 256), 4, torch.float32
+    plan = dist.DistPlan(*shape, dtype, G, 0)
+    part = plan.nbytes(dist.DIST_SLAB)
+    plan.close()
+    if not dist.UnifiedExchange.usable(part):
+        pytest.skip("part size %d is not a multiple of the VMM granularity" % part)
+    f = inputs.normal_grid(shape, dtype, seed=23).cuda()
+    mono = fft.Plan(*shape, dtype=dtype, virtual_slabs=G)
+    ref = mono.r2c(f)
+    em = dist.EmulatedRanks(*shape, dtype, G, layout=dist.XCHG_UNIFIED, vmm=True)
+    spec = torch.empty_like(ref)
+    em.forward(f, spec)
+    back = torch.empty_like(f)
+    em.inverse(spec, back)
+    torch.cuda.synchronize()
+    assert torch.equal(torch.view_as_real(spec), torch.view_as_real(ref))
+    assert torch.equal(back, mono.c2r(ref))
+    em.close()
+    mono.close()
+
+
+def test_dist_argument_errors(fft):
+    from paper_2202_12756_b200 import dist
+    with pytest.raises(fft.Fft3dError):
+        dist.DistPlan(64, 64, 64, torch.float32, 3, 0)        # G must divide Nx and Ny
+    with pytest.raises(fft.Fft3dError):
+        dist.DistPlan(64, 64, 64, torch.float32, 4, 4)        # rank out of range
+    with pytest.raises(fft.Fft3dError):
+        dist.DistPlan(64, 64, 64, torch.float32, 32, 0)       # G <= 16
+    p = dist.DistPlan(64, 64, 64, torch.float32, 4, 1)
+    assert p.nbytes(dist.DIST_REAL) == 16 * 64 * 64 * 4 and p.nbytes(dist.DIST_SPEC) == 64 * 16 * 33 * 8
+    assert p.nbytes(dist.DIST_SLAB) == 64 * 16 * 32 * 8 and p.nbytes(dist.DIST_PLANES) == 2 * 64 * 16 * 8
+    lib = fft.load_library()
+    x = torch.zeros(1 << 20, device="cuda")
+    assert lib.fft3d_r2c(p._h, x.data_ptr(), x.data_ptr(), x.data_ptr(), None) == 1     # a distributed plan is not a plain one
+    mono = fft.Plan(64, 64, 64, dtype=torch.float32, virtual_slabs=4)
+    assert lib.fft3d_dist_fwd_x(mono._h, x.data_ptr(), x.data_ptr(), None) == 1
+    p.close(); mono.close()
