@@ -50,18 +50,26 @@ def _uniform01(n0: int, n1: int, seed: int, stream: int, device) -> torch.Tensor
     return _hash_u53(idx, seed, stream).to(torch.float64) * (1.0 / (1 << 53))
 
 
-def _fill(shape, dtype, device, fn, chunk=1 << 24) -> torch.Tensor:
+def _fill(shape, dtype, device, fn, chunk=1 << 24, x_range=None) -> torch.Tensor:
+    """fn(a, b) = values for linear indices a..b-1 of the whole grid; x_range = (x0, x1) fills only the x-slab
+    [x0, x1) of it (a rank's slab of a distributed field: the same values as in the whole grid)."""
+    if x_range is not None:
+        plane = int(np.prod(shape[1:]))
+        shape = (x_range[1] - x_range[0],) + tuple(shape[1:])
+        base = x_range[0] * plane
+    else:
+        base = 0
     n = int(np.prod(shape))
     out = torch.empty(n, dtype=dtype, device=device)
     for a in range(0, n, chunk):
         b = min(n, a + chunk)
-        out[a:b] = fn(a, b).to(dtype)
+        out[a:b] = fn(base + a, base + b).to(dtype)
     return out.reshape(shape)
 
 
-def uniform_grid(shape, dtype=torch.float64, seed=0, device="cpu") -> torch.Tensor:
+def uniform_grid(shape, dtype=torch.float64, seed=0, device="cpu", x_range=None) -> torch.Tensor:
     """i.i.d. uniform[-1,1) (BASELINE.json configs[0] and configs[4])."""
-    return _fill(shape, dtype, device, lambda a, b: 2.0 * _uniform01(a, b, seed, 0, device) - 1.0)
+    return _fill(shape, dtype, device, lambda a, b: 2.0 * _uniform01(a, b, seed, 0, device) - 1.0, x_range=x_range)
 
 
 def _normal(a, b, seed, stream, device):
@@ -70,12 +78,12 @@ def _normal(a, b, seed, stream, device):
     return torch.sqrt(-2.0 * torch.log1p(-u1)) * torch.cos(2.0 * math.pi * u2)
 
 
-def normal_grid(shape, dtype=torch.float32, seed=0, device="cpu", sigma=1.0) -> torch.Tensor:
+def normal_grid(shape, dtype=torch.float32, seed=0, device="cpu", sigma=1.0, x_range=None) -> torch.Tensor:
     """i.i.d. N(0, sigma^2) by Box-Muller on the hash uniforms (configs[3])."""
-    return _fill(shape, dtype, device, lambda a, b: sigma * _normal(a, b, seed, 2, device))
+    return _fill(shape, dtype, device, lambda a, b: sigma * _normal(a, b, seed, 2, device), x_range=x_range)
 
 
-def _mode_sum(shape, modes, dtype, device, xchunk=32) -> torch.Tensor:
+def _mode_sum(shape, modes, dtype, device, xchunk=32, x_range=None) -> torch.Tensor:
     """f(j) = sum_m A_m cos(2 pi (kx jx/Nx + ky jy/Ny + kz jz/Nz) + phi_m), evaluated in
     fp64 as Re sum_m A_m e^{i phi_m} X_m[jx] Y_m[jy] Z_m[jz] (plain products, no transform)."""
     Nx, Ny, Nz = shape
@@ -93,14 +101,15 @@ def _mode_sum(shape, modes, dtype, device, xchunk=32) -> torch.Tensor:
     X, Y, Z = phase(Nx, k[:, 0]), phase(Ny, k[:, 1]), phase(Nz, k[:, 2])
     coef = torch.complex(amp * torch.cos(phi), amp * torch.sin(phi))
     YZ = (Y[:, :, None] * Z[:, None, :]).reshape(len(modes), Ny * Nz)              # (M,Ny*Nz)
-    out = torch.empty((Nx, Ny * Nz), dtype=dtype, device=device)
-    for a in range(0, Nx, xchunk):
-        b = min(Nx, a + xchunk)
+    x0, x1 = x_range if x_range is not None else (0, Nx)
+    out = torch.empty((x1 - x0, Ny * Nz), dtype=dtype, device=device)
+    for a in range(x0, x1, xchunk):
+        b = min(x1, a + xchunk)
         XA = (coef[:, None] * X[:, a:b]).transpose(0, 1)                           # (xc,M)
         # real part of a complex product-sum, written with real tensors
         re = XA.real.contiguous() @ YZ.real.contiguous() - XA.imag.contiguous() @ YZ.imag.contiguous()
-        out[a:b] = re.to(dtype)
-    return out.reshape(Nx, Ny, Nz)
+        out[a - x0:b - x0] = re.to(dtype)
+    return out.reshape(x1 - x0, Ny, Nz)
 
 
 def sinusoid_grid(shape, dtype=torch.float32, seed=0, device="cpu", n_modes=16, kmax=20,
@@ -119,7 +128,7 @@ def sinusoid_grid(shape, dtype=torch.float32, seed=0, device="cpu", n_modes=16, 
     return g.to(dtype), modes
 
 
-def turbulence_grid(shape, dtype=torch.float32, seed=0, device="cpu", n_modes=128, kmax=None):
+def turbulence_grid(shape, dtype=torch.float32, seed=0, device="cpu", n_modes=128, kmax=None, x_range=None):
     """configs[2] stand-in (reading R16): a turbulence-like field built directly in
     physical space as n_modes random-phase Fourier modes, wavevectors drawn uniformly from the
     integer lattice shell 1 <= |k| <= kmax (kmax = N//3 = 341 at 1024^3) with kz >= 0, distinct
@@ -148,7 +157,7 @@ def turbulence_grid(shape, dtype=torch.float32, seed=0, device="cpu", n_modes=12
     ms = sum(a * a for _, a, _ in modes) / 2.0        # mean square of a sum of distinct cosines
     s = 1.0 / math.sqrt(ms)
     modes = [(k, a * s, ph) for k, a, ph in modes]
-    return _mode_sum(shape, modes, dtype, device), modes
+    return _mode_sum(shape, modes, dtype, device, x_range=x_range), modes
 
 
 def eq5_grid(shape, dtype=torch.float64, device="cpu") -> torch.Tensor:

@@ -1,8 +1,8 @@
-"""The N>1 plumbing of bench.py on CPU: world_size-2 gloo process groups.
+"""The N>1 timing plumbing of bench.py on CPU: world_size-2 gloo process groups.
 
-The path does not shard (one transform = one GPU): bench.py --gpus N runs N replicas with no
-data-path collective; what the ranks exchange is the barrier and the max-over-ranks of the timed
-region.  These tests run that host logic with two real processes.
+bench.py --gpus N slab-decomposes ONE grid over the N ranks (strong scaling; the exchange itself is covered by
+tests/test_dist_plumbing.py); what bench.py adds is the barrier and the max-over-ranks of the timed region and the
+whole-job rate.  These tests run that host logic with two real processes.
 """
 import json
 import os
@@ -36,7 +36,7 @@ def _worker(rank, world, port, q):
     dist.barrier()
     # rank r "measured" (10 + 5 r) ms per step: the job is as slow as its slowest replica
     ms = bench.max_over_ranks(10.0 + 5.0 * r, dist)
-    value = bench.job_gflops(w, (64, 64, 64), ms * 1e-3)
+    value = bench.job_gflops((64, 64, 64), ms * 1e-3)
     dist.barrier()
     dist.destroy_process_group()
     q.put((r, w, lr, ms, value))
@@ -58,7 +58,7 @@ def test_max_over_ranks_and_job_value_world2():
     for r, (rank, world, local_rank, ms, value) in enumerate(out):
         assert (rank, world, local_rank) == (r, 2, r)
         assert ms == 15.0                                  # max over ranks, seen by every rank
-        assert value == pytest.approx(2 * one)             # whole-job aggregate = 2 replicas
+        assert value == pytest.approx(one)                 # strong scaling: ONE grid over the ranks in the slowest rank's time
 
 
 def test_single_process_needs_no_group():
@@ -67,7 +67,7 @@ def test_single_process_needs_no_group():
     assert bench.max_over_ranks(3.5, None) == 3.5
     n = 1024 ** 3
     assert bench.flops_pair((1024, 1024, 1024)) == 5.0 * n * 30          # 5 N^3 log2 N^3, BASELINE.json metric
-    assert bench.job_gflops(1, (1024,) * 3, 1.0) == pytest.approx(5.0 * n * 30 / 1e9)
+    assert bench.job_gflops((1024,) * 3, 1.0) == pytest.approx(5.0 * n * 30 / 1e9)
 
 
 def test_reference_arm_under_torchrun_prints_one_line():
