@@ -310,7 +310,7 @@ def run_cuda(args):
     world, rank, local_rank = dist_env()
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: the FFT path has no CPU fallback")
-    if world > 1:
+    if world > 1 or args.dist:
         return run_cuda_dist(args)
     torch.cuda.set_device(local_rank)
     dev = torch.device("cuda", local_rank)
@@ -449,7 +449,13 @@ def run_cuda_dist(args):
     world, rank, local_rank = dist_env()
     torch.cuda.set_device(local_rank)
     dev = torch.device("cuda", local_rank)
-    dist = dist_init(world, "nccl", dev)
+    if world == 1:                                  # --dist on one rank: a one-member group
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        os.environ.setdefault("MASTER_PORT", "29531")
+        import torch.distributed as dist
+        dist.init_process_group("nccl", rank=0, world_size=1, device_id=dev)
+    else:
+        dist = dist_init(world, "nccl", dev)
     n = args.n
     label, kind, _p = workload_for(n)
     shape = (n, n, n)
@@ -633,6 +639,7 @@ def main():
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--size", "--n", dest="n", type=int, default=1024)
     ap.add_argument("--slabs", type=int, default=0, help="virtual_slabs (0: the value BASELINE.json gives for the size)")
+    ap.add_argument("--dist", action="store_true", help="run the slab-decomposed driver even with one rank")
     ap.add_argument("--exchange", default="chunks", choices=["chunks", "unified"],
                     help="N > 1: all-to-all of chunks over NCCL, or stores straight into the peers' memory (VMM)")
     ap.add_argument("--e2e-steps", type=int, default=2)

@@ -128,6 +128,19 @@ int fft3d_plan_c2c(fft3d_plan_t **plan_out, long long Nx, long long Ny, long lon
 int fft3d_c2c(const fft3d_plan_t *plan, const void *d_cplx_in, void *d_cplx_out,
               void *d_work, int direction, void *cuda_stream);
 
+/* Padded in-place layout (P:67 counts Nx/p x Ny x (Nz/2+1) "data points" per GPU: FFTW's in-place
+ * convention).  ONE buffer of fft3d_complex_bytes() holds the real field as rows of Nz+2 reals,
+ *     f[jx][jy][jz] at ((jx*Ny + jy)*(Nz+2) + jz), the last two reals of a row unused,
+ * and, after fft3d_r2c_inplace, its half spectrum in the slab layout [p][Nx][Ny/p][Nz/2+1] (p = 1: F[kx][ky][kz]
+ * over the same rows).  fft3d_c2r_inplace is the inverse (scaled by 1/(NxNyNz)); it overwrites the spectrum.
+ * d_work: fft3d_workspace_bytes() bytes (the slab array + one Nx*Ny complex plane).  Same extents as fft3d_plan.
+ * Rows of this layout start on 8-byte boundaries in fp32, so its z pass and the natural side of its y pass run the
+ * plain-load kernels (fft3d_launch_impl reports "plain"); expect ~1.3x the time of the out-of-place transform.
+ * fft3d_r2c / fft3d_c2r reject such a plan and vice versa (FFT3D_EINVAL). */
+int fft3d_plan_inplace(fft3d_plan_t **plan_out, long long Nx, long long Ny, long long Nz, int dtype, int virtual_slabs);
+int fft3d_r2c_inplace(const fft3d_plan_t *plan, void *d_data, void *d_work, void *cuda_stream);
+int fft3d_c2r_inplace(const fft3d_plan_t *plan, void *d_data, void *d_work, void *cuda_stream);
+
 /* ---- Slab decomposition over G GPUs, one process and one plan per GPU -------------------------
  * This is the paper's method itself (P:54 slabs along x; P:67-77 steps 1-5; P:86 inverse), with its exchange fused
  * into the y pass.  Rank r of G owns

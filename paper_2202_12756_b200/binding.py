@@ -22,6 +22,7 @@ EXPORTS = (
     "fft3d_c2r_host", "fft3d_launches", "fft3d_launch_name", "fft3d_set_variant", "fft3d_destroy", "fft3d_strerror",
     "fft3d_timing_enable", "fft3d_timing_read", "fft3d_plan_c2c", "fft3d_c2c", "fft3d_c2c_host",
     "fft3d_launch_impl", "fft3d_set_option",
+    "fft3d_plan_inplace", "fft3d_r2c_inplace", "fft3d_c2r_inplace",
     "fft3d_plan_dist", "fft3d_dist_bytes", "fft3d_dist_fwd_local", "fft3d_dist_fwd_x", "fft3d_dist_fwd_col0",
     "fft3d_dist_fwd_unpack", "fft3d_dist_inv_planes", "fft3d_dist_inv_pack", "fft3d_dist_inv_x", "fft3d_dist_inv_local",
     "fft3d_vmm_granularity", "fft3d_vmm_create", "fft3d_vmm_import", "fft3d_vmm_map", "fft3d_vmm_unmap", "fft3d_vmm_release",
@@ -77,6 +78,11 @@ def load_library() -> ctypes.CDLL:
     lib.fft3d_set_variant.argtypes = [vp, i]
     lib.fft3d_set_variant.restype = i
     ull = ctypes.c_ulonglong
+    lib.fft3d_plan_inplace.argtypes = [ctypes.POINTER(vp), ll, ll, ll, i, i]
+    lib.fft3d_plan_inplace.restype = i
+    for nm in ("fft3d_r2c_inplace", "fft3d_c2r_inplace"):
+        getattr(lib, nm).argtypes = [vp, vp, vp, vp]
+        getattr(lib, nm).restype = i
     lib.fft3d_plan_dist.argtypes = [ctypes.POINTER(vp), ll, ll, ll, i, i, i]
     lib.fft3d_plan_dist.restype = i
     lib.fft3d_dist_bytes.argtypes = [vp, i]
@@ -299,6 +305,40 @@ class Plan:
             self.close()
         except Exception:
             pass
+
+
+class PlanInplace(Plan):
+    """fft3d_plan_inplace: the padded in-place layout (rows of Nz+2 reals; the spectrum overwrites the field)."""
+
+    _PLAN_FN = "fft3d_plan_inplace"
+
+    def empty_data(self, device="cuda"):
+        """The shared buffer, as a real tensor [Nx][Ny][Nz+2]."""
+        Nx, Ny, Nz = self.shape
+        return torch.empty((Nx, Ny, Nz + 2), dtype=self.real_dtype, device=device)
+
+    def as_spectrum(self, data: torch.Tensor) -> torch.Tensor:
+        """The same memory viewed as the flat slab-layout spectrum."""
+        return torch.view_as_complex(data.reshape(-1, 2))
+
+    def _run(self, name, data, work, stream):
+        self._check(data, self.real_dtype, self.complex_bytes, "data")
+        tmp = []
+        if work is None:
+            work = self.empty_workspace(data.device)
+            tmp.append(work)
+        self._check_work(work, data)
+        s = self._stream(stream, data, tmp)
+        rc = getattr(self._lib, name)(self._h, data.data_ptr(), work.data_ptr(), ctypes.c_void_p(s.cuda_stream))
+        if rc != 0:
+            raise Fft3dError(rc, name)
+        return data
+
+    def r2c_inplace(self, data, work=None, stream=None):
+        return self._run("fft3d_r2c_inplace", data, work, stream)
+
+    def c2r_inplace(self, data, work=None, stream=None):
+        return self._run("fft3d_c2r_inplace", data, work, stream)
 
 
 class PlanC2C(Plan):

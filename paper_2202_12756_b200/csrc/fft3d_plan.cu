@@ -116,6 +116,9 @@ struct fft3d_plan_s {
     long long sNx;             // x extent of one virtual-slab block of the slab array: its q stride is sNx*L*M (Nx)
     int qn;                    // virtual slabs handled by the x passes, pointers already at the first one (p)
     int dist_G, dist_rank;     // distributed plans: number of ranks and this rank (0, 0 otherwise)
+    long long nat_pitch;       // complex elements per row of the natural-layout intermediate [x][y][.]: M, or M+1 for
+                               // the padded in-place layout, whose rows only the plain-load kernels can address
+    int inplace;               // 1: plan of fft3d_plan_inplace (fft3d_r2c_inplace / fft3d_c2r_inplace)
 };
 
 namespace {
@@ -480,7 +483,7 @@ static int plan_create(fft3d_plan_t** out, long long Nx, long long Ny, long long
     std::memset(pl, 0, sizeof(*pl));
     pl->Nx = Nx; pl->Ny = Ny; pl->Nz = Nz; pl->M = Mcols; pl->kind = kind; pl->p = virtual_slabs; pl->L = Ny / virtual_slabs;
     pl->dtype = dtype; pl->esize = dtype == FFT3D_F32 ? 4 : 8;
-    pl->xpn = Nx; pl->xp0 = 0; pl->sNx = Nx; pl->qn = virtual_slabs;
+    pl->xpn = Nx; pl->xp0 = 0; pl->sNx = Nx; pl->qn = virtual_slabs; pl->nat_pitch = Mcols;
     pl->kz = kz; pl->ky = ky; pl->kx = kx; pl->num_sms = sms;
 
     int rc = upload_stage_twiddles(kz->nst, kz->radix, kz->twn, pl->esize, &pl->tw_z);
@@ -668,6 +671,7 @@ long long fft3d_index(const fft3d_plan_t* pl, long long kx, long long ky, long l
 }
 
 static bool use_fused(const fft3d_plan_t* pl) {
+    if (pl->nat_pitch != pl->M) return false;
     return (pl->variant == 0 && pl->fused_default) || (pl->variant == 3 && pl->fused);
 }
 static bool use_tma(const fft3d_plan_t* pl) { return pl->variant != 1; }
@@ -675,8 +679,9 @@ static bool use_tma(const fft3d_plan_t* pl) { return pl->variant != 1; }
 // Which implementation each pass of an R2C/C2R plan runs with the current variant (one place: the launch
 // code below and fft3d_launch_impl both ask these).
 enum PassImpl { IMPL_PLAIN = 0, IMPL_TMA, IMPL_TMA_SPLIT2, IMPL_TMA_SPLIT4, IMPL_BULK, IMPL_FUSED, IMPL_FIXUP };
-static PassImpl z_impl(const fft3d_plan_t* pl) { return use_tma(pl) && pl->bulk_z ? IMPL_BULK : IMPL_PLAIN; }
+static PassImpl z_impl(const fft3d_plan_t* pl) { return use_tma(pl) && pl->bulk_z && pl->nat_pitch == pl->M ? IMPL_BULK : IMPL_PLAIN; }
 static PassImpl y_impl(const fft3d_plan_t* pl) {
+    if (pl->nat_pitch != pl->M) return IMPL_PLAIN;         // rows of M+1 fp32 complex are not 16-byte aligned: no TMA
     if (use_tma(pl) && pl->split_y && pl->variant != 2) return IMPL_TMA_SPLIT2;
     return use_tma(pl) && pl->tma_y ? IMPL_TMA : IMPL_PLAIN;
 }
@@ -781,6 +786,7 @@ static int stage_fwd_zy(const fft3d_plan_t* pl, const void* d_in, void* scratch,
     const KernelSet* kz = pl->kz;
     ZArgs z{};
     z.in = d_in; z.out = scratch; z.tw = pl->tw_z; z.twz = pl->twz; z.nrows = Nxp * Ny; z.scale = 1.0;
+    z.in_pitch = z.out_pitch = pl->nat_pitch;
     if (z_impl(pl) == IMPL_BULK) rc = launch_zbulk(pl, 0, d_in, scratch, 1.0, st);
     else rc = launch(kz->z_fn[0], (z.nrows + kz->z_rpb - 1) / kz->z_rpb, pl->grid_z[0], kz->z_threads, kz->z_smem, &z, st);
     if (rc != FFT3D_OK) return rc;
@@ -804,7 +810,7 @@ static int stage_fwd_zy(const fft3d_plan_t* pl, const void* d_in, void* scratch,
         a.out = reinterpret_cast<unsigned char*>(slab) + (size_t)pl->xp0 * L * M * 2 * pl->esize;
         a.ntz = (int)((M + ky->tc - 1) / ky->tc); a.ncols = (int)M; a.a_lo = 1; a.L = (int)L;
         a.ntiles = Nxp * a.ntz;
-        a.in_hi = Ny * M; a.in_lo = 0; a.in_rq = 0; a.in_rl = M;
+        a.in_hi = Ny * pl->nat_pitch; a.in_lo = 0; a.in_rq = 0; a.in_rl = pl->nat_pitch;
         a.out_hi = L * M; a.out_lo = 0; a.out_rq = pl->sNx * L * M; a.out_rl = M;
         rc = launch(ky->s_fn[0][KIND_LIN_SLAB], a.ntiles, pl->grid_y[0], ky->s_threads, ky->s_smem, &a, st);
     }
@@ -921,7 +927,7 @@ static int stage_inv_yz(const fft3d_plan_t* pl, const void* slab, void* scratch,
         a.ntz = (int)((M + ky->tc - 1) / ky->tc); a.ncols = (int)M; a.a_lo = 1; a.L = (int)L;
         a.ntiles = Nxp * a.ntz;
         a.in_hi = L * M; a.in_lo = 0; a.in_rq = pl->sNx * L * M; a.in_rl = M;
-        a.out_hi = Ny * M; a.out_lo = 0; a.out_rq = 0; a.out_rl = M;
+        a.out_hi = Ny * pl->nat_pitch; a.out_lo = 0; a.out_rq = 0; a.out_rl = pl->nat_pitch;
         rc = launch(ky->s_fn[1][KIND_SLAB_LIN], a.ntiles, pl->grid_y[1], ky->s_threads, ky->s_smem, &a, st);
     }
     if (rc != FFT3D_OK) return rc;
@@ -931,6 +937,7 @@ static int stage_inv_yz(const fft3d_plan_t* pl, const void* slab, void* scratch,
     const KernelSet* kz = pl->kz;
     ZArgs z{};
     z.in = scratch; z.out = d_out; z.tw = pl->tw_z; z.twz = pl->twz; z.nrows = Nxp * Ny;
+    z.in_pitch = z.out_pitch = pl->nat_pitch;
     z.scale = 1.0 / ((double)pl->Nx * (double)Ny * (double)pl->Nz);
     if (z_impl(pl) == IMPL_BULK) rc = launch_zbulk(pl, 1, scratch, d_out, z.scale, st);
     else rc = launch(kz->z_fn[1], (z.nrows + kz->z_rpb - 1) / kz->z_rpb, pl->grid_z[1], kz->z_threads, kz->z_smem, &z, st);
@@ -946,7 +953,7 @@ static unsigned* ws_flags(const fft3d_plan_t* pl, void* d_work) {
 }
 
 int fft3d_r2c(const fft3d_plan_t* pl, const void* d_in, void* d_out, void* d_work, void* stream) {
-    if (pl == nullptr || pl->kind != 0 || pl->dist_G != 0 || d_in == nullptr || d_out == nullptr || d_work == nullptr) return FFT3D_EINVAL;
+    if (pl == nullptr || pl->kind != 0 || pl->dist_G != 0 || pl->inplace || d_in == nullptr || d_out == nullptr || d_work == nullptr) return FFT3D_EINVAL;
     const size_t rb = fft3d_real_bytes(pl), cb = fft3d_complex_bytes(pl), wb = fft3d_workspace_bytes(pl);
     if (((uintptr_t)d_in | (uintptr_t)d_out | (uintptr_t)d_work) & 15) return FFT3D_EINVAL;
     if (overlap(d_in, rb, d_out, cb) || overlap(d_in, rb, d_work, wb) || overlap(d_out, cb, d_work, wb))
@@ -969,7 +976,7 @@ int fft3d_r2c(const fft3d_plan_t* pl, const void* d_in, void* d_out, void* d_wor
 }
 
 int fft3d_c2r(const fft3d_plan_t* pl, const void* d_in, void* d_out, void* d_work, void* stream) {
-    if (pl == nullptr || pl->kind != 0 || pl->dist_G != 0 || d_in == nullptr || d_out == nullptr || d_work == nullptr) return FFT3D_EINVAL;
+    if (pl == nullptr || pl->kind != 0 || pl->dist_G != 0 || pl->inplace || d_in == nullptr || d_out == nullptr || d_work == nullptr) return FFT3D_EINVAL;
     const size_t rb = fft3d_real_bytes(pl), cb = fft3d_complex_bytes(pl), wb = fft3d_workspace_bytes(pl);
     if (((uintptr_t)d_in | (uintptr_t)d_out | (uintptr_t)d_work) & 15) return FFT3D_EINVAL;
     if (overlap(d_in, cb, d_out, rb) || overlap(d_in, cb, d_work, wb) || overlap(d_out, rb, d_work, wb))
@@ -992,6 +999,65 @@ int fft3d_c2r(const fft3d_plan_t* pl, const void* d_in, void* d_out, void* d_wor
     int rc = stage_inv_x(pl, d_in, side, slab, st, rec, slot);
     if (rc != FFT3D_OK) return rc;
     return stage_inv_yz(pl, slab, d_work, d_out, ws_ring(pl, d_work), ws_flags(pl, d_work), st, rec, slot);
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// Padded in-place layout ("each GPU now contains Nx/p x Ny x (Nz/2+1) data points", i.e.
+// FFTW-style rows of 2*(Nz/2+1) reals): the real field and its half spectrum share ONE buffer, with the single
+// workspace beside it.  Rows of Nz/2+1 fp32 complex start on 8-byte boundaries, which neither bulk copies
+// nor tensor maps can address, so the passes that touch this layout -- z (in place, row by row) and the natural
+// side of y -- run the plain-load kernels; the x pass and the slab side keep the TMA kernels.
+//   forward : z R2C in place (pitch M+1) -> y C2C: data -> slab array in the workspace -> x C2C: workspace -> data
+//   inverse : x C2C: data -> workspace -> y C2C: workspace -> data (pitch M+1) -> z C2R in place
+// ---------------------------------------------------------------------------------------------------------
+int fft3d_plan_inplace(fft3d_plan_t** out, long long Nx, long long Ny, long long Nz, int dtype, int virtual_slabs) {
+    int rc = plan_create(out, Nx, Ny, Nz, dtype, virtual_slabs, 0);
+    if (rc != FFT3D_OK) return rc;
+    fft3d_plan_t* pl = *out;
+    pl->inplace = 1;
+    pl->nat_pitch = pl->M + 1;
+    pl->fused = pl->fused_default = false;
+    pl->ring_bytes = 0;
+    pl->flags_bytes = 0;
+    pl->side_bytes = ((size_t)Nx * Ny * 2 * pl->esize + 255) & ~(size_t)255;      // packed column of the inverse
+    return FFT3D_OK;
+}
+
+int fft3d_r2c_inplace(const fft3d_plan_t* pl, void* d_data, void* d_work, void* stream) {
+    if (pl == nullptr || !pl->inplace || d_data == nullptr || d_work == nullptr) return FFT3D_EINVAL;
+    if (((uintptr_t)d_data | (uintptr_t)d_work) & 15) return FFT3D_EINVAL;
+    if (overlap(d_data, fft3d_complex_bytes(pl), d_work, fft3d_workspace_bytes(pl))) return FFT3D_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    Recorder rec(pl, 0, st);
+    int slot = 0;
+    rec.mark(slot++);
+    int rc = stage_fwd_zy(pl, d_data, d_data, d_work, nullptr, nullptr, st, rec, slot);
+    if (rc != FFT3D_OK) return rc;
+    rc = stage_fwd_x(pl, d_work, d_data, st, rec, slot);
+    if (rc != FFT3D_OK) return rc;
+    PlaneArgs f{};
+    f.src = nullptr; f.dst = d_data; f.Nx = (int)pl->Nx; f.Ny = (int)pl->Ny; f.L = (int)pl->L; f.M = (int)pl->M;
+    if (launch_unpack_nyquist(pl->dtype, f, st) != cudaSuccess) { cudaGetLastError(); return FFT3D_ECUDA; }
+    rec.mark(slot++);
+    return FFT3D_OK;
+}
+
+int fft3d_c2r_inplace(const fft3d_plan_t* pl, void* d_data, void* d_work, void* stream) {
+    if (pl == nullptr || !pl->inplace || d_data == nullptr || d_work == nullptr) return FFT3D_EINVAL;
+    if (((uintptr_t)d_data | (uintptr_t)d_work) & 15) return FFT3D_EINVAL;
+    if (overlap(d_data, fft3d_complex_bytes(pl), d_work, fft3d_workspace_bytes(pl))) return FFT3D_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    Recorder rec(pl, 1, st);
+    int slot = 0;
+    rec.mark(slot++);
+    void* side = reinterpret_cast<unsigned char*>(d_work) + pl->slab_bytes;       // behind the slab array
+    PlaneArgs f{};
+    f.src = d_data; f.dst = side; f.Nx = (int)pl->Nx; f.Ny = (int)pl->Ny; f.L = (int)pl->L; f.M = (int)pl->M;
+    if (launch_pack_nyquist(pl->dtype, f, st) != cudaSuccess) { cudaGetLastError(); return FFT3D_ECUDA; }
+    rec.mark(slot++);
+    int rc = stage_inv_x(pl, d_data, side, d_work, st, rec, slot);
+    if (rc != FFT3D_OK) return rc;
+    return stage_inv_yz(pl, d_work, d_data, d_data, nullptr, nullptr, st, rec, slot);
 }
 
 // ---------------------------------------------------------------------------------------------------------

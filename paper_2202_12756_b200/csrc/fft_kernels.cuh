@@ -47,6 +47,8 @@ struct ZArgs {
     const void* twz;             // exp(-2 pi i k / Nz), k < M
     long long nrows;
     double scale;                // C2R only: 1/(Nx Ny Nz)
+    long long in_pitch, out_pitch;   // complex elements between consecutive rows (0 = M, dense); M+1 for the padded
+                                     // in-place layout (rows of Nz+2 reals), where in == out is allowed
 };
 
 // row padding of shared-memory tiles: one extra row every PADR rows (0 = none)
@@ -501,8 +503,8 @@ __global__ void __launch_bounds__(Cfg::S * RPB, MINB) fft_z_r2c_kernel(const ZAr
         const long long row = g * RPB + rr;
         const bool ok = row < a.nrows;
         // a row of Nz reals read as M (even, odd) pairs: z[m] = x[2m] + i x[2m+1]
-        const C* in = reinterpret_cast<const C*>(a.in) + row * M;
-        C* out = reinterpret_cast<C*>(a.out) + row * M;
+        const C* in = reinterpret_cast<const C*>(a.in) + row * (a.in_pitch ? a.in_pitch : M);
+        C* out = reinterpret_cast<C*>(a.out) + row * (a.out_pitch ? a.out_pitch : M);
         C v[P];
 #pragma unroll
         for (int m = 0; m < P; ++m) v[m] = ok ? in[t + m * S] : mk<T>((T)0, (T)0);
@@ -549,8 +551,8 @@ __global__ void __launch_bounds__(Cfg::S * RPB, MINB) fft_z_c2r_kernel(const ZAr
     for (long long g = blockIdx.x; g < ngroups; g += gridDim.x) {
         const long long row = g * RPB + rr;
         const bool ok = row < a.nrows;
-        const C* in = reinterpret_cast<const C*>(a.in) + row * M;
-        C* out = reinterpret_cast<C*>(a.out) + row * M;
+        const C* in = reinterpret_cast<const C*>(a.in) + row * (a.in_pitch ? a.in_pitch : M);
+        C* out = reinterpret_cast<C*>(a.out) + row * (a.out_pitch ? a.out_pitch : M);
         C v[P];
 #pragma unroll
         for (int m = 0; m < P; ++m) v[m] = ok ? in[t + m * S] : mk<T>((T)0, (T)0);

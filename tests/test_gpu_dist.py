@@ -113,3 +113,51 @@ def test_dist_argument_errors(fft):
     mono = fft.Plan(64, 64, 64, dtype=torch.float32, virtual_slabs=4)
     assert lib.fft3d_dist_fwd_x(mono._h, x.data_ptr(), x.data_ptr(), None) == 1
     p.close(); mono.close()
+
+
+_NCCL_ONE_RANK = r'''
+import os, sys
+sys.path.insert(0, %(root)r)
+os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=%(port)r, WORLD_SIZE="1", RANK="0", LOCAL_RANK="0")
+import torch, torch.distributed as dist
+import paper_2202_12756_b200 as pkg
+from paper_2202_12756_b200 import dist as D, inputs
+torch.cuda.set_device(0)
+dist.init_process_group("nccl", device_id=torch.device("cuda", 0))
+shape = (128, 256, 256)
+f = inputs.uniform_grid(shape, torch.float32, seed=3, device="cuda")
+mono = pkg.Plan(*shape, dtype=torch.float32, virtual_slabs=1)
+ref = mono.r2c(f)
+for exchange in ("chunks", "unified"):
+    fft = D.SlabFFT.create(*shape, torch.float32, dist, torch.device("cuda", 0), exchange=exchange)
+    fft.timed = True
+    spec = fft.plan.empty_spec_part("cuda")
+    back = fft.plan.empty_real_slab("cuda")
+    fft.forward(f, spec)
+    fft.inverse(spec, back)
+    torch.cuda.synchronize()
+    fft.collect_times()
+    assert torch.equal(torch.view_as_real(spec.reshape(-1)), torch.view_as_real(ref)), exchange
+    assert torch.equal(back, mono.c2r(ref)), exchange
+    assert fft.times["comp"] > 0.0
+    fft.close()
+dist.destroy_process_group()
+print("OK")
+'''
+
+
+def test_slab_fft_over_nccl_one_rank(fft):
+    """SlabFFT's GPU code path (NCCL all-to-all / all-gather calls, VMM exchange, phase events) with a one-rank
+    group: what a one-GPU box can run of the multi-process driver."""
+    import os
+    import socket
+    import subprocess
+    import sys
+    s = socket.socket()
+    s.bind(("127.0.0.1", 0))
+    port = str(s.getsockname()[1])
+    s.close()
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    res = subprocess.run([sys.executable, "-c", _NCCL_ONE_RANK % {"root": root, "port": port}],
+                         capture_output=True, text=True, timeout=600)
+    assert res.returncode == 0 and "OK" in res.stdout, res.stderr[-3000:]
