@@ -83,7 +83,8 @@ enum {
 int fft3d_plan(fft3d_plan_t **out, long long Nx, long long Ny, long long Nz,
                int dtype, int virtual_slabs);
 
-/* 1 if this build has a C2C kernel of length n (n = 2^a in 4..4096, 3*2^a in 6..3072 or 5*2^a in 20..1280), else 0. */
+/* 1 if this build has a C2C kernel of length n (n = 2^a in 4..4096, 3*2^a in 6..3072, 5*2^a in 20..1280
+ * or 7*2^a in 28..1792), else 0. */
 int fft3d_supported_length(long long n);
 
 /* Sizes in bytes.  Workspace: the single work buffer shared by R2C and C2R (opt. 1):

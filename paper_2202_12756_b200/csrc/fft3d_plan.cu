@@ -1440,7 +1440,7 @@ const char* fft3d_strerror(int status) {
     switch (status) {
         case FFT3D_OK: return "ok";
         case FFT3D_EINVAL: return "invalid argument (extents, virtual_slabs, dtype, pointers or aliasing)";
-        case FFT3D_EUNSUPPORTED: return "unsupported extent (need Nz even; Nx, Ny, Nz/2 of the form 2^a, 3*2^a or 5*2^a within the built range)";
+        case FFT3D_EUNSUPPORTED: return "unsupported extent (need Nz even; Nx, Ny, Nz/2 of the form 2^a, 3*2^a, 5*2^a or 7*2^a within the built range)";
         case FFT3D_ENOMEM: return "out of memory";
         case FFT3D_ECUDA: return "CUDA error (no device, or a launch/runtime failure)";
         case FFT3D_EWORKSPACE: return "workspace too small or misaligned";

@@ -1,16 +1,17 @@
 // fft_configs.cuh -- which FFT lengths this build has kernels for, and how each is factored.
 //
 // CfgFor<T, N>::type = FftCfg<N, P, r0, r1, ...>: P points per thread, stage radices r_i (each
-// dividing P).  Lengths are 2^a (4..4096), 3*2^a (6..3072) and 5*2^a (20..1280): every extent in
+// dividing P).  Lengths are 2^a (4..4096), 3*2^a (6..3072), 5*2^a (20..1280) and 7*2^a (28..1792): every extent in
 // BASELINE.json's configs (64, 256, 1024, 1536 = 3*2^9, 2048) and their halves for the z pass, plus the radix-5
-// family of SURVEY.md 8(f)-4.
+// and radix-7 families of SURVEY.md 8(f)-4.
 #pragma once
 #include "fft_core.cuh"
 
 #define FFT3D_FOREACH_N(X) \
     X(4) X(8) X(16) X(32) X(64) X(128) X(256) X(512) X(1024) X(2048) X(4096) \
     X(6) X(12) X(24) X(48) X(96) X(192) X(384) X(768) X(1536) X(3072) \
-    X(20) X(40) X(80) X(160) X(320) X(640) X(1280)
+    X(20) X(40) X(80) X(160) X(320) X(640) X(1280) \
+    X(28) X(56) X(112) X(224) X(448) X(896) X(1792)
 
 namespace fft3d {
 
@@ -51,6 +52,15 @@ FFT3D_CFG(float, 320, 20, 20, 4, 4)
 FFT3D_CFG(float, 640, 20, 20, 4, 4, 2)
 FFT3D_CFG(float, 1280, 20, 20, 4, 4, 4)
 
+// 7*2^a (radix-7 leaf in fft_radix.cuh)
+FFT3D_CFG(float, 28, 28, 28)
+FFT3D_CFG(float, 56, 28, 28, 2)
+FFT3D_CFG(float, 112, 28, 28, 4)
+FFT3D_CFG(float, 224, 28, 28, 4, 2)
+FFT3D_CFG(float, 448, 28, 28, 4, 4)
+FFT3D_CFG(float, 896, 28, 28, 4, 4, 2)
+FFT3D_CFG(float, 1792, 28, 28, 4, 4, 4)
+
 // fp64: registers are twice as wide, so fewer points per thread
 FFT3D_CFG(double, 4, 4, 4)
 FFT3D_CFG(double, 8, 8, 8)
@@ -81,6 +91,14 @@ FFT3D_CFG(double, 160, 20, 20, 4, 2)
 FFT3D_CFG(double, 320, 20, 20, 4, 4)
 FFT3D_CFG(double, 640, 20, 20, 4, 4, 2)
 FFT3D_CFG(double, 1280, 20, 20, 4, 4, 4)
+
+FFT3D_CFG(double, 28, 28, 28)
+FFT3D_CFG(double, 56, 28, 28, 2)
+FFT3D_CFG(double, 112, 28, 28, 4)
+FFT3D_CFG(double, 224, 28, 28, 4, 2)
+FFT3D_CFG(double, 448, 28, 28, 4, 4)
+FFT3D_CFG(double, 896, 28, 28, 4, 4, 2)
+FFT3D_CFG(double, 1792, 28, 28, 4, 4, 4)
 
 // Factorisation used by the bulk-pipelined z kernels (fft_zpass.cuh): the strided-pass one unless
 // a shape with fewer exchanges fits a row's threads inside one warp.

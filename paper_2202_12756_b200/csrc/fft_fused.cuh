@@ -12,7 +12,7 @@
 // does fit the 126 MB L2 many times over.  So the kernel is a persistent dataflow pipeline over
 // ALL SMs, one CTA per SM, each CTA with a fixed ROLE: "z CTAs" transform z tiles (RPT whole rows),
 // "y CTAs" transform y tiles (TC columns of a plane).  Planes are handled in order; the tiles of a
-// role are dealt round-robin to the CTAs of that role.  The "phase-1" role (forward: z, inverse: y)
+// role are dealt in order to the CTAs of that role.  The "phase-1" role (forward: z, inverse: y)
 // writes its result into ring slot x % R, the "phase-2" role reads it from
 // there as soon as the plane is complete -- so the ring lives in L2 (written with an evict_last
 // policy; the streaming input and output use evict_first) and HBM sees ONE read and ONE write of
@@ -27,17 +27,23 @@
 //
 // Why roles: the two tile bodies are ~35 KB of straight-line code each and the two SMs of a TPC
 // share an instruction cache; with both bodies alive in one TPC 60 % of the issue stalls in the
-// FFT code were instruction fetches (ncu, profiles/).  Roles follow %smid so that a TPC never mixes; ranks inside a
-// role come from an atomic ticket (no assumption about the ids), and every spin on a global counter is bounded.
+// FFT code were instruction fetches (ncu, profiles/).  Roles follow %smid so that a TPC never mixes.  The tiles of a
+// role are dealt DYNAMICALLY, in order, by an atomic counter per role (a CTA draws its next tile when a ring slot of
+// its own is about to become free): no assumption about the SM ids, and a CTA that runs slower than its peers simply
+// takes fewer tiles instead of holding every plane back (measured: forward 2.87 -> 2.74 ms at 1024^3).  Every spin
+// on a global counter is bounded.
 //
 // Ordering between CTAs uses two counters per plane in global memory (zeroed before the launch):
 //   p1_done[x]    += 1 when a phase-1 tile of plane x has been stored (store complete, released at once)
 //   p2_loaded[x]  += 1 when a phase-2 tile of plane x has landed in shared memory
 // A phase-2 load of plane x waits for p1_done[x] == N1; a phase-1 store of plane x waits for
 // p2_loaded[x-R] == N2 (the ring slot has been read out).  Phase-2 CTAs never wait on anything a
-// later plane produces and phase-1 CTAs only on phase-2 loads R planes back, every CTA handles its
-// tiles in plane order, so with all CTAs co-resident (cooperative launch, one CTA per SM) the
-// pipeline cannot deadlock.
+// later plane produces and phase-1 CTAs only on phase-2 loads R planes back; tiles are drawn in plane
+// order and every CTA handles its tiles in the order it drew them, so with all CTAs co-resident
+// (cooperative launch) the pipeline cannot deadlock: the lowest unfinished tile of either role is
+// always held by a CTA whose earlier tiles depend on lower planes only.
+// End of work: a load warp that draws a tile index past the end posts NSTAGE "end items" (index -1) through the
+// same barriers, so that every consumer group and every store warp sees one and leaves.
 //
 // Inside a CTA: a load warp, one store warp per ring slot (one elected lane each) and NG consumer groups
 // that own alternate tiles and transform them IN PLACE in an NSTAGE-deep shared-memory ring, with
@@ -105,6 +111,9 @@ __device__ __forceinline__ unsigned ld_acquire(const unsigned* p) {
 __device__ __forceinline__ void red_release_add(unsigned* p, unsigned v) {
     asm volatile("red.release.gpu.global.add.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
 }
+__device__ __forceinline__ void red_relaxed_add(unsigned* p, unsigned v) {
+    asm volatile("red.relaxed.gpu.global.add.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
 // Spin on a global counter, bounded: ~1 us per poll, 2^24 polls > 10 s.  A pipeline that cannot make progress
 // traps -- the host then sees a launch failure and the API returns FFT3D_ECUDA -- instead of hanging the device.
 __device__ __forceinline__ void wait_count(const unsigned* p, unsigned target) {
@@ -135,12 +144,25 @@ struct FusedTile {
         return n > 4 ? 4 : n;
     }
     static constexpr int THREADS = threads(max_stages());
+    // Register re-allocation between the warp groups (setmaxnreg): the kernel is launched with REGS_LAUNCH registers
+    // per thread (what __launch_bounds__(THREADS, 1) allows); the producer warp group (load warp + three store warps)
+    // keeps REGS_PROD and the consumer warp groups take what that frees.  Only where the producers are exactly one
+    // warp group and the consumers whole warp groups.
+    static constexpr int NCONS_ALL = NG * GROUP;
+    static constexpr int REGS_LAUNCH = ((65536 / THREADS) / 8) * 8;
+    static constexpr int REGS_PROD = 32;
+    static constexpr int REGS_CONS_RAW = (((REGS_LAUNCH * THREADS - 128 * REGS_PROD) / NCONS_ALL) / 8) * 8;
+    static constexpr int REGS_CONS = REGS_CONS_RAW > 232 ? 232 : REGS_CONS_RAW;
+    static constexpr bool REALLOC = (NCONS_ALL % 128 == 0) && (THREADS - NCONS_ALL == 128) && THREADS >= 384 &&
+                                    REGS_LAUNCH <= 248 && REGS_CONS > REGS_LAUNCH;
 };
 
 // words of the control block that follows the 2*Nx plane counters in the flags area (zeroed before the launch)
-enum { FZ_CTL_NZ = 0, FZ_CTL_NY = 1, FZ_CTL_ARRIVED = 2, FZ_CTL_WORDS = 8 };
+enum { FZ_CTL_NZ = 0, FZ_CTL_NY = 1, FZ_CTL_ARRIVED = 2, FZ_CTL_NEXT_Z = 3, FZ_CTL_NEXT_Y = 4, FZ_CTL_WORDS = 8 };
 
 struct FItem { int p1, x, j; };
+struct TrueT { static constexpr bool value = true; };
+struct FalseT { static constexpr bool value = false; };
 
 // C2C = true: the rows are Nz complex numbers and the z tiles run the plain C2C transform (3D C2C plans)
 template <class ZCfg, int RPT, class YCfg, int TC, int DIR, typename T, int NSTAGE, int NG_, bool C2C = false>
@@ -169,7 +191,8 @@ fft_zy_fused_kernel(const __grid_constant__ TensorMapBlob ring_map, const __grid
     // the groups in turn (NSTAGE need not be a multiple of NG) and a parity wait is only meaningful
     // within one phase of the barrier's current one, so a group polls seen[s] before it waits for ITS phase.
     volatile int* seen = reinterpret_cast<volatile int*>(empty + NSTAGE);
-    volatile int* role_s = seen + NSTAGE;                // [role_z, rank, nrole] broadcast from thread 0
+    volatile int* role_s = seen + NSTAGE;                // [role_z] broadcast from thread 0
+    volatile int* item_q = role_s + 4;                   // [s] global tile index in slot s (-1: no more tiles), [NSTAGE] first end item, [NSTAGE+1+s] its plane
 
     const int tid = threadIdx.x;
     if (tid == NCONS) {
@@ -177,6 +200,7 @@ fft_zy_fused_kernel(const __grid_constant__ TensorMapBlob ring_map, const __grid
             tma::mbar_init(&full[s], 1); tma::mbar_init(&done[s], GROUP / 32); tma::mbar_init(&empty[s], 1);
             seen[s] = 0;
         }
+        item_q[NSTAGE] = -1;
         tma::fence_mbar_init();
     }
     if (tid < NCONS) {
@@ -190,8 +214,8 @@ fft_zy_fused_kernel(const __grid_constant__ TensorMapBlob ring_map, const __grid
     // Role of this CTA: z tiles or y tiles, never both -- the two bodies are ~35 KB of straight-line code each,
     // and the SMs of a TPC share an instruction cache, so both SMs of a TPC get the same role: SMs [0, kz) take
     // the z tiles (kz even), the rest the y tiles; kz = 0: CTA pairs (4k, 4k+1) -> z, (4k+2, 4k+3) -> y.
-    // Nothing is assumed about %smid being dense or about one CTA per SM: every CTA draws its rank inside its
-    // role from an atomic ticket and learns the role sizes after a grid-wide arrival counter (cooperative launch:
+    // Nothing is assumed about %smid being dense or about one CTA per SM: the tiles of a role are dealt by an
+    // atomic counter (below), and the role sizes are checked after a grid-wide arrival counter (cooperative launch:
     // all CTAs are co-resident).  If a role came out empty, all CTAs fall back to alternating by blockIdx.
     unsigned* ctl = a.flags + 2 * a.Nx;
     if (tid == 0) {
@@ -199,21 +223,16 @@ fft_zy_fused_kernel(const __grid_constant__ TensorMapBlob ring_map, const __grid
         asm("mov.u32 %0, %%smid;" : "=r"(smid));
         const int b = blockIdx.x, G = gridDim.x;
         int rz = (a.kz > 0 && a.kz < G) ? ((int)smid < a.kz) : !((b >> 1) & 1);
-        int rk = (int)atomicAdd(&ctl[rz ? FZ_CTL_NZ : FZ_CTL_NY], 1u);
+        atomicAdd(&ctl[rz ? FZ_CTL_NZ : FZ_CTL_NY], 1u);
         __threadfence();
         tma::red_release_add(&ctl[FZ_CTL_ARRIVED], 1u);
         tma::wait_count(&ctl[FZ_CTL_ARRIVED], (unsigned)G);
         const int nz = (int)tma::ld_acquire(&ctl[FZ_CTL_NZ]), ny = (int)tma::ld_acquire(&ctl[FZ_CTL_NY]);
-        int nr = rz ? nz : ny;
-        if (nz == 0 || ny == 0) {
-            rz = !(b & 1);
-            rk = b >> 1;
-            nr = rz ? (G + 1) / 2 : G / 2;
-        }
-        role_s[0] = rz; role_s[1] = rk; role_s[2] = nr;
+        if (nz == 0 || ny == 0) rz = !(b & 1);
+        role_s[0] = rz;
     }
     __syncthreads();
-    const int role_z = role_s[0], rank = role_s[1], nrole = role_s[2];
+    const int role_z = role_s[0];
     const int my_p1 = FWD ? role_z : !role_z;            // this CTA's tiles are the phase-1 tiles
     const int nper = role_z ? n_z : n_y;                 // tiles per plane of this role
     const int total = a.Nx * nper;
@@ -222,15 +241,26 @@ fft_zy_fused_kernel(const __grid_constant__ TensorMapBlob ring_map, const __grid
     const long long plane_bytes = (long long)a.Ny * M * (long long)sizeof(C);
 
     if (tid >= NCONS) {
+        if constexpr (FT::REALLOC) asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(FT::REGS_PROD));
         if (tid == NCONS) {
             // ------------------------- load warp -------------------------
             const unsigned long long pol_stream = tma::policy_evict_first(), pol_keep = tma::policy_evict_last();
             int i = 0, ready = -1;                       // planes <= ready are known to be complete in the ring
-            for (int g = rank; g < total; g += nrole) {
-                FItem it; it.p1 = my_p1; it.x = g / nper; it.j = g - it.x * nper;
+            unsigned* next = &ctl[role_z ? FZ_CTL_NEXT_Z : FZ_CTL_NEXT_Y];
+            int g = (int)atomicAdd(next, 1u);            // the next tile of this role, in order
+            for (;;) {
                 const int s = i % NSTAGE, n = i / NSTAGE;
                 unsigned char* dst = stages + s * FT::STAGE_BYTES;
                 if (n > 0) tma::mbar_wait(&empty[s], (unsigned)((n - 1) & 1));
+                if (g >= total) {                        // NSTAGE end items: every group and every store warp sees one
+                    if (item_q[NSTAGE] < 0) item_q[NSTAGE] = i;
+                    item_q[s] = -1;
+                    tma::mbar_arrive(&full[s]);
+                    if (++i >= item_q[NSTAGE] + NSTAGE) break;
+                    continue;
+                }
+                FItem it; it.p1 = my_p1; it.x = g / nper; it.j = g - it.x * nper;
+                item_q[s] = g; item_q[NSTAGE + 1 + s] = it.x;
                 if (!it.p1 && it.x > ready) {
                     tma::wait_count(&p1_done[it.x], (unsigned)n1);
                     tma::fence_proxy_async_all();
@@ -266,18 +296,20 @@ fft_zy_fused_kernel(const __grid_constant__ TensorMapBlob ring_map, const __grid
                     }
                 }
                 ++i;
+                g = (int)atomicAdd(next, 1u);            // drawn ahead: its latency hides behind the wait for the slot
             }
         } else if ((tid & 31) == 0) {
             // ------------------------- store warp of ring slot my_s -------------------------
             const int my_s = (tid - NCONS) / 32 - 1;
             const unsigned long long pol_stream = tma::policy_evict_first(), pol_keep = tma::policy_evict_last();
-            int i = 0, freed = -1;
-            for (int g = rank; g < total; g += nrole) {
-                FItem it; it.p1 = my_p1; it.x = g / nper; it.j = g - it.x * nper;
-                const int s = i % NSTAGE, n = i / NSTAGE;
-                if (s != my_s) { ++i; continue; }
+            int freed = -1;
+            for (int i = my_s;; i += NSTAGE) {
+                const int s = my_s, n = i / NSTAGE;
                 const unsigned char* src = stages + s * FT::STAGE_BYTES;
                 tma::mbar_wait(&done[s], (unsigned)(n & 1));
+                const int g = item_q[s];
+                if (g < 0) break;
+                FItem it; it.p1 = my_p1; it.x = g / nper; it.j = g - it.x * nper;
                 if (it.p1 && it.x >= a.R && it.x - a.R > freed) {          // ring slot must have been read out
                     tma::wait_count(&p2_loaded[it.x - a.R], (unsigned)n2);
                     freed = it.x - a.R;
@@ -319,7 +351,6 @@ fft_zy_fused_kernel(const __grid_constant__ TensorMapBlob ring_map, const __grid
                     tma::fence_proxy_async_all();
                     tma::red_release_add(&p1_done[it.x], 1u);
                 }
-                ++i;
             }
             tma::store_wait_all();
         }
@@ -327,79 +358,93 @@ fft_zy_fused_kernel(const __grid_constant__ TensorMapBlob ring_map, const __grid
     }
 
     // ---------------- consumers: group gq takes the CTA's items gq, gq+NG, ... ----------------
+    if constexpr (FT::REALLOC) asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(FT::REGS_CONS));
     const int gq = tid / GROUP, gt = tid % GROUP;
     const GroupSync sync{1 + gq, GROUP};
-    // z-tile role: thread tz of row rr
-    const int tz = gt % ZCfg::S, rr = gt / ZCfg::S;
-    const SmLayout<1, 0> z_dense{rr * M};
-    const SmLayout<1, ZT::PADR> z_padded{rr * ZT::PITCH};
-    C* scr = scratch + gq * (RPT * ZCfg::P) + rr * ZCfg::P;
-    C wt = mk<T>((T)1, (T)0);                            // exp(-2 pi i t/Nz), conjugated for the inverse
-    if constexpr (!C2C) {
-        wt = reinterpret_cast<const C*>(a.twz)[tz];
-        if constexpr (DIR > 0) wt.y = -wt.y;
-    }
-    const T scale = (T)a.scale;
-    // y-tile role: thread ty of column cc
-    const int cc = gt % TC, ty = gt / TC;
-    const SmLayout<TC, 0> y_dense{cc};
-    const SmLayout<TC, YT::PADR> y_padded{cc};
-
-    int i = 0;
-    for (int g = rank; g < total; g += nrole) {
-        FItem it; it.p1 = my_p1; it.x = g / nper; it.j = g - it.x * nper;
-        const int mine = (i % NG) == gq;
-        const int s = i % NSTAGE, n = i / NSTAGE;
-        ++i;
-        if (!mine) continue;
-        C* buf = reinterpret_cast<C*>(stages + s * FT::STAGE_BYTES);
-        while (seen[s] < n) { }                          // the previous phase of this slot has been observed
-        tma::mbar_wait(&full[s], (unsigned)(n & 1));
-        if (gt == 0) seen[s] = n + 1;
-        if (!it.p1 && gt == 0) tma::red_release_add(&p2_loaded[it.x], 1u);   // the ring tile has been read
-        const bool isz = FWD ? it.p1 : !it.p1;
-        if (isz) {
-            constexpr int P = ZCfg::P;
-            C v[P];
-            read_own<ZCfg, T>(v, buf, tz, z_dense);
-            if constexpr (DIR > 0 && !C2C) {
-                if (tz == 0) {
-#pragma unroll
-                    for (int m = 0; m < P; ++m) scr[m] = v[m];
-                }
-                __syncwarp();
-                hermitian_step<ZCfg, true, T>(v, wt, tz, scr);
-                __syncwarp();
-            }
-            if constexpr (ZCfg::NST > 1) sync();
-            fft_stages<ZCfg, 0, DIR, T>(v, buf, twz_s, tz, z_padded, sync);
-            if constexpr (DIR < 0 && !C2C) {
-                if (tz == 0) {
-#pragma unroll
-                    for (int m = 0; m < P; ++m) scr[m] = v[m];
-                }
-                __syncwarp();
-                hermitian_step<ZCfg, false, T>(v, wt, tz, scr);
-                __syncwarp();
-            } else if constexpr (DIR > 0) {
-#pragma unroll
-                for (int m = 0; m < P; ++m) v[m] = mk<T>(v[m].x * scale, v[m].y * scale);
-            }
-            if constexpr (ZCfg::NST > 1) sync();
-            write_own<ZCfg, T>(v, buf, tz, z_dense);
-        } else {
-            constexpr int P = YCfg::P;
-            C v[P];
-            read_own<YCfg, T>(v, buf, ty, y_dense);
-            if constexpr (YCfg::NST > 1) sync();
-            fft_stages<YCfg, 0, DIR, T>(v, buf, twy_s, ty, y_padded, sync);
-            if constexpr (YCfg::NST > 1) sync();
-            write_own<YCfg, T>(v, buf, ty, y_dense);
+    // one loop per role (the role is fixed for the CTA's lifetime): only that role's invariants stay in registers
+    auto consume = [&](auto zrole) {
+        constexpr bool ISZ = decltype(zrole)::value;
+        constexpr bool P1 = FWD ? ISZ : !ISZ;
+        // z-tile role: thread tz of row rr;  y-tile role: thread ty of column cc
+        const int tz = gt % ZCfg::S, rr = gt / ZCfg::S;
+        const int cc = gt % TC, ty = gt / TC;
+        const SmLayout<1, 0> z_dense{rr * M};
+        const SmLayout<1, ZT::PADR> z_padded{rr * ZT::PITCH};
+        const SmLayout<TC, 0> y_dense{cc};
+        const SmLayout<TC, YT::PADR> y_padded{cc};
+        C* scr = scratch + gq * (RPT * ZCfg::P) + rr * ZCfg::P;
+        C wt = mk<T>((T)1, (T)0);                        // exp(-2 pi i t/Nz), conjugated for the inverse
+        if constexpr (ISZ && !C2C) {
+            wt = reinterpret_cast<const C*>(a.twz)[tz];
+            if constexpr (DIR > 0) wt.y = -wt.y;
         }
-        tma::fence_proxy_async();
-        __syncwarp();
-        if ((tid & 31) == 0) tma::mbar_arrive(&done[s]);
-    }
+        const T scale = (T)a.scale;
+        for (int i = gq;; i += NG) {
+            const int s = i % NSTAGE, n = i / NSTAGE;
+            C* buf = reinterpret_cast<C*>(stages + s * FT::STAGE_BYTES);
+            while (seen[s] < n) { }                      // the previous phase of this slot has been observed
+            tma::mbar_wait(&full[s], (unsigned)(n & 1));
+            const int g = item_q[s];
+            if (g < 0) {                                 // end item: pass it on to the slot's store warp
+                if (gt == 0) seen[s] = n + 1;
+                __syncwarp();
+                if ((tid & 31) == 0) tma::mbar_arrive(&done[s]);
+                if (i + NG >= item_q[NSTAGE] + NSTAGE) break;
+                continue;
+            }
+            // (kept free of branches: a lane that leaves its warp here would stay apart for the whole tile body,
+            //  and the body's warp shuffles then take the slow path for diverged warps)
+            if (gt == 0) seen[s] = n + 1;
+            if constexpr (!P1) {
+                // the ring tile has landed in shared memory (complete_tx observed): nothing of it can be read any
+                // later, so a relaxed increment is enough to let the ring slot be overwritten
+                if (gt == 0) tma::red_relaxed_add(&p2_loaded[item_q[NSTAGE + 1 + s]], 1u);
+            }
+            __syncwarp();
+            if constexpr (ISZ) {
+                constexpr int P = ZCfg::P;
+                C v[P];
+                read_own<ZCfg, T>(v, buf, tz, z_dense);
+                if constexpr (DIR > 0 && !C2C) {
+                    if (tz == 0) {
+#pragma unroll
+                        for (int m = 0; m < P; ++m) scr[m] = v[m];
+                    }
+                    __syncwarp();
+                    hermitian_step<ZCfg, true, T>(v, wt, tz, scr);
+                    __syncwarp();
+                }
+                if constexpr (ZCfg::NST > 1) sync();
+                fft_stages<ZCfg, 0, DIR, T>(v, buf, twz_s, tz, z_padded, sync);
+                if constexpr (DIR < 0 && !C2C) {
+                    if (tz == 0) {
+#pragma unroll
+                        for (int m = 0; m < P; ++m) scr[m] = v[m];
+                    }
+                    __syncwarp();
+                    hermitian_step<ZCfg, false, T>(v, wt, tz, scr);
+                    __syncwarp();
+                } else if constexpr (DIR > 0) {
+#pragma unroll
+                    for (int m = 0; m < P; ++m) v[m] = cscale(v[m], scale);
+                }
+                if constexpr (ZCfg::NST > 1) sync();
+                write_own<ZCfg, T>(v, buf, tz, z_dense);
+            } else {
+                constexpr int P = YCfg::P;
+                C v[P];
+                read_own<YCfg, T>(v, buf, ty, y_dense);
+                if constexpr (YCfg::NST > 1) sync();
+                fft_stages<YCfg, 0, DIR, T>(v, buf, twy_s, ty, y_padded, sync);
+                if constexpr (YCfg::NST > 1) sync();
+                write_own<YCfg, T>(v, buf, ty, y_dense);
+            }
+            tma::fence_proxy_async();
+            __syncwarp();
+            if ((tid & 31) == 0) tma::mbar_arrive(&done[s]);
+        }
+    };
+    if (role_z) consume(TrueT{}); else consume(FalseT{});
 }
 
 }  // namespace fft3d

@@ -1,5 +1,5 @@
 // fft_radix.cuh -- register-level building blocks: complex helpers, compile-time twiddles and a
-// fully unrolled in-register DFT of any length R = 2^a * 3^b * 5^c (R <= 48 used).
+// fully unrolled in-register DFT of any length R = 2^a * 3^b * 5^c * 7^d (R <= 48 used).
 //
 // The transform implemented is the 1D DFT of Eq. (1)/(2) of the paper:
 //   X[k] = sum_j x[j] exp(DIR * 2 pi i j k / R),  DIR = -1 forward, +1 inverse (unnormalised).
@@ -21,6 +21,20 @@ template <typename C> __device__ __forceinline__ C cmul(C a, C b) {
     C r; r.x = a.x * b.x - a.y * b.y; r.y = a.x * b.y + a.y * b.x; return r;
 }
 template <typename C> __device__ __forceinline__ C cconj(C a) { C r; r.x = a.x; r.y = -a.y; return r; }
+// fp32: Blackwell's packed f32x2 arithmetic (FADD2 / FMUL2 / FFMA2: one issue slot per complex operation; the
+// swap / broadcast / per-half negation of the operands are free operand modifiers in SASS)
+#ifdef __CUDA_ARCH__
+__device__ __forceinline__ float2 cadd(float2 a, float2 b) { return __fadd2_rn(a, b); }
+__device__ __forceinline__ float2 csub(float2 a, float2 b) { return __fadd2_rn(a, make_float2(-b.x, -b.y)); }
+__device__ __forceinline__ float2 cmul(float2 a, float2 w) {
+    const float2 t = __fmul2_rn(w, make_float2(a.x, a.x));
+    return __ffma2_rn(make_float2(-w.y, w.x), make_float2(a.y, a.y), t);
+}
+#endif
+template <typename C, typename T> __device__ __forceinline__ C cscale(C a, T s) { C r; r.x = a.x * s; r.y = a.y * s; return r; }
+#ifdef __CUDA_ARCH__
+__device__ __forceinline__ float2 cscale(float2 a, float s) { return __fmul2_rn(a, make_float2(s, s)); }
+#endif
 // multiply by s*i, s = +1 or -1 (compile time)
 template <int S, typename C> __device__ __forceinline__ C cmul_i(C a) {
     C r;
@@ -67,7 +81,7 @@ constexpr cs cossin(long long num, long long den) {
 }  // namespace ct
 
 // a * exp(DIR * 2 pi i NUM / DEN) with the trivial rotations done without multiplications.
-template <int NUM, int DEN, int DIR, typename T>
+template <int NUM, int DEN, int DIR, typename T, bool PACK = true>
 __device__ __forceinline__ cx<T> mul_root(cx<T> a) {
     constexpr int n = ((NUM % DEN) + DEN) % DEN;
     if constexpr (n == 0) {
@@ -82,10 +96,18 @@ __device__ __forceinline__ cx<T> mul_root(cx<T> a) {
         constexpr ct::cs w = ct::cossin(n, DEN);
         constexpr T c = (T)w.c;
         constexpr T s = (T)(DIR > 0 ? w.s : -w.s);
-        cx<T> r;
-        r.x = a.x * c - a.y * s;
-        r.y = a.x * s + a.y * c;
-        return r;
+#ifdef __CUDA_ARCH__
+        if constexpr (sizeof(T) == 4 && PACK) {
+            const float2 t = __fmul2_rn(a, make_float2(c, c));
+            return __ffma2_rn(make_float2(-a.y, a.x), make_float2(s, s), t);
+        } else
+#endif
+        {
+            cx<T> r;
+            r.x = a.x * c - a.y * s;
+            r.y = a.x * s + a.y * c;
+            return r;
+        }
     }
 }
 
@@ -159,10 +181,34 @@ __device__ __forceinline__ void dft(cx<T> (&v)[R]) {
         v[4] = csub(a1, b1);
         v[2] = cadd(a2, b2);
         v[3] = csub(a2, b2);
+    } else if constexpr (R == 7) {
+        // X_k = x0 + sum_{j=1..3} [ s_j cos(2 pi jk/7) + DIR i d_j sin(2 pi jk/7) ],  s_j = x_j + x_{7-j}, d_j = x_j - x_{7-j};
+        // X_{7-k} is the same with the sign of the second term flipped
+        constexpr T c1 = (T)0.62348980185873353052500488400423981;    // cos(2 pi/7)
+        constexpr T c2 = (T)-0.22252093395631440428890256449679476;   // cos(4 pi/7)
+        constexpr T c3 = (T)-0.90096886790241912623610231950744505;   // cos(6 pi/7)
+        constexpr T k1 = (T)0.78183148246802980870844452667405775;    // sin(2 pi/7)
+        constexpr T k2 = (T)0.97492791218182360701813168299393122;    // sin(4 pi/7)
+        constexpr T k3 = (T)0.43388373911755812047576833284835875;    // sin(6 pi/7)
+        const C s1 = cadd(v[1], v[6]), s2 = cadd(v[2], v[5]), s3 = cadd(v[3], v[4]);
+        const C d1 = csub(v[1], v[6]), d2 = csub(v[2], v[5]), d3 = csub(v[3], v[4]);
+        const C a1 = mk<T>(v[0].x + c1 * s1.x + c2 * s2.x + c3 * s3.x, v[0].y + c1 * s1.y + c2 * s2.y + c3 * s3.y);
+        const C a2 = mk<T>(v[0].x + c2 * s1.x + c3 * s2.x + c1 * s3.x, v[0].y + c2 * s1.y + c3 * s2.y + c1 * s3.y);
+        const C a3 = mk<T>(v[0].x + c3 * s1.x + c1 * s2.x + c2 * s3.x, v[0].y + c3 * s1.y + c1 * s2.y + c2 * s3.y);
+        const C b1 = cmul_i<DIR>(mk<T>(k1 * d1.x + k2 * d2.x + k3 * d3.x, k1 * d1.y + k2 * d2.y + k3 * d3.y));
+        const C b2 = cmul_i<DIR>(mk<T>(k2 * d1.x - k3 * d2.x - k1 * d3.x, k2 * d1.y - k3 * d2.y - k1 * d3.y));
+        const C b3 = cmul_i<DIR>(mk<T>(k3 * d1.x - k1 * d2.x + k2 * d3.x, k3 * d1.y - k1 * d2.y + k2 * d3.y));
+        v[0] = mk<T>(v[0].x + s1.x + s2.x + s3.x, v[0].y + s1.y + s2.y + s3.y);
+        v[1] = cadd(a1, b1);
+        v[6] = csub(a1, b1);
+        v[2] = cadd(a2, b2);
+        v[5] = csub(a2, b2);
+        v[3] = cadd(a3, b3);
+        v[4] = csub(a3, b3);
     } else {
-        constexpr int R1 = (R % 4 == 0) ? 4 : ((R % 2 == 0) ? 2 : ((R % 3 == 0) ? 3 : 5));
+        constexpr int R1 = (R % 4 == 0) ? 4 : ((R % 2 == 0) ? 2 : ((R % 3 == 0) ? 3 : ((R % 5 == 0) ? 5 : 7)));
         constexpr int R2 = R / R1;
-        static_assert(R1 * R2 == R, "radix must be 2^a 3^b 5^c");
+        static_assert(R1 * R2 == R, "radix must be 2^a 3^b 5^c 7^d");
         C sub[R1][R2];
 #pragma unroll
         for (int q = 0; q < R1; ++q)

@@ -91,20 +91,20 @@ __device__ __forceinline__ double2 shfl_cx<double>(double2 v, int src, int width
 }
 
 // R2C:  X[k] = (Z[k] + conj Z[M-k])/2 - (i/2) w^k (Z[k] - conj Z[M-k]),  w = exp(-2 pi i/Nz)
+// (scalar arithmetic on purpose, here and in the per-thread rotations of w: the operands come out of warp shuffles
+//  word by word; the packed f32x2 forms of fft_radix.cuh cost register moves here and were slower, measured)
 template <typename T>
 __device__ __forceinline__ cx<T> herm_post(cx<T> z, cx<T> zp, cx<T> w) {
-    const cx<T> zm = cconj(zp);
-    const cx<T> e = cadd(z, zm), d = csub(z, zm);
-    const cx<T> wd = cmul(w, d);
-    return mk<T>((T)0.5 * (e.x + wd.y), (T)0.5 * (e.y - wd.x));
+    const T ex = z.x + zp.x, ey = z.y - zp.y, dx = z.x - zp.x, dy = z.y + zp.y;
+    const T wdx = w.x * dx - w.y * dy, wdy = w.x * dy + w.y * dx;
+    return mk<T>((T)0.5 * (ex + wdy), (T)0.5 * (ey - wdx));
 }
 // C2R:  Z[k] = (X[k] + conj X[M-k]) + i conj(w)^k (X[k] - conj X[M-k])
 template <typename T>
 __device__ __forceinline__ cx<T> herm_pre(cx<T> x, cx<T> xp, cx<T> wc) {
-    const cx<T> xm = cconj(xp);
-    const cx<T> e = cadd(x, xm), d = csub(x, xm);
-    const cx<T> wd = cmul(wc, d);
-    return mk<T>(e.x - wd.y, e.y + wd.x);
+    const T ex = x.x + xp.x, ey = x.y - xp.y, dx = x.x - xp.x, dy = x.y + xp.y;
+    const T wdx = wc.x * dx - wc.y * dy, wdy = wc.x * dy + wc.y * dx;
+    return mk<T>(ex - wdy, ey + wdx);
 }
 
 // The Hermitian step on the thread's P values, in place, pair (m, P-1-m) at a time.
@@ -125,8 +125,8 @@ __device__ __forceinline__ void hermitian_step(cx<T> (&v)[Cfg::P], cx<T> wt, int
             pb = scr[P - m2];
         }
         // w^(t + m S) = wt * exp(-+2 pi i m/(2P))
-        const C wa = mul_root<m, 2 * P, INV ? +1 : -1, T>(wt);
-        const C wb = mul_root<m2, 2 * P, INV ? +1 : -1, T>(wt);
+        const C wa = mul_root<m, 2 * P, INV ? +1 : -1, T, false>(wt);
+        const C wb = mul_root<m2, 2 * P, INV ? +1 : -1, T, false>(wt);
         if constexpr (!INV) {
             C ra = herm_post<T>(a, pa, wa);
             if constexpr (m == 0) { if (t == 0) ra = mk<T>(a.x + a.y, a.x - a.y); }   // (X[0], X[Nz/2]) packed

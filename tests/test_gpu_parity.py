@@ -66,6 +66,11 @@ SMALL = [
     ((20, 20, 40), 1),
     ((320, 160, 80), 8),
     ((80, 40, 1280), 4),        # 640-point rows through the bulk z kernel
+    ((56, 112, 224), 4),        # 7*2^a lengths on every axis (radix-7 leaf; z half: 112)
+    ((28, 28, 56), 1),
+    ((448, 224, 112), 8),
+    ((112, 56, 1792), 4),       # 896-point rows
+    ((1792, 16, 56), 4),        # Nx = 1792
     ((64, 192, 64), 32),        # L = 6: the two-class shifted windows (four classes need L % 4 == 0)
     ((2048, 8, 32), 2),         # Nx = 2048: inverse x pass as four 512-point quarter tiles + a radix-4 combine
     ((2048, 16, 64), 4),
@@ -259,7 +264,7 @@ def test_argument_errors(fft):
         fft.Plan(64, 64, 64, virtual_slabs=3)
     assert e.value.status == 1
     with pytest.raises(fft.Fft3dError) as e:
-        fft.Plan(56, 64, 64)                       # 56 = 7*8: no radix 7
+        fft.Plan(44, 64, 64)                       # 44 = 11*4: no radix 11
     assert e.value.status == 2
     plan = fft.Plan(16, 16, 16, dtype=torch.float32)
     x = plan.empty_real()

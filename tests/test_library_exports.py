@@ -35,7 +35,7 @@ def test_every_declared_symbol_is_exported(lib):
 
 def test_host_only_calls(lib):
     import paper_2202_12756_b200 as m
-    for n in (4, 64, 256, 1024, 1536, 2048, 768, 3072, 4096, 20, 640, 1280):
+    for n in (4, 64, 256, 1024, 1536, 2048, 768, 3072, 4096, 20, 640, 1280, 28, 896, 1792):
         assert m.supported_length(n)
     for n in (1, 5, 7, 1000, 8192, 9):
         assert not m.supported_length(n)
@@ -51,7 +51,7 @@ def test_plan_validation_needs_no_gpu(lib):
     assert lib.fft3d_plan(ctypes.byref(h), 64, 64, 64, 0, 3) == 1        # p does not divide
     assert lib.fft3d_plan(ctypes.byref(h), 64, 64, 64, 5, 1) == 1        # bad dtype
     assert lib.fft3d_plan(ctypes.byref(h), 1, 64, 64, 0, 1) == 1         # extent < 2
-    assert lib.fft3d_plan(ctypes.byref(h), 56, 64, 64, 0, 1) == 2        # 56 = 7*8 unsupported (no radix 7)
+    assert lib.fft3d_plan(ctypes.byref(h), 44, 64, 64, 0, 1) == 2        # 44 = 11*4 unsupported (no radix 11)
     assert lib.fft3d_plan(None, 64, 64, 64, 0, 1) == 1
 
 
