@@ -113,9 +113,9 @@ int fft3d_c2r(const fft3d_plan_t *plan, const void *d_cplx_in, void *d_real_out,
 
 /* 3D complex-to-complex transform (in the paper's library R2C, C2C and C2R share one
  * workspace).  fft3d_plan_c2c creates a plan for an Nx x Ny x Nz COMPLEX grid over p virtual
- * x-slabs: same requirements as fft3d_plan except that Nz may be odd-free of the "even" rule but must
- * itself be a supported length >= 128 (fp32) / 64 (fp64) whose row kernel exists, and Nx*Ny must be a
- * multiple of its tile (<= 32 rows); otherwise FFT3D_EUNSUPPORTED.  For such a plan
+ * x-slabs: same requirements as fft3d_plan except that Nz need not be even: Nx, Ny and Nz must be supported
+ * lengths, p | Nx, p | Ny.  Rows of >= 1 KiB in whole tiles run the bulk-pipelined row kernel, all others a
+ * plain-load one (fft3d_launch_impl says which).  For such a plan
  * fft3d_complex_bytes = Nx*Ny*Nz complex (input, output), fft3d_workspace_bytes the same,
  * fft3d_real_bytes = 0, fft3d_index(kx,ky,kz) = ((q*Nx + kx)*(Ny/p) + ky % (Ny/p))*Nz + kz.
  * fft3d_c2c: direction -1 = forward, unnormalised, d_in natural [Nx][Ny][Nz] -> d_out in the slab layout

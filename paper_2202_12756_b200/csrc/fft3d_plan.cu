@@ -83,6 +83,8 @@ struct fft3d_plan_s {
     void* tw_zb;                        // stage twiddles of the bulk-pipelined z kernels
     int num_sms;
     int grid_z[2], grid_y[2], grid_x[2];   // persistent grid sizes [fwd, inv]
+    int grid_zp[2];                        // C2C plans: the plain-load row kernels
+    bool bulk_zc;                          // C2C plans: the bulk-pipelined row kernel can run (whole tiles of long rows)
     // buffers of the host-pointer entry points (lazy)
     void *h_real, *h_cplx, *h_work;
     cudaStream_t h_stream;
@@ -469,8 +471,6 @@ static int plan_create(fft3d_plan_t** out, long long Nx, long long Ny, long long
     const KernelSet* ky = find_kernels(Ny, dtype);
     const KernelSet* kx = find_kernels(Nx, dtype);
     if (kz == nullptr || ky == nullptr || kx == nullptr) return FFT3D_EUNSUPPORTED;
-    // C2C plans: the row pass exists only as the bulk-pipelined kernel (whole tiles of zc_rpt rows)
-    if (kind == 1 && (kz->zc_fn[0] == nullptr || (Nx * Ny) % kz->zc_rpt != 0)) return FFT3D_EUNSUPPORTED;
 
     int dev = 0, sms = 0;
     if (cudaGetDevice(&dev) != cudaSuccess ||
@@ -494,11 +494,18 @@ static int plan_create(fft3d_plan_t** out, long long Nx, long long Ny, long long
     if (rc == FFT3D_OK && kind == 0) rc = upload_z_twiddles(Nz, pl->M, pl->esize, &pl->twz);
     if (rc == FFT3D_OK && kind == 1) {
         pl->x_rows = (int)largest_divisor_le(Nx, 256);
-        rc = upload_stage_twiddles(kz->zc_nst, kz->zc_radix, kz->zc_twn, pl->esize, &pl->tw_zc);
-        for (int d = 0; d < 2 && rc == FFT3D_OK; ++d) {
-            int g = 0;
-            rc = prepare_kernel(kz->zc_fn[d], kz->zc_threads, kz->zc_smem, sms, &g);
+        // rows of >= 1 KiB in whole tiles go through the bulk-pipelined row kernel, everything else (and variant 1)
+        // through the plain-load one
+        pl->bulk_zc = kz->zc_fn[0] != nullptr && (Nx * Ny) % kz->zc_rpt == 0;
+        if (pl->bulk_zc) {
+            rc = upload_stage_twiddles(kz->zc_nst, kz->zc_radix, kz->zc_twn, pl->esize, &pl->tw_zc);
+            for (int d = 0; d < 2 && rc == FFT3D_OK; ++d) {
+                int g = 0;
+                rc = prepare_kernel(kz->zc_fn[d], kz->zc_threads, kz->zc_smem, sms, &g);
+            }
         }
+        for (int d = 0; d < 2 && rc == FFT3D_OK; ++d)
+            rc = prepare_kernel(kz->zp_fn[d], kz->z_threads, kz->z_smem, sms, &pl->grid_zp[d]);
     }
     for (int d = 0; d < 2 && rc == FFT3D_OK; ++d) {
         rc = prepare_kernel(kz->z_fn[d], kz->z_threads, kz->z_smem, sms, &pl->grid_z[d]);
@@ -617,7 +624,7 @@ static int plan_create(fft3d_plan_t** out, long long Nx, long long Ny, long long
     }
     // C2C plans: the same fused pipeline over rows of Nz complex points (Nz == Ny)
     if (rc == FFT3D_OK && kind == 1 && pl->tma_y && ky->fc_fn[0] != nullptr && Nz == Ny && ky->fc_tc == ky->tma_tc &&
-        Ny % ky->fc_rpt == 0 && pl->M % ky->fc_tc == 0 && pl->M / ky->fc_tc <= 256 && kz->zc_fn[0] != nullptr) {
+        Ny % ky->fc_rpt == 0 && pl->M % ky->fc_tc == 0 && pl->M / ky->fc_tc <= 256 && pl->bulk_zc) {
         const size_t plane = (size_t)Ny * pl->M * 2 * pl->esize;
         int R = (int)(((size_t)48 << 20) / plane);
         if (R > 8) R = 8;
@@ -737,7 +744,7 @@ const char* fft3d_launch_impl(const fft3d_plan_t* pl, int which, int i) {
     PassImpl im = IMPL_FIXUP;
     if (std::strstr(nm, "fused") != nullptr) im = IMPL_FUSED;
     else if (std::strcmp(nm, "x_c2c_inv_col0") == 0) im = IMPL_PLAIN;
-    else if (nm[0] == 'z') im = pl->kind == 1 ? IMPL_BULK : z_impl(pl);
+    else if (nm[0] == 'z') im = pl->kind == 1 ? (use_tma(pl) && pl->bulk_zc ? IMPL_BULK : IMPL_PLAIN) : z_impl(pl);
     else if (nm[0] == 'y') im = y_impl(pl);
     else if (nm[0] == 'x') im = x_impl(pl, which);
     return names[im];
@@ -1223,6 +1230,12 @@ int fft3d_c2c(const fft3d_plan_t* pl, const void* d_in, void* d_out, void* d_wor
     rec.mark(slot++);
 
     auto z_pass = [&](const void* in, void* out) -> int {
+        if (!(use_tma(pl) && pl->bulk_zc)) {            // plain-load rows: any length, any row count
+            ZArgs zp{};
+            zp.in = in; zp.out = out; zp.tw = pl->tw_z; zp.twz = nullptr; zp.nrows = Nx * Ny;
+            zp.scale = 1.0 / ((double)Nx * (double)Ny * (double)pl->Nz);
+            return launch(kz->zp_fn[d], (zp.nrows + kz->z_rpb - 1) / kz->z_rpb, pl->grid_zp[d], kz->z_threads, kz->z_smem, &zp, st);
+        }
         ZBulkArgs z{};
         z.in = in; z.out = out; z.tw = pl->tw_zc; z.twz = nullptr;
         z.ntiles = Nx * Ny / kz->zc_rpt;

@@ -167,6 +167,8 @@ static KernelSet make_set(int dtype) {
     k.z_smem = Z_SMEM;
     k.z_fn[0] = (const void*)fft_z_r2c_kernel<Cfg, RPB, T, Z_MINB>;
     k.z_fn[1] = (const void*)fft_z_c2r_kernel<Cfg, RPB, T, Z_MINB>;
+    k.zp_fn[0] = (const void*)fft_z_c2c_kernel<Cfg, RPB, -1, T, Z_MINB>;
+    k.zp_fn[1] = (const void*)fft_z_c2c_kernel<Cfg, RPB, +1, T, Z_MINB>;
     constexpr int TTC = tma_tile_cols(Cfg::N, Cfg::S, (int)sizeof(C));
     if constexpr (TTC > 0) {
         // complex fp32 rows of the user's spectrum (M+1 entries) start on 8-byte boundaries for odd l:

@@ -583,4 +583,39 @@ __global__ void __launch_bounds__(Cfg::S * RPB, MINB) fft_z_c2r_kernel(const ZAr
     }
 }
 
+// Plain-load C2C row kernel: rows of N complex numbers, forward or inverse (scaled) -- the z pass of 3D C2C plans
+// whose rows are too short, or whose row count is not a whole number of tiles, for the bulk-pipelined kernel
+// (P:81).  Same thread mapping and exchange buffer as the R2C / C2R kernels above.
+template <class Cfg, int RPB, int DIR, typename T, int MINB>
+__global__ void __launch_bounds__(Cfg::S * RPB, MINB) fft_z_c2c_kernel(const ZArgs a) {
+    using C = cx<T>;
+    constexpr int P = Cfg::P, S = Cfg::S, N = Cfg::N;
+    using Pad = RowPad<Cfg>;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    C* tw = reinterpret_cast<C*>(smem_raw);
+    C* rows = tw + ((Cfg::TWN + 1) & ~1) + N;            // same carve as the R2C kernel (its twz table is unused here)
+    load_twiddles<DIR, T>(tw, reinterpret_cast<const C*>(a.tw), Cfg::TWN, threadIdx.x, blockDim.x);
+
+    const int t = threadIdx.x % S, rr = threadIdx.x / S;
+    const SmLayout<1, Pad::PADR> lay{rr * Pad::PITCH};
+    const long long ngroups = (a.nrows + RPB - 1) / RPB;
+    const T scale = (T)a.scale;
+
+    for (long long g = blockIdx.x; g < ngroups; g += gridDim.x) {
+        const long long row = g * RPB + rr;
+        const bool ok = row < a.nrows;
+        const C* in = reinterpret_cast<const C*>(a.in) + row * (a.in_pitch ? a.in_pitch : N);
+        C* out = reinterpret_cast<C*>(a.out) + row * (a.out_pitch ? a.out_pitch : N);
+        C v[P];
+#pragma unroll
+        for (int m = 0; m < P; ++m) v[m] = ok ? in[t + m * S] : mk<T>((T)0, (T)0);
+        __syncthreads();                               // tables loaded / previous group's exchange fully read
+        fft_stages<Cfg, 0, DIR, T>(v, rows, tw, t, lay, CtaSync{});
+        if (ok) {
+#pragma unroll
+            for (int m = 0; m < P; ++m) out[t + m * S] = DIR > 0 ? mk<T>(v[m].x * scale, v[m].y * scale) : v[m];
+        }
+    }
+}
+
 }  // namespace fft3d

@@ -23,6 +23,7 @@ struct KernelSet {
     int z_threads;
     size_t z_smem;
     const void* z_fn[2];       // [0 = R2C, 1 = C2R]
+    const void* zp_fn[2];      // plain-load C2C row kernels [0 = forward, 1 = inverse (scaled)]: same launch shape
     // TMA-pipelined strided kernels (null if not compiled for this length)
     const void* tma_fn[4];     // [TMA_Y_FWD, TMA_Y_INV, TMA_X_FWD, TMA_X_INV]
     int tma_tc;                // tile columns of the Y passes

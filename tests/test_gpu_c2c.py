@@ -36,6 +36,12 @@ CASES = [
     ((128, 128, 128), 8),
     ((32, 256, 1024), 16),       # 64 KiB row tiles; y pass through the TMA kernels
     ((8, 64, 1536), 1),          # rows whose threads span two warps (no Hermitian step, so allowed)
+    ((32, 32, 16), 2),           # rows shorter than 1 KiB: the plain-load row kernel
+    ((16, 24, 64), 4),
+    ((12, 20, 28), 2),           # radix 3, 5 and 7 lengths, Nz not a multiple of the bulk tile
+    ((6, 10, 40), 2),
+    ((64, 64, 96), 8),
+    ((10, 6, 1024), 2),          # long rows, but Nx*Ny = 60 is not a whole number of 8-row tiles: plain rows
 ]
 
 
@@ -103,8 +109,13 @@ def test_plan_kinds_do_not_mix(fft):
     assert lib.fft3d_r2c(c._h, x.data_ptr(), x.data_ptr(), w.data_ptr(), None) == 1      # FFT3D_EINVAL
     assert lib.fft3d_c2c(c._h, x.data_ptr(), x.data_ptr(), w.data_ptr(), -1, None) == 1  # in == out rejected
     assert lib.fft3d_c2c(c._h, x.data_ptr(), w.data_ptr(), w.data_ptr(), 0, None) == 1   # bad direction
-    with pytest.raises(fft.Fft3dError):
-        fft.PlanC2C(32, 32, 16, dtype=torch.float32, virtual_slabs=2)                     # rows too short: unsupported
+    with pytest.raises(fft.Fft3dError) as e:
+        fft.PlanC2C(32, 32, 44, dtype=torch.float32, virtual_slabs=2)                     # 44 = 11*4: no kernel
+    assert e.value.status == 2
+    short = fft.PlanC2C(32, 32, 16, dtype=torch.float32, virtual_slabs=2)                 # short rows: plain-load rows
+    assert short.launch_impls(0)[0] == "plain" and short.launch_impls(1)[-1] == "plain"
+    assert c.launch_impls(0)[0] == "bulk"
+    short.close()
     c.close(); r.close()
 
 
