@@ -23,4 +23,9 @@ from .slab_layout import (  # noqa: F401
     natural_to_slab,
     slab_to_natural,
     simulate_paper_steps_2_to_4,
+    pencil_cz,
+    pencil_index,
+    natural_to_pencil,
+    pencil_to_natural,
+    simulate_pencil_transposes,
 )

@@ -235,3 +235,31 @@ def test_paper_steps_2_to_4_compose_to_slab_index(oracle_mod, shape, p):
     # x-stride of step 5: Ny/p * (Nz/2+1)
     if Nx > 1:
         assert off[1, 0, 0] - off[0, 0, 0] == (Ny // p) * Nzh
+
+
+# ---------------------------------------------------------------- the pencil layout (reading R17)
+@pytest.mark.parametrize("shape", [(8, 8, 8), (8, 16, 12), (16, 8, 16)])
+@pytest.mark.parametrize("px,py", [(1, 1), (2, 1), (1, 2), (2, 2), (4, 2), (2, 4), (8, 2)])
+def test_pencil_transposes_compose_to_pencil_index(oracle_mod, shape, px, py):
+    Nx, Ny, Nz = shape
+    Nzh = Nz // 2 + 1
+    if Nx % px or Ny % px or Ny % py or (Nz // 2) % py:
+        pytest.skip("extents not divisible by the rank grid")
+    D1 = np.arange(Nx * Ny * Nzh, dtype=np.float64).reshape(Nx, Ny, Nzh)     # every element carries its identity
+    sim = oracle_mod.simulate_pencil_transposes(D1, px, py)
+    kx, ky, kz = np.meshgrid(np.arange(Nx), np.arange(Ny), np.arange(Nzh), indexing="ij")
+    off = oracle_mod.pencil_index(px, py, Nx, Ny, Nz, kx, ky, kz)
+    assert sorted(off.ravel().tolist()) == list(range(Nx * Ny * Nzh))       # a bijection
+    assert np.array_equal(sim[off], D1)
+    assert np.array_equal(sim, oracle_mod.natural_to_pencil(D1, px, py))
+    assert np.array_equal(oracle_mod.pencil_to_natural(sim, shape, px, py), D1)
+    # py = 1 is the slab layout with p = px (the paper's own decomposition)
+    if py == 1:
+        assert np.array_equal(off, oracle_mod.slab_index(px, Nx, Ny, Nz, kx, ky, kz))
+    # inside a rank x is the slowest index with stride (Ny/px) * cz_b, y next with stride cz_b
+    cz0 = int(oracle_mod.pencil_cz(py, Nz, 0))
+    assert off[1, 0, 0] - off[0, 0, 0] == (Ny // px) * cz0
+    if Ny // px > 1:
+        assert off[0, 1, 0] - off[0, 0, 0] == cz0
+    # the last rank column also holds the Nyquist column
+    assert int(oracle_mod.pencil_cz(py, Nz, py - 1)) == (Nz // 2) // py + 1
