@@ -142,6 +142,20 @@ int fft3d_plan_inplace(fft3d_plan_t **plan_out, long long Nx, long long Ny, long
 int fft3d_r2c_inplace(const fft3d_plan_t *plan, void *d_data, void *d_work, void *cuda_stream);
 int fft3d_c2r_inplace(const fft3d_plan_t *plan, void *d_data, void *d_work, void *cuda_stream);
 
+/* Pencil layout (p = px x py ranks, each holding (Nx/px) x (Ny/py) x Nz real points --
+ * the paper describes this decomposition and does not build it; reading R17 in D:3 fixes the layout).  A second VIRTUAL
+ * layout of the same transform: fft3d_r2c leaves the half spectrum as a px x py rank grid would hold it after the
+ * standard two-exchange scheme, rank (a, b) owning
+ *     F[kx][ky_l][kz_l],  ky = a*Ny/px + ky_l,  kz = b*Nz/(2 py) + kz_l,      [Nx][Ny/px][cz_b]
+ * with cz_b = Nz/(2 py) columns, the last rank column b = py-1 also holding the Nyquist column kz = Nz/2 (cz = Nz/(2 py)+1);
+ * x is the slowest index inside a rank (stride (Ny/px)*cz_b) and the ranks are concatenated in the order
+ * r = a*py + b.  fft3d_index() returns that offset; py = 1 is the slab layout with virtual_slabs = px.  fft3d_c2r takes
+ * the same layout back.  Requirements: those of fft3d_plan with p = px, and py | Ny, py | Nz/2, py <= 64.
+ * Implementation: the slab transform with p = px, its rows cut into the py column ranges by one more pass over the
+ * spectrum ("pencil_split" / "pencil_merge" in fft3d_launch_name); the slab-layout spectrum is staged in the workspace,
+ * so fft3d_workspace_bytes() is larger by fft3d_complex_bytes().  Sizes and all other calls as for fft3d_plan. */
+int fft3d_plan_pencil(fft3d_plan_t **plan_out, long long Nx, long long Ny, long long Nz, int dtype, int px, int py);
+
 /* ---- Slab decomposition over G GPUs, one process and one plan per GPU -------------------------
  * This is the paper's method itself (P:54 slabs along x; P:67-77 steps 1-5; P:86 inverse), with its exchange fused
  * into the y pass.  Rank r of G owns
@@ -217,7 +231,7 @@ int fft3d_c2r_host(fft3d_plan_t *plan, const void *h_cplx_in, void *h_real_out);
 
 /* Number of kernels one fft3d_r2c (which = 0) or fft3d_c2r (which = 1) call launches, and the
  * name of launch i (a static string; NULL if i is out of range).  Names: "z_r2c", "y_c2c_fwd",
- * "x_c2c_fwd", "nyquist_unpack", "nyquist_pack", "x_c2c_inv", "x_c2c_inv_col0" (the packed
+ * "x_c2c_fwd", "nyquist_unpack", "pencil_split", "pencil_merge" (pencil-layout plans), "nyquist_pack", "x_c2c_inv", "x_c2c_inv_col0" (the packed
  * column 0 of the inverse x pass, TMA path only), "y_c2c_inv", "z_c2r", and -- when the z and y
  * passes of a plane run as one kernel through an L2-resident ring --
  * "zy_r2c_fused" (paper step 1 + steps 2-4) and "yz_c2r_fused" (their reverse); C2C plans:

@@ -4,4 +4,4 @@ The compute path is ``libfft3d.so`` (hand-written sm_100a CUDA behind the C ABI 
 ``include/fft3d.h``); ``binding`` marshals torch tensors into it.  ``inputs`` holds the seeded
 synthetic workloads and none of the method's arithmetic.
 """
-from .binding import F32, F64, Fft3dError, Plan, PlanC2C, PlanInplace, load_library, strerror, supported_length  # noqa: F401
+from .binding import F32, F64, Fft3dError, Plan, PlanC2C, PlanInplace, PlanPencil, load_library, strerror, supported_length  # noqa: F401

@@ -22,7 +22,7 @@ EXPORTS = (
     "fft3d_c2r_host", "fft3d_launches", "fft3d_launch_name", "fft3d_set_variant", "fft3d_destroy", "fft3d_strerror",
     "fft3d_timing_enable", "fft3d_timing_read", "fft3d_plan_c2c", "fft3d_c2c", "fft3d_c2c_host",
     "fft3d_launch_impl", "fft3d_set_option",
-    "fft3d_plan_inplace", "fft3d_r2c_inplace", "fft3d_c2r_inplace",
+    "fft3d_plan_inplace", "fft3d_r2c_inplace", "fft3d_c2r_inplace", "fft3d_plan_pencil",
     "fft3d_plan_dist", "fft3d_dist_bytes", "fft3d_dist_fwd_local", "fft3d_dist_fwd_x", "fft3d_dist_fwd_col0",
     "fft3d_dist_fwd_unpack", "fft3d_dist_inv_planes", "fft3d_dist_inv_pack", "fft3d_dist_inv_x", "fft3d_dist_inv_local",
     "fft3d_vmm_granularity", "fft3d_vmm_create", "fft3d_vmm_import", "fft3d_vmm_map", "fft3d_vmm_unmap", "fft3d_vmm_release",
@@ -52,6 +52,8 @@ def load_library() -> ctypes.CDLL:
     lib.fft3d_plan.restype = i
     lib.fft3d_plan_c2c.argtypes = [ctypes.POINTER(vp), ll, ll, ll, i, i]
     lib.fft3d_plan_c2c.restype = i
+    lib.fft3d_plan_pencil.argtypes = [ctypes.POINTER(vp), ll, ll, ll, i, i, i]
+    lib.fft3d_plan_pencil.restype = i
     lib.fft3d_c2c.argtypes = [vp, vp, vp, vp, i, vp]
     lib.fft3d_c2c.restype = i
     lib.fft3d_c2c_host.argtypes = [vp, vp, vp, i]
@@ -305,6 +307,53 @@ class Plan:
             self.close()
         except Exception:
             pass
+
+
+class PlanPencil(Plan):
+    """fft3d_plan_pencil(Nx, Ny, Nz, dtype, px, py): the spectrum laid out as a px x py rank grid would hold it."""
+
+    def __init__(self, Nx: int, Ny: int, Nz: int, dtype=torch.float32, px: int = 1, py: int = 1):
+        lib = load_library()
+        self.dtype_code = {torch.float32: F32, torch.float64: F64}[dtype]
+        self.shape = (int(Nx), int(Ny), int(Nz))
+        self.p, self.px, self.py = int(px), int(px), int(py)
+        h = ctypes.c_void_p()
+        rc = lib.fft3d_plan_pencil(ctypes.byref(h), Nx, Ny, Nz, self.dtype_code, self.px, self.py)
+        if rc != 0:
+            raise Fft3dError(rc, "fft3d_plan_pencil(%d,%d,%d,px=%d,py=%d)" % (Nx, Ny, Nz, px, py))
+        self._h = h
+        self._lib = lib
+        self.real_dtype = _REAL[self.dtype_code]
+        self.complex_dtype = _CPLX[self.dtype_code]
+        self.real_bytes = lib.fft3d_real_bytes(h)
+        self.complex_bytes = lib.fft3d_complex_bytes(h)
+        self.workspace_bytes = lib.fft3d_workspace_bytes(h)
+        self.n_complex = self.complex_bytes // (2 * (4 if self.dtype_code == F32 else 8))
+
+    def _blocks(self):
+        Nx, Ny, Nz = self.shape
+        L, c = Ny // self.px, (Nz // 2) // self.py
+        off = 0
+        for a in range(self.px):
+            for b in range(self.py):
+                cz = c + 1 if b == self.py - 1 else c
+                yield a, b, off, L, c, cz
+                off += Nx * L * cz
+
+    def to_natural(self, cplx_flat: torch.Tensor) -> torch.Tensor:
+        """Pencil-layout spectrum -> [Nx][Ny][Nz/2+1] (a permuted copy; index arithmetic only)."""
+        Nx, Ny, Nz = self.shape
+        out = torch.empty((Nx, Ny, Nz // 2 + 1), dtype=cplx_flat.dtype, device=cplx_flat.device)
+        for a, b, off, L, c, cz in self._blocks():
+            out[:, a * L:(a + 1) * L, b * c:b * c + cz] = cplx_flat[off:off + Nx * L * cz].reshape(Nx, L, cz)
+        return out
+
+    def from_natural(self, cplx_nat: torch.Tensor) -> torch.Tensor:
+        Nx, Ny, Nz = self.shape
+        out = torch.empty(Nx * Ny * (Nz // 2 + 1), dtype=cplx_nat.dtype, device=cplx_nat.device)
+        for a, b, off, L, c, cz in self._blocks():
+            out[off:off + Nx * L * cz] = cplx_nat[:, a * L:(a + 1) * L, b * c:b * c + cz].reshape(-1)
+        return out
 
 
 class PlanInplace(Plan):

@@ -176,4 +176,46 @@ cudaError_t launch_pack_nyquist(int dtype, const PlaneArgs& a, cudaStream_t st) 
                       : run<double>(pack_nyquist_kernel<double>, a, st);
 }
 
+// ---------------------------------------------------------------------------------------------------------
+// Pencil layout (reading R17): the spectrum of a px x py rank grid is the slab spectrum
+// with p = px whose rows of M+1 entries are cut into py pieces: rank (a, b) holds [Nx][Ny/px][cz_b], cz_b = M/py
+// (+1 for the last b: the Nyquist column), blocks concatenated in the order [a][b].  One pass over the array:
+// dir = 0: slab rows -> pencil blocks (after the forward transform), dir = 1: pencil blocks -> slab rows.
+// ---------------------------------------------------------------------------------------------------------
+struct PencilArgs {
+    const void* src;
+    void* dst;
+    long long nrows;          // px * Nx * (Ny/px) rows of M+1 entries
+    long long rows_per_a;     // Nx * (Ny/px)
+    int M, py, dir;
+};
+
+template <typename T>
+__global__ void pencil_convert_kernel(const PencilArgs a) {
+    using C = cx<T>;
+    const int pitch = a.M + 1, c = a.M / a.py;
+    const C* src = reinterpret_cast<const C*>(a.src);
+    C* dst = reinterpret_cast<C*>(a.dst);
+    for (long long row = blockIdx.x; row < a.nrows; row += gridDim.x) {
+        const long long ia = row / a.rows_per_a, r = row - ia * a.rows_per_a;     // rank row a, row (kx, ky_l) inside it
+        const long long slab = row * pitch;
+        const long long blk0 = ia * a.rows_per_a * pitch;                          // start of the blocks (a, 0..py-1)
+        for (int k = threadIdx.x; k < pitch; k += blockDim.x) {
+            int b = k / c;
+            if (b > a.py - 1) b = a.py - 1;
+            const int cz = b == a.py - 1 ? c + 1 : c;
+            const long long pen = blk0 + (long long)b * a.rows_per_a * c + r * cz + (k - b * c);
+            if (a.dir == 0) dst[pen] = src[slab + k];
+            else dst[slab + k] = src[pen];
+        }
+    }
+}
+
+cudaError_t launch_pencil_convert(int dtype, const PencilArgs& a, cudaStream_t st) {
+    long long blocks = a.nrows < 148 * 16 ? a.nrows : 148 * 16;
+    if (dtype == 0) pencil_convert_kernel<float><<<(unsigned)blocks, 256, 0, st>>>(a);
+    else pencil_convert_kernel<double><<<(unsigned)blocks, 256, 0, st>>>(a);
+    return cudaGetLastError();
+}
+
 }  // namespace fft3d

@@ -47,6 +47,13 @@ struct PlaneArgs {
     int Nx, Ny, L, M;     // M = Nz/2; rows of the spectrum have M+1 entries
 };
 cudaError_t launch_unpack_nyquist(int dtype, const PlaneArgs& a, cudaStream_t st);
+struct PencilArgs {
+    const void* src;
+    void* dst;
+    long long nrows, rows_per_a;
+    int M, py, dir;
+};
+cudaError_t launch_pencil_convert(int dtype, const PencilArgs& a, cudaStream_t st);
 cudaError_t launch_pack_nyquist(int dtype, const PlaneArgs& a, cudaStream_t st);
 
 // the same bookkeeping for distributed plans: planes published as dense copies, own rows only (fft3d_fixup.cu)
@@ -118,6 +125,7 @@ struct fft3d_plan_s {
     long long sNx;             // x extent of one virtual-slab block of the slab array: its q stride is sNx*L*M (Nx)
     int qn;                    // virtual slabs handled by the x passes, pointers already at the first one (p)
     int dist_G, dist_rank;     // distributed plans: number of ranks and this rank (0, 0 otherwise)
+    int pencil_py;             // pencil-layout plans: py (> 0), px = p; 0 otherwise
     long long nat_pitch;       // complex elements per row of the natural-layout intermediate [x][y][.]: M, or M+1 for
                                // the padded in-place layout, whose rows only the plain-load kernels can address
     int inplace;               // 1: plan of fft3d_plan_inplace (fft3d_r2c_inplace / fft3d_c2r_inplace)
@@ -654,12 +662,28 @@ static int plan_create(fft3d_plan_t** out, long long Nx, long long Ny, long long
 int fft3d_plan(fft3d_plan_t** out, long long Nx, long long Ny, long long Nz, int dtype, int virtual_slabs) {
     return plan_create(out, Nx, Ny, Nz, dtype, virtual_slabs, 0);
 }
+// Pencil layout: px x py virtual ranks.  The transform is the slab transform with p = px; its rows
+// are then cut into the py column ranges (one more pass over the spectrum, fft3d_fixup.cu).
+int fft3d_plan_pencil(fft3d_plan_t** out, long long Nx, long long Ny, long long Nz, int dtype, int px, int py) {
+    if (out == nullptr) return FFT3D_EINVAL;
+    *out = nullptr;
+    if (px < 1 || py < 1 || py > 64) return FFT3D_EINVAL;
+    // (Nx/px) x (Ny/py) x Nz pencils in real space, kz = 0..Nz/2-1 in py equal ranges (+ the Nyquist column)
+    if (Nz >= 2 && Nz % 2 == 0 && (Ny % py != 0 || (Nz / 2) % py != 0)) return FFT3D_EINVAL;
+    int rc = plan_create(out, Nx, Ny, Nz, dtype, px, 0);                // checks px | Nx and px | Ny
+    if (rc != FFT3D_OK) return rc;
+    (*out)->pencil_py = py;
+    return FFT3D_OK;
+}
 int fft3d_plan_c2c(fft3d_plan_t** out, long long Nx, long long Ny, long long Nz, int dtype, int virtual_slabs) {
     return plan_create(out, Nx, Ny, Nz, dtype, virtual_slabs, 1);
 }
 
 size_t fft3d_workspace_bytes(const fft3d_plan_t* pl) {
-    return pl ? pl->slab_bytes + pl->ring_bytes + pl->side_bytes + pl->flags_bytes : 0;
+    if (pl == nullptr) return 0;
+    const size_t base = pl->slab_bytes + pl->ring_bytes + pl->side_bytes + pl->flags_bytes;
+    // pencil-layout plans stage the slab-layout spectrum behind the ordinary workspace
+    return pl->pencil_py > 0 ? ((base + 255) & ~(size_t)255) + fft3d_complex_bytes(pl) : base;
 }
 size_t fft3d_real_bytes(const fft3d_plan_t* pl) {
     return (pl && pl->kind == 0) ? (size_t)pl->Nx * pl->Ny * pl->Nz * pl->esize : 0;
@@ -674,6 +698,13 @@ long long fft3d_index(const fft3d_plan_t* pl, long long kx, long long ky, long l
     const long long pitch = pl->kind == 0 ? pl->M + 1 : pl->Nz;
     if (kz >= pitch) return -1;
     const long long q = ky / pl->L, l = ky % pl->L;
+    if (pl->pencil_py > 0) {                               // blocks [a = q][b]; block (a, b) is [Nx][Ny/px][cz_b]
+        const long long c = pl->M / pl->pencil_py;
+        long long b = kz / c;
+        if (b > pl->pencil_py - 1) b = pl->pencil_py - 1;
+        const long long cz = b == pl->pencil_py - 1 ? c + 1 : c;
+        return q * pl->Nx * pl->L * pitch + b * pl->Nx * pl->L * c + (kx * pl->L + l) * cz + (kz - b * c);
+    }
     return ((q * pl->Nx + kx) * pl->L + l) * pitch + kz;
 }
 
@@ -707,6 +738,7 @@ int fft3d_launches(const fft3d_plan_t* pl, int which) {
     if (pl->kind == 1) return use_fused(pl) ? 2 : 3;
     // c2r on the TMA path runs the packed column 0 of the x pass as a separate small kernel
     int n = (which == 1 && use_tma(pl) && pl->tma_x) ? 5 : 4;
+    if (pl->pencil_py > 0) ++n;                  // pencil_split (last) / pencil_merge (first)
     return use_fused(pl) ? n - 1 : n;
 }
 
@@ -722,13 +754,14 @@ const char* fft3d_launch_name(const fft3d_plan_t* pl, int which, int i) {
     }
     const bool fz = use_fused(pl);
     if (which == 0) {
-        static const char* const u[] = {"z_r2c", "y_c2c_fwd", "x_c2c_fwd", "nyquist_unpack"};
-        static const char* const f[] = {"zy_r2c_fused", "x_c2c_fwd", "nyquist_unpack"};
+        static const char* const u[] = {"z_r2c", "y_c2c_fwd", "x_c2c_fwd", "nyquist_unpack", "pencil_split"};
+        static const char* const f[] = {"zy_r2c_fused", "x_c2c_fwd", "nyquist_unpack", "pencil_split"};
         return fz ? f[i] : u[i];
     }
     const bool col0 = use_tma(pl) && pl->tma_x;
-    const char* seq[5];
+    const char* seq[6];
     int n = 0;
+    if (pl->pencil_py > 0) seq[n++] = "pencil_merge";
     seq[n++] = "nyquist_pack";
     seq[n++] = "x_c2c_inv";
     if (col0) seq[n++] = "x_c2c_inv_col0";
@@ -743,6 +776,7 @@ const char* fft3d_launch_impl(const fft3d_plan_t* pl, int which, int i) {
     static const char* const names[] = {"plain", "tma", "tma_split2", "tma_split4", "bulk", "fused_ring", "fixup"};
     PassImpl im = IMPL_FIXUP;
     if (std::strstr(nm, "fused") != nullptr) im = IMPL_FUSED;
+    else if (std::strncmp(nm, "pencil", 6) == 0) im = IMPL_FIXUP;
     else if (std::strcmp(nm, "x_c2c_inv_col0") == 0) im = IMPL_PLAIN;
     else if (nm[0] == 'z') im = pl->kind == 1 ? (use_tma(pl) && pl->bulk_zc ? IMPL_BULK : IMPL_PLAIN) : z_impl(pl);
     else if (nm[0] == 'y') im = y_impl(pl);
@@ -959,6 +993,18 @@ static unsigned* ws_flags(const fft3d_plan_t* pl, void* d_work) {
     return reinterpret_cast<unsigned*>(reinterpret_cast<unsigned char*>(d_work) + pl->slab_bytes + pl->ring_bytes + pl->side_bytes);
 }
 
+static void* pencil_staging(const fft3d_plan_t* pl, void* d_work) {
+    const size_t base = pl->slab_bytes + pl->ring_bytes + pl->side_bytes + pl->flags_bytes;
+    return reinterpret_cast<unsigned char*>(d_work) + ((base + 255) & ~(size_t)255);
+}
+static int pencil_convert(const fft3d_plan_t* pl, const void* src, void* dst, int dir, cudaStream_t st) {
+    PencilArgs a{};
+    a.src = src; a.dst = dst; a.rows_per_a = pl->Nx * pl->L; a.nrows = (long long)pl->p * a.rows_per_a;
+    a.M = (int)pl->M; a.py = pl->pencil_py; a.dir = dir;
+    if (launch_pencil_convert(pl->dtype, a, st) != cudaSuccess) { cudaGetLastError(); return FFT3D_ECUDA; }
+    return FFT3D_OK;
+}
+
 int fft3d_r2c(const fft3d_plan_t* pl, const void* d_in, void* d_out, void* d_work, void* stream) {
     if (pl == nullptr || pl->kind != 0 || pl->dist_G != 0 || pl->inplace || d_in == nullptr || d_out == nullptr || d_work == nullptr) return FFT3D_EINVAL;
     const size_t rb = fft3d_real_bytes(pl), cb = fft3d_complex_bytes(pl), wb = fft3d_workspace_bytes(pl);
@@ -969,6 +1015,10 @@ int fft3d_r2c(const fft3d_plan_t* pl, const void* d_in, void* d_out, void* d_wor
     Recorder rec(pl, 0, st);
     int slot = 0;
     rec.mark(slot++);
+    // pencil-layout plans: the slab-layout spectrum (p = px) is staged behind the workspace and cut into the py
+    // column ranges of the rank grid by one more pass
+    void* user_out = d_out;
+    if (pl->pencil_py > 0) d_out = pencil_staging(pl, d_work);
     // fused: real -> (ring in L2) -> slab array in the workspace; unfused: real -> d_out (scratch use) -> workspace
     int rc = stage_fwd_zy(pl, d_in, d_out, d_work, ws_ring(pl, d_work), ws_flags(pl, d_work), st, rec, slot);
     if (rc != FFT3D_OK) return rc;
@@ -979,6 +1029,10 @@ int fft3d_r2c(const fft3d_plan_t* pl, const void* d_in, void* d_out, void* d_wor
     f.src = nullptr; f.dst = d_out; f.Nx = (int)pl->Nx; f.Ny = (int)pl->Ny; f.L = (int)pl->L; f.M = (int)pl->M;
     if (launch_unpack_nyquist(pl->dtype, f, st) != cudaSuccess) { cudaGetLastError(); return FFT3D_ECUDA; }
     rec.mark(slot++);
+    if (pl->pencil_py > 0) {
+        if (pencil_convert(pl, d_out, user_out, 0, st) != FFT3D_OK) return FFT3D_ECUDA;
+        rec.mark(slot++);
+    }
     return FFT3D_OK;
 }
 
@@ -992,6 +1046,12 @@ int fft3d_c2r(const fft3d_plan_t* pl, const void* d_in, void* d_out, void* d_wor
     Recorder rec(pl, 1, st);
     int slot = 0;
     rec.mark(slot++);
+    if (pl->pencil_py > 0) {                       // pencil blocks -> slab rows in the staging area, then as usual
+        void* staged = pencil_staging(pl, d_work);
+        if (pencil_convert(pl, d_in, staged, 1, st) != FFT3D_OK) return FFT3D_ECUDA;
+        rec.mark(slot++);
+        d_in = staged;
+    }
     const bool fz = use_fused(pl);
     // pre-pack: side[q][kx][ky_l] = sym(plane kz=0) + i sym(plane kz=Nz/2) (reading R8: only the Hermitian part of
     // the two self-conjugate planes enters Eq. (2)+(3)).  Fused: I1 writes the slab array in the workspace and I2+I3
