@@ -617,9 +617,9 @@ static int plan_create(fft3d_plan_t** out, long long Nx, long long Ny, long long
 
             if (ok) {
                 pl->fused = true; pl->fz_R = pl->fz_R_max = R;
-                // a z tile costs ~1.2x the instructions of a y tile: 54 % of the SMs (80 of 148: best of a
-                // sweep 70..84 in both directions), rounded to whole TPCs
-                pl->fz_kz[0] = pl->fz_kz[1] = (int)(sms * 0.54 + 1.0) & ~1;
+                // a z tile costs more than a y tile (Hermitian step, HBM-side latency): 57 % of the SMs (84 of 148: best
+                // of a sweep 72..96 in both directions with the round-2 kernels; 80 before), rounded to whole TPCs
+                pl->fz_kz[0] = pl->fz_kz[1] = (int)(sms * 0.57 + 0.5) & ~1;
                 // measured on B200: the fused pass wins once the array is far larger than L2 and the CTA has
                 // two consumer groups on a 3-slot ring (fp32 1024^3: 2.64 vs 3.13 ms); below that the
                 // counters' latency and the single group (fp64: 2 slots) cost more than the HBM pass saved
