@@ -33,8 +33,13 @@
  *            fft3d_index() returns the element offset of (kx,ky,kz).
  *
  * OWNERSHIP: the caller owns every data buffer and the stream.  A plan owns only its small
- * device twiddle tables and host metadata; it is immutable after creation and may be used
- * from several streams concurrently as long as each call has its own workspace.
+ * device twiddle tables and host metadata.  It belongs to the device that was current when it was
+ * created: every compute call returns FFT3D_EINVAL when another device is current.  Transform calls
+ * do not change the plan, so one plan may be used from several streams concurrently as long as each
+ * call has its own workspace; fft3d_set_variant, fft3d_set_option and fft3d_timing_* DO change it and
+ * need exclusive access.  The fused z+y kernels are cooperative launches: if the driver refuses one
+ * (SM partitions, MPS limits) the call returns FFT3D_ECUDA; fft3d_set_variant(plan, 2) selects the
+ * unfused passes.
  *
  * DEVICE entry points (fft3d_r2c / fft3d_c2r) take DEVICE pointers, 16-byte aligned, and
  * return after enqueueing work on `cuda_stream` (a cudaStream_t passed as void*; NULL = the

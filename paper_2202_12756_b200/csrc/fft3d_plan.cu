@@ -89,6 +89,7 @@ struct fft3d_plan_s {
     void *tw_z, *tw_y, *tw_x, *twz;     // device tables
     void* tw_zb;                        // stage twiddles of the bulk-pipelined z kernels
     int num_sms;
+    int device;                // the device the plan was created on: its tables, attributes and launches belong there
     int grid_z[2], grid_y[2], grid_x[2];   // persistent grid sizes [fwd, inv]
     int grid_zp[2];                        // C2C plans: the plain-load row kernels
     bool bulk_zc;                          // C2C plans: the bulk-pipelined row kernel can run (whole tiles of long rows)
@@ -458,6 +459,12 @@ bool overlap(const void* a, size_t na, const void* b, size_t nb) {
     uintptr_t x = (uintptr_t)a, y = (uintptr_t)b;
     return x < y + nb && y < x + na;
 }
+// a plan belongs to the device it was created on (twiddle tables, function attributes, SM count)
+bool wrong_device(const fft3d_plan_s* pl) {
+    int d = -1;
+    if (cudaGetDevice(&d) != cudaSuccess) { cudaGetLastError(); return true; }
+    return d != pl->device;
+}
 
 }  // namespace
 
@@ -492,7 +499,7 @@ static int plan_create(fft3d_plan_t** out, long long Nx, long long Ny, long long
     pl->Nx = Nx; pl->Ny = Ny; pl->Nz = Nz; pl->M = Mcols; pl->kind = kind; pl->p = virtual_slabs; pl->L = Ny / virtual_slabs;
     pl->dtype = dtype; pl->esize = dtype == FFT3D_F32 ? 4 : 8;
     pl->xpn = Nx; pl->xp0 = 0; pl->sNx = Nx; pl->qn = virtual_slabs; pl->nat_pitch = Mcols;
-    pl->kz = kz; pl->ky = ky; pl->kx = kx; pl->num_sms = sms;
+    pl->kz = kz; pl->ky = ky; pl->kx = kx; pl->num_sms = sms; pl->device = dev;
 
     int rc = upload_stage_twiddles(kz->nst, kz->radix, kz->twn, pl->esize, &pl->tw_z);
     if (rc == FFT3D_OK) rc = upload_stage_twiddles(ky->nst, ky->radix, ky->twn, pl->esize, &pl->tw_y);
@@ -1007,6 +1014,7 @@ static int pencil_convert(const fft3d_plan_t* pl, const void* src, void* dst, in
 
 int fft3d_r2c(const fft3d_plan_t* pl, const void* d_in, void* d_out, void* d_work, void* stream) {
     if (pl == nullptr || pl->kind != 0 || pl->dist_G != 0 || pl->inplace || d_in == nullptr || d_out == nullptr || d_work == nullptr) return FFT3D_EINVAL;
+    if (wrong_device(pl)) return FFT3D_EINVAL;          // the current device is not the plan's
     const size_t rb = fft3d_real_bytes(pl), cb = fft3d_complex_bytes(pl), wb = fft3d_workspace_bytes(pl);
     if (((uintptr_t)d_in | (uintptr_t)d_out | (uintptr_t)d_work) & 15) return FFT3D_EINVAL;
     if (overlap(d_in, rb, d_out, cb) || overlap(d_in, rb, d_work, wb) || overlap(d_out, cb, d_work, wb))
@@ -1038,6 +1046,7 @@ int fft3d_r2c(const fft3d_plan_t* pl, const void* d_in, void* d_out, void* d_wor
 
 int fft3d_c2r(const fft3d_plan_t* pl, const void* d_in, void* d_out, void* d_work, void* stream) {
     if (pl == nullptr || pl->kind != 0 || pl->dist_G != 0 || pl->inplace || d_in == nullptr || d_out == nullptr || d_work == nullptr) return FFT3D_EINVAL;
+    if (wrong_device(pl)) return FFT3D_EINVAL;          // the current device is not the plan's
     const size_t rb = fft3d_real_bytes(pl), cb = fft3d_complex_bytes(pl), wb = fft3d_workspace_bytes(pl);
     if (((uintptr_t)d_in | (uintptr_t)d_out | (uintptr_t)d_work) & 15) return FFT3D_EINVAL;
     if (overlap(d_in, cb, d_out, rb) || overlap(d_in, cb, d_work, wb) || overlap(d_out, rb, d_work, wb))
@@ -1092,6 +1101,7 @@ int fft3d_plan_inplace(fft3d_plan_t** out, long long Nx, long long Ny, long long
 
 int fft3d_r2c_inplace(const fft3d_plan_t* pl, void* d_data, void* d_work, void* stream) {
     if (pl == nullptr || !pl->inplace || d_data == nullptr || d_work == nullptr) return FFT3D_EINVAL;
+    if (wrong_device(pl)) return FFT3D_EINVAL;          // the current device is not the plan's
     if (((uintptr_t)d_data | (uintptr_t)d_work) & 15) return FFT3D_EINVAL;
     if (overlap(d_data, fft3d_complex_bytes(pl), d_work, fft3d_workspace_bytes(pl))) return FFT3D_EINVAL;
     cudaStream_t st = (cudaStream_t)stream;
@@ -1111,6 +1121,7 @@ int fft3d_r2c_inplace(const fft3d_plan_t* pl, void* d_data, void* d_work, void* 
 
 int fft3d_c2r_inplace(const fft3d_plan_t* pl, void* d_data, void* d_work, void* stream) {
     if (pl == nullptr || !pl->inplace || d_data == nullptr || d_work == nullptr) return FFT3D_EINVAL;
+    if (wrong_device(pl)) return FFT3D_EINVAL;          // the current device is not the plan's
     if (((uintptr_t)d_data | (uintptr_t)d_work) & 15) return FFT3D_EINVAL;
     if (overlap(d_data, fft3d_complex_bytes(pl), d_work, fft3d_workspace_bytes(pl))) return FFT3D_EINVAL;
     cudaStream_t st = (cudaStream_t)stream;
@@ -1190,6 +1201,7 @@ static int dist_view_zy(const fft3d_plan_t* pl, int layout, fft3d_plan_t* v) {
 
 int fft3d_dist_fwd_local(const fft3d_plan_t* pl, const void* d_real_slab, void* d_xchg, int layout, void* d_work, void* stream) {
     if (pl == nullptr || pl->dist_G == 0 || d_real_slab == nullptr || d_xchg == nullptr || d_work == nullptr) return FFT3D_EINVAL;
+    if (wrong_device(pl)) return FFT3D_EINVAL;          // the current device is not the plan's
     if (((uintptr_t)d_real_slab | (uintptr_t)d_xchg | (uintptr_t)d_work) & 15) return FFT3D_EINVAL;
     fft3d_plan_t v;
     int rc = dist_view_zy(pl, layout, &v);
@@ -1202,6 +1214,7 @@ int fft3d_dist_fwd_local(const fft3d_plan_t* pl, const void* d_real_slab, void* 
 
 int fft3d_dist_fwd_x(const fft3d_plan_t* pl, const void* d_slab_part, void* d_spec_part, void* stream) {
     if (pl == nullptr || pl->dist_G == 0 || d_slab_part == nullptr || d_spec_part == nullptr) return FFT3D_EINVAL;
+    if (wrong_device(pl)) return FFT3D_EINVAL;          // the current device is not the plan's
     if (((uintptr_t)d_slab_part | (uintptr_t)d_spec_part) & 15) return FFT3D_EINVAL;
     fft3d_plan_t v = *pl;
     v.timing = nullptr;
@@ -1229,6 +1242,9 @@ int fft3d_dist_inv_planes(const fft3d_plan_t* pl, const void* d_spec_part, void*
 
 int fft3d_dist_fwd_unpack(const fft3d_plan_t* pl, void* d_spec_part, const void* const* d_plane_parts, void* stream) {
     if (pl == nullptr || pl->dist_G == 0 || d_spec_part == nullptr || d_plane_parts == nullptr) return FFT3D_EINVAL;
+    if (wrong_device(pl)) return FFT3D_EINVAL;          // the current device is not the plan's
+    if (wrong_device(pl)) return FFT3D_EINVAL;          // the current device is not the plan's
+    if (wrong_device(pl)) return FFT3D_EINVAL;          // the current device is not the plan's
     DistPlaneArgs a{};
     a.spec_out = d_spec_part;
     for (int q = 0; q < pl->dist_G; ++q) { if (d_plane_parts[q] == nullptr) return FFT3D_EINVAL; a.parts[q] = d_plane_parts[q]; }
@@ -1239,6 +1255,7 @@ int fft3d_dist_fwd_unpack(const fft3d_plan_t* pl, void* d_spec_part, const void*
 
 int fft3d_dist_inv_pack(const fft3d_plan_t* pl, const void* const* d_plane_parts, void* d_work, void* stream) {
     if (pl == nullptr || pl->dist_G == 0 || d_plane_parts == nullptr || d_work == nullptr) return FFT3D_EINVAL;
+    if (wrong_device(pl)) return FFT3D_EINVAL;          // the current device is not the plan's
     DistPlaneArgs a{};
     a.side = dist_side(pl, d_work);
     for (int q = 0; q < pl->dist_G; ++q) { if (d_plane_parts[q] == nullptr) return FFT3D_EINVAL; a.parts[q] = d_plane_parts[q]; }
@@ -1249,6 +1266,7 @@ int fft3d_dist_inv_pack(const fft3d_plan_t* pl, const void* const* d_plane_parts
 
 int fft3d_dist_inv_x(const fft3d_plan_t* pl, const void* d_spec_part, void* d_slab_part, void* d_work, void* stream) {
     if (pl == nullptr || pl->dist_G == 0 || d_spec_part == nullptr || d_slab_part == nullptr || d_work == nullptr) return FFT3D_EINVAL;
+    if (wrong_device(pl)) return FFT3D_EINVAL;          // the current device is not the plan's
     if (((uintptr_t)d_slab_part | (uintptr_t)d_spec_part | (uintptr_t)d_work) & 15) return FFT3D_EINVAL;
     fft3d_plan_t v = *pl;
     v.timing = nullptr;
@@ -1261,6 +1279,7 @@ int fft3d_dist_inv_x(const fft3d_plan_t* pl, const void* d_spec_part, void* d_sl
 
 int fft3d_dist_inv_local(const fft3d_plan_t* pl, const void* d_xchg, int layout, void* d_real_slab, void* d_work, void* stream) {
     if (pl == nullptr || pl->dist_G == 0 || d_real_slab == nullptr || d_xchg == nullptr || d_work == nullptr) return FFT3D_EINVAL;
+    if (wrong_device(pl)) return FFT3D_EINVAL;          // the current device is not the plan's
     if (((uintptr_t)d_real_slab | (uintptr_t)d_xchg | (uintptr_t)d_work) & 15) return FFT3D_EINVAL;
     fft3d_plan_t v;
     int rc = dist_view_zy(pl, layout, &v);
@@ -1276,6 +1295,7 @@ int fft3d_dist_inv_local(const fft3d_plan_t* pl, const void* d_xchg, int layout,
 // +1: inverse, scaled by 1/(NxNyNz), the passes in reverse order.
 int fft3d_c2c(const fft3d_plan_t* pl, const void* d_in, void* d_out, void* d_work, int direction, void* stream) {
     if (pl == nullptr || pl->kind != 1 || d_in == nullptr || d_out == nullptr || d_work == nullptr) return FFT3D_EINVAL;
+    if (wrong_device(pl)) return FFT3D_EINVAL;          // the current device is not the plan's
     if (direction != -1 && direction != 1) return FFT3D_EINVAL;
     const size_t cb = fft3d_complex_bytes(pl), wb = fft3d_workspace_bytes(pl);
     if (((uintptr_t)d_in | (uintptr_t)d_out | (uintptr_t)d_work) & 15) return FFT3D_EINVAL;
@@ -1424,8 +1444,9 @@ int fft3d_timing_read(fft3d_plan_t* pl, int which, float* ms_sum, int* calls) {
 
 static int ensure_host_buffers(fft3d_plan_t* pl) {
     if (pl->h_real != nullptr) return FFT3D_OK;
-    if (cudaStreamCreateWithFlags(&pl->h_stream, cudaStreamNonBlocking) != cudaSuccess) {
+    if (pl->h_stream == nullptr && cudaStreamCreateWithFlags(&pl->h_stream, cudaStreamNonBlocking) != cudaSuccess) {
         cudaGetLastError();
+        pl->h_stream = nullptr;
         return FFT3D_ECUDA;
     }
     if (cudaMalloc(&pl->h_real, pl->kind == 0 ? fft3d_real_bytes(pl) : fft3d_complex_bytes(pl)) != cudaSuccess ||
@@ -1441,6 +1462,7 @@ static int ensure_host_buffers(fft3d_plan_t* pl) {
 
 int fft3d_r2c_host(fft3d_plan_t* pl, const void* h_in, void* h_out) {
     if (pl == nullptr || pl->kind != 0 || h_in == nullptr || h_out == nullptr) return FFT3D_EINVAL;
+    if (wrong_device(pl)) return FFT3D_EINVAL;          // the current device is not the plan's
     int rc = ensure_host_buffers(pl);
     if (rc != FFT3D_OK) return rc;
     cudaStream_t st = pl->h_stream;
@@ -1460,6 +1482,7 @@ int fft3d_r2c_host(fft3d_plan_t* pl, const void* h_in, void* h_out) {
 
 int fft3d_c2r_host(fft3d_plan_t* pl, const void* h_in, void* h_out) {
     if (pl == nullptr || pl->kind != 0 || h_in == nullptr || h_out == nullptr) return FFT3D_EINVAL;
+    if (wrong_device(pl)) return FFT3D_EINVAL;          // the current device is not the plan's
     int rc = ensure_host_buffers(pl);
     if (rc != FFT3D_OK) return rc;
     cudaStream_t st = pl->h_stream;
@@ -1479,6 +1502,7 @@ int fft3d_c2r_host(fft3d_plan_t* pl, const void* h_in, void* h_out) {
 
 int fft3d_c2c_host(fft3d_plan_t* pl, const void* h_in, void* h_out, int direction) {
     if (pl == nullptr || pl->kind != 1 || h_in == nullptr || h_out == nullptr) return FFT3D_EINVAL;
+    if (wrong_device(pl)) return FFT3D_EINVAL;          // the current device is not the plan's
     if (direction != -1 && direction != 1) return FFT3D_EINVAL;
     int rc = ensure_host_buffers(pl);
     if (rc != FFT3D_OK) return rc;
