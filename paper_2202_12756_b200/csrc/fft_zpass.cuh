@@ -90,56 +90,65 @@ __device__ __forceinline__ double2 shfl_cx<double>(double2 v, int src, int width
     return r;
 }
 
-// R2C:  X[k] = (Z[k] + conj Z[M-k])/2 - (i/2) w^k (Z[k] - conj Z[M-k]),  w = exp(-2 pi i/Nz)
-// (scalar arithmetic on purpose, here and in the per-thread rotations of w: the operands come out of warp shuffles
-//  word by word; the packed f32x2 forms of fft_radix.cuh cost register moves here and were slower, measured)
-template <typename T>
-__device__ __forceinline__ cx<T> herm_post(cx<T> z, cx<T> zp, cx<T> w) {
-    const T ex = z.x + zp.x, ey = z.y - zp.y, dx = z.x - zp.x, dy = z.y + zp.y;
+// The Hermitian step, one PAIR (k, M-k) at a time.  With e = A + conj B, d = A - conj B (A = element k, B = element
+// M-k, both before the step), w = exp(-+2 pi i k/Nz) and w^(M-k) = -conj(w^k):
+//   R2C (after the forward FFT):   X[k] = (e - i w d)/2,   X[M-k] = conj((e + i w d)/2)
+//   C2R (before the inverse FFT):  Z[k] =  e + i w d,      Z[M-k] = conj(e - i w d)
+// so the two outputs of a pair share e, d and w d: 12 operations for both instead of 12 each.  `w` arrives already
+// halved for R2C.  (Scalar arithmetic on purpose, here and in the per-thread rotations of w: the operands come out of
+// warp shuffles word by word; the packed f32x2 forms of fft_radix.cuh cost register moves here and were slower, measured.)
+template <bool INV, typename T>
+__device__ __forceinline__ void herm_pair(cx<T> a, cx<T> b, cx<T> w, cx<T>& rk, cx<T>& rmk) {
+    const T ex = a.x + b.x, ey = a.y - b.y, dx = a.x - b.x, dy = a.y + b.y;
     const T wdx = w.x * dx - w.y * dy, wdy = w.x * dy + w.y * dx;
-    return mk<T>((T)0.5 * (ex + wdy), (T)0.5 * (ey - wdx));
-}
-// C2R:  Z[k] = (X[k] + conj X[M-k]) + i conj(w)^k (X[k] - conj X[M-k])
-template <typename T>
-__device__ __forceinline__ cx<T> herm_pre(cx<T> x, cx<T> xp, cx<T> wc) {
-    const T ex = x.x + xp.x, ey = x.y - xp.y, dx = x.x - xp.x, dy = x.y + xp.y;
-    const T wdx = wc.x * dx - wc.y * dy, wdy = wc.x * dy + wc.y * dx;
-    return mk<T>(ex - wdy, ey + wdx);
+    if constexpr (!INV) {
+        rk = mk<T>((T)0.5 * ex + wdy, (T)0.5 * ey - wdx);
+        rmk = mk<T>((T)0.5 * ex - wdy, (T)-0.5 * ey - wdx);
+    } else {
+        rk = mk<T>(ex - wdy, ey + wdx);
+        rmk = mk<T>(ex + wdy, wdx - ey);
+    }
 }
 
-// The Hermitian step on the thread's P values, in place, pair (m, P-1-m) at a time.
+// The Hermitian step on the thread's P values, in place.  Thread t of a row holds elements k = t + m S in v[m]; element
+// M-k lives in lane (S-t) mod S, register P-1-m.  Per register pair (m, m2 = P-1-m) a lane fetches the partner of its
+// v[m] with one shuffle per word, computes BOTH outputs of that pair, keeps X[k] and hands X[M-k] back to the partner
+// lane (whose register m2 it belongs to) with another shuffle per word -- while receiving its own v[m2] from there.
+// Lane 0 pairs with itself (k = m S <-> (P-m) S, register P-m): its partners come from the scratch copy `scr` of its
+// values and its second output goes to its own register P-m; its element 0 is the packed real pair (X[0], X[Nz/2]) and
+// its element M/2 (register P/2) is self-conjugate.
 //   INV = false: post-process after the forward FFT (wt = exp(-2 pi i t/Nz))
 //   INV = true : pre-process before the inverse FFT (wt = exp(+2 pi i t/Nz))
 template <class Cfg, bool INV, typename T, int MM = 0>
-__device__ __forceinline__ void hermitian_step(cx<T> (&v)[Cfg::P], cx<T> wt, int t, const cx<T>* scr) {
+__device__ __forceinline__ void hermitian_rec(cx<T> (&v)[Cfg::P], cx<T> wt, int t, const cx<T>* scr) {
     using C = cx<T>;
     constexpr int P = Cfg::P, S = Cfg::S;
     if constexpr (MM < P / 2) {
         constexpr int m = MM, m2 = P - 1 - MM;
-        const C a = v[m], b = v[m2];
         const int src = (S - t) & (S - 1);
-        C pa = shfl_cx<T>(b, src, S);            // element M - (t + m S)  = lane S-t, register P-1-m
-        C pb = shfl_cx<T>(a, src, S);            // element M - (t + m2 S) = lane S-t, register m
-        if (t == 0) {                            // lane 0 pairs with itself: k = mS <-> (P-m)S
-            if constexpr (m > 0) pa = scr[P - m];
-            pb = scr[P - m2];
-        }
+        const C a = v[m];
+        C pa = shfl_cx<T>(v[m2], src, S);        // element M - (t + m S) = lane S-t, register P-1-m
+        if constexpr (m > 0) { if (t == 0) pa = scr[P - m]; }
         // w^(t + m S) = wt * exp(-+2 pi i m/(2P))
         const C wa = mul_root<m, 2 * P, INV ? +1 : -1, T, false>(wt);
-        const C wb = mul_root<m2, 2 * P, INV ? +1 : -1, T, false>(wt);
-        if constexpr (!INV) {
-            C ra = herm_post<T>(a, pa, wa);
-            if constexpr (m == 0) { if (t == 0) ra = mk<T>(a.x + a.y, a.x - a.y); }   // (X[0], X[Nz/2]) packed
-            v[m] = ra;
-            v[m2] = herm_post<T>(b, pb, wb);
-        } else {
-            C ra = herm_pre<T>(a, pa, wa);
-            if constexpr (m == 0) { if (t == 0) ra = mk<T>(a.x + a.y, a.x - a.y); }   // Z[0] = (X0+XM) + i(X0-XM)
-            v[m] = ra;
-            v[m2] = herm_pre<T>(b, pb, wb);
-        }
-        hermitian_step<Cfg, INV, T, MM + 1>(v, wt, t, scr);
+        C rk, rmk;
+        herm_pair<INV, T>(a, pa, wa, rk, rmk);
+        if constexpr (m == 0) { if (t == 0) rk = mk<T>(a.x + a.y, a.x - a.y); }   // (X[0], X[Nz/2]) packed / Z[0]
+        const C got = shfl_cx<T>(rmk, src, S);   // X[M - (src + m S)] = my element t + m2 S, computed by lane S-t
+        v[m] = rk;
+        if (t != 0) v[m2] = got;
+        if constexpr (m > 0) { if (t == 0) v[P - m] = rmk; }
+        hermitian_rec<Cfg, INV, T, MM + 1>(v, wt, t, scr);
     }
+}
+
+template <class Cfg, bool INV, typename T>
+__device__ __forceinline__ void hermitian_step(cx<T> (&v)[Cfg::P], cx<T> wt, int t, const cx<T>* scr) {
+    constexpr int P = Cfg::P;
+    const cx<T> mid = v[P / 2];                  // lane 0: element M/2, w^(M/2) = -+i: X = conj Z, Z = 2 conj X
+    if constexpr (!INV) wt = mk<T>((T)0.5 * wt.x, (T)0.5 * wt.y);
+    hermitian_rec<Cfg, INV, T>(v, wt, t, scr);
+    if (t == 0) v[P / 2] = INV ? mk<T>(mid.x + mid.x, -(mid.y + mid.y)) : mk<T>(mid.x, -mid.y);
 }
 
 // DIR = -1: R2C (pass F1);  DIR = +1: C2R with normalisation (pass I3)
