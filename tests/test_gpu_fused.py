@@ -146,3 +146,52 @@ def test_repeated_calls_are_bit_identical(fft, variant):
         assert torch.equal(torch.view_as_real(out), torch.view_as_real(out0))
         assert torch.equal(back, back0)
     plan.close()
+
+
+def test_fused_options_do_not_change_the_result(fft):
+    """fft3d_set_option: any split of the SMs between the z and the y role and any ring depth gives the same bits
+    (tiles are dealt dynamically: with 2 or 146 SMs in a role most CTAs of the other role find no tile at all and
+    must leave through the end items), and out-of-range values are refused."""
+    from paper_2202_12756_b200 import inputs
+    B = fft.binding
+    shape = (16, 512, 512)
+    f = inputs.uniform_grid(shape, torch.float32, seed=31).cuda()
+    plan = fft.Plan(*shape, dtype=torch.float32, virtual_slabs=2)
+    plan.set_variant(3)
+    assert plan.launch_names(0)[0] == "zy_r2c_fused"
+    out0 = plan.r2c(f).clone()
+    back0 = plan.c2r(out0).clone()
+    for kz, ring in ((2, 8), (146, 8), (0, 8), (84, 2), (40, 3), (100, 5)):
+        plan.set_option(B.OPT_FUSED_Z_SMS_FWD, kz)
+        plan.set_option(B.OPT_FUSED_Z_SMS_INV, kz)
+        plan.set_option(B.OPT_FUSED_RING_PLANES, ring)
+        out = plan.r2c(f)
+        back = plan.c2r(out0)
+        torch.cuda.synchronize()
+        assert torch.equal(torch.view_as_real(out), torch.view_as_real(out0)), (kz, ring)
+        assert torch.equal(back, back0), (kz, ring)
+    for opt, val in ((B.OPT_FUSED_RING_PLANES, 1), (B.OPT_FUSED_RING_PLANES, 99), (B.OPT_FUSED_Z_SMS_FWD, 3), (99, 1)):
+        with pytest.raises(B.Fft3dError):
+            plan.set_option(opt, val)
+    plan.close()
+
+
+def test_fused_with_fewer_tiles_than_ctas(fft, oracle_mod):
+    """Nx = 8 planes of 256 x 256: 128 z tiles and 128 y tiles for 148 CTAs -- some CTAs get one tile, some none."""
+    from paper_2202_12756_b200 import inputs
+    shape = (8, 256, 256)
+    f = inputs.uniform_grid(shape, torch.float32, seed=32)
+    plan = fft.Plan(*shape, dtype=torch.float32, virtual_slabs=1)
+    plan.set_variant(3)
+    if plan.launch_names(0)[0] != "zy_r2c_fused":
+        plan.close()
+        pytest.skip("no fused kernels for this shape")
+    out = plan.r2c(f.cuda())
+    back = plan.c2r(out)
+    torch.cuda.synchronize()
+    F_ref = oracle_mod.r2c(f.double().numpy())
+    err = np.linalg.norm((plan.to_natural(out).cpu().numpy().astype(np.complex128) - F_ref).ravel()) / np.linalg.norm(F_ref.ravel())
+    bound = 2e-6 * math.log2(shape[0] * shape[1] * shape[2])
+    assert err <= bound
+    assert (back.cpu() - f).abs().max().item() <= bound
+    plan.close()
