@@ -282,9 +282,12 @@ int fft3d_set_variant(fft3d_plan_t *plan, int variant);
  * fft3d_set_variant these change the plan: call them while no transform on this plan is being enqueued.
  * Results do not depend on them (bit-identical).  Returns FFT3D_EINVAL for an unknown option or a value out
  * of range.
- *   FUSED_Z_SMS_FWD / _INV   SMs [0, value) run the z tiles, the others the y tiles (even; 0 = alternate CTA pairs)
+ *   FUSED_MIXED              1 (default): every CTA runs both roles, one consumer group on z tiles and one on y tiles,
+ *                            its load warp dealing the ring slots to the two streams; 0: one role per CTA
+ *   FUSED_Z_SMS_FWD / _INV   with one role per CTA: SMs [0, value) run the z tiles, the others the y tiles (even;
+ *                            0 = alternate CTA pairs)
  *   FUSED_RING_PLANES        yz-planes in the L2 ring (2 .. the number the workspace was sized for) */
-enum { FFT3D_OPT_FUSED_Z_SMS_FWD = 1, FFT3D_OPT_FUSED_Z_SMS_INV = 2, FFT3D_OPT_FUSED_RING_PLANES = 3 };
+enum { FFT3D_OPT_FUSED_Z_SMS_FWD = 1, FFT3D_OPT_FUSED_Z_SMS_INV = 2, FFT3D_OPT_FUSED_RING_PLANES = 3, FFT3D_OPT_FUSED_MIXED = 4 };
 int fft3d_set_option(fft3d_plan_t *plan, int option, long long value);
 
 int fft3d_destroy(fft3d_plan_t *plan);          /* NULL is accepted */

@@ -117,6 +117,7 @@ struct fft3d_plan_s {
     bool fused_default;        // ... and expected to win (variant 0 uses them)
     int fz_R;                  // ring depth (planes)
     int fz_kz[2];              // [fwd, inv] SMs [0, kz) run the z tiles, the others the y tiles (0: split by CTA pairs)
+    int fz_mixed;              // 1: every CTA runs both roles (one consumer group each); needs two consumer groups
     int fz_R_max;              // ring planes the workspace was sized for
     size_t slab_bytes, ring_bytes, side_bytes, flags_bytes;
     // Sub-ranges the passes work on.  A plain plan covers the whole problem; the stage entry points of a
@@ -320,6 +321,7 @@ int launch_fused(const fft3d_plan_s* pl, int d, const void* in, void* out, void*
     FusedArgs a{};
     a.in = in; a.out = out; a.ring = ring; a.tw_z = c2c ? pl->tw_zc : pl->tw_zb; a.twz = pl->twz; a.tw_y = pl->tw_y; a.flags = flags;
     a.Nx = (int)pl->xpn; a.Ny = (int)pl->Ny; a.L = (int)pl->L; a.R = pl->fz_R; a.kz = pl->fz_kz[d];
+    a.mixed = (pl->fz_mixed && (c2c ? ky->fc_ng : ky->fz_ng) == 2) ? 1 : 0;
     a.rows_slab = pl->y_rows_slab;
     a.scale = 1.0 / ((double)pl->Nx * (double)pl->Ny * (double)pl->Nz);
     void* argv[3] = {(void*)&ring_map, (void*)&slab_map, (void*)&a};
@@ -623,7 +625,7 @@ static int plan_create(fft3d_plan_t** out, long long Nx, long long Ny, long long
             }
 
             if (ok) {
-                pl->fused = true; pl->fz_R = pl->fz_R_max = R;
+                pl->fused = true; pl->fz_R = pl->fz_R_max = R; pl->fz_mixed = 1;
                 // a z tile costs more than a y tile (Hermitian step, HBM-side latency): 57 % of the SMs (84 of 148: best
                 // of a sweep 72..96 in both directions with the round-2 kernels; 80 before), rounded to whole TPCs
                 pl->fz_kz[0] = pl->fz_kz[1] = (int)(sms * 0.57 + 0.5) & ~1;
@@ -653,7 +655,7 @@ static int plan_create(fft3d_plan_t** out, long long Nx, long long Ny, long long
             }
 
             if (ok) {
-                pl->fused = true; pl->fz_R = pl->fz_R_max = R;
+                pl->fused = true; pl->fz_R = pl->fz_R_max = R; pl->fz_mixed = 1;
                 pl->fz_kz[0] = pl->fz_kz[1] = (sms / 2 + 1) & ~1;      // z and y tiles cost about the same here
                 pl->fused_default = pl->slab_bytes >= ((size_t)2 << 30);
                 pl->ring_bytes = plane * R;
@@ -798,6 +800,10 @@ int fft3d_set_option(fft3d_plan_t* pl, int option, long long value) {
         case FFT3D_OPT_FUSED_Z_SMS_INV:
             if (value < 0 || value >= pl->num_sms || (value & 1)) return FFT3D_EINVAL;   // whole TPCs; 0 = split by CTA pairs
             pl->fz_kz[option == FFT3D_OPT_FUSED_Z_SMS_FWD ? 0 : 1] = (int)value;
+            return FFT3D_OK;
+        case FFT3D_OPT_FUSED_MIXED:
+            if (value != 0 && value != 1) return FFT3D_EINVAL;
+            pl->fz_mixed = (int)value;
             return FFT3D_OK;
         case FFT3D_OPT_FUSED_RING_PLANES:
             if (!pl->fused || value < 2 || value > pl->fz_R_max || value > pl->Nx) return FFT3D_EINVAL;

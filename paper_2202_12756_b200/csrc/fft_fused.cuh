@@ -33,6 +33,16 @@
 // takes fewer tiles instead of holding every plane back (measured: forward 2.87 -> 2.74 ms at 1024^3).  Every spin
 // on a global counter is bounded.
 //
+// BOTH ROLES IN EVERY CTA (FusedArgs::mixed, the default where the CTA has two consumer groups): since the packed
+// arithmetic shrank the two tile bodies to ~37 KB together, a TPC's instruction cache holds both (roles mixed inside
+// TPCs cost 1 % now, 50 % before), so a CTA need not be bound to one role: consumer group 0 transforms z tiles, group 1
+// y tiles, and the load warp deals the ring slots to the two streams -- a phase-2 tile when its plane is complete, a
+// phase-1 tile otherwise, alternating when both are possible; phase-1 tiles never hold all the slots (their stores may
+// wait for the ring's back-pressure, which only phase-2 loads relieve) and are not taken a ring's depth ahead of the
+// phase-2 tickets.  Both groups look at every item in order and take the ones of their role.  Every SM then carries
+// the same mix of compute-heavy z tiles and latency-heavy y tiles, and no SM split has to be tuned
+// (measured at 1024^3: forward 2.57 -> 2.49 ms, inverse 2.82 -> 2.76 ms on the same box).
+//
 // Ordering between CTAs uses two counters per plane in global memory (zeroed before the launch):
 //   p1_done[x]    += 1 when a phase-1 tile of plane x has been stored (store complete, released at once)
 //   p2_loaded[x]  += 1 when a phase-2 tile of plane x has landed in shared memory
@@ -70,6 +80,7 @@ struct FusedArgs {
     int rows_slab;           // rows per TMA box on the slab side of a y tile
     double scale;            // inverse: 1/(Nx Ny Nz)
     int kz;                  // SMs [0, kz) take the z tiles (0: split by CTA pairs)
+    int mixed;               // 1: every CTA runs both roles (consumer group 0 the z tiles, group 1 the y tiles)
 };
 
 namespace tma {
@@ -195,7 +206,7 @@ fft_zy_fused_kernel(const __grid_constant__ TensorMapBlob ring_map, const __grid
     // within one phase of the barrier's current one, so a group polls seen[s] before it waits for ITS phase.
     volatile int* seen = reinterpret_cast<volatile int*>(empty + NSTAGE);
     volatile int* role_s = seen + NSTAGE;                // [role_z] broadcast from thread 0
-    volatile int* item_q = role_s + 4;                   // [s] global tile index in slot s (-1: no more tiles), [NSTAGE] first end item, [NSTAGE+1+s] its plane
+    volatile int* item_q = role_s + 4;                   // [s] global tile index in slot s (-1: no more tiles), [NSTAGE] first end item, [NSTAGE+1+s] its plane, [2 NSTAGE+1+s] 1 = a z tile
 
     const int tid = threadIdx.x;
     if (tid == NCONS) {
@@ -248,12 +259,113 @@ fft_zy_fused_kernel(const __grid_constant__ TensorMapBlob ring_map, const __grid
         if (tid == NCONS) {
             // ------------------------- load warp -------------------------
             const unsigned long long pol_stream = tma::policy_evict_first(), pol_keep = tma::policy_evict_last();
+            // the loads of one tile into ring slot s
+            auto issue_load = [&](bool isz, int x, int j, int s) {
+                unsigned char* dst = stages + s * FT::STAGE_BYTES;
+                if (isz) {
+                    tma::mbar_expect_tx(&full[s], ZT::TILE_BYTES);
+                    if constexpr (FWD) {                 // rows of the real input (HBM stream)
+                        const unsigned char* src = reinterpret_cast<const unsigned char*>(a.in) + (long long)x * plane_bytes +
+                                                   (long long)j * ZT::TILE_BYTES;
+                        constexpr int CHUNK = 65536;
+                        for (int o = 0; o < ZT::TILE_BYTES; o += CHUNK)
+                            tma::bulk_load_h(dst + o, src + o, ZT::TILE_BYTES - o < CHUNK ? ZT::TILE_BYTES - o : CHUNK, &full[s], pol_stream);
+                    } else {                             // RPT rows gathered from the column-tiled ring: one box
+                        tma::load4_h(dst, &ring_map, &full[s], 0, 0, j * RPT, x % a.R, pol_keep);
+                    }
+                } else {
+                    tma::mbar_expect_tx(&full[s], YT::TILE_BYTES);
+                    if constexpr (FWD) {                 // column tile j of the ring plane: one contiguous block
+                        const unsigned char* src = reinterpret_cast<const unsigned char*>(a.ring) +
+                                                   (long long)(x % a.R) * plane_bytes + (long long)j * YT::TILE_BYTES;
+                        constexpr int CHUNK = 65536;
+                        for (int o = 0; o < YT::TILE_BYTES; o += CHUNK)
+                            tma::bulk_load_h(dst + o, src + o, YT::TILE_BYTES - o < CHUNK ? YT::TILE_BYTES - o : CHUNK, &full[s], pol_keep);
+                    } else {                             // columns of plane x gathered from the slab layout
+                        const int nb = NY / a.rows_slab;
+                        for (int b = 0; b < nb; ++b) {
+                            const int r0 = b * a.rows_slab;
+                            tma::load4_h(dst + (size_t)b * a.rows_slab * YT::ROW_BYTES, &slab_map, &full[s],
+                                         j * TC * W, r0 % a.L, x, r0 / a.L, pol_stream);
+                        }
+                    }
+                }
+            };
+            if (NG == 2 && a.mixed) {
+                // ---- both roles in this CTA: the load warp deals the ring slots to the two streams.  A phase-2 tile is
+                // taken when its plane is complete (checked without blocking), a phase-1 tile otherwise; when both are
+                // possible the streams alternate.  Phase-1 tiles never hold all the slots (their stores may wait for the
+                // ring's back-pressure, which only phase-2 loads relieve) unless no phase-2 tile is left to take.
+                const int tot1 = a.Nx * n1, tot2 = a.Nx * n2;
+                unsigned* next1 = &ctl[FWD ? FZ_CTL_NEXT_Z : FZ_CTL_NEXT_Y];
+                unsigned* next2 = &ctl[FWD ? FZ_CTL_NEXT_Y : FZ_CTL_NEXT_Z];
+                int g1 = (int)atomicAdd(next1, 1u), g2 = (int)atomicAdd(next2, 1u);
+                int ready = -1, inflight1 = 0, last1 = 0, ends = 0;
+                unsigned p1mask = 0;                     // bit s: the item in slot s is a phase-1 tile
+                for (int i = 0;; ++i) {
+                    const int s = i % NSTAGE, n = i / NSTAGE;
+                    // the readiness of the next phase-2 ticket's plane is read BEFORE the wait for the slot (an L2 round
+                    // trip that would otherwise sit between the slot becoming free and its next load)
+                    if (g2 < tot2) {
+                        const int x2 = g2 / n2;
+                        if (x2 > ready && tma::ld_acquire(&p1_done[x2]) >= (unsigned)n1) { tma::fence_proxy_async_all(); ready = x2; }
+                    }
+                    if (n > 0) {
+                        tma::mbar_wait(&empty[s], (unsigned)((n - 1) & 1));
+                        inflight1 -= (int)((p1mask >> s) & 1u);
+                        p1mask &= ~(1u << s);
+                    }
+                    int take = 0;                        // 1: phase-1 tile, 2: phase-2 tile, 0: nothing left
+                    for (unsigned polls = 0;;) {
+                        const bool has1 = g1 < tot1, has2 = g2 < tot2;
+                        if (!has1 && !has2) break;
+                        const int x2 = has2 ? g2 / n2 : 0x3fffffff;
+                        // a phase-1 tile whose plane is a ring's depth ahead of the phase-2 tickets would only sit in
+                        // its slot waiting for the ring's back-pressure: leave the slot to a phase-2 tile instead
+                        const bool can1 = has1 && (!has2 || (inflight1 < NSTAGE - 1 && g1 / n1 < x2 + a.R));
+                        if (can1 && (last1 == 0 || !has2)) { take = 1; break; }
+                        bool can2 = has2 && x2 <= ready;
+                        if (has2 && !can2 && polls > 0 && tma::ld_acquire(&p1_done[x2]) >= (unsigned)n1) {
+                            tma::fence_proxy_async_all(); ready = x2; can2 = true;
+                        }
+                        if (can2) { take = 2; break; }
+                        if (can1) { take = 1; break; }
+                        if (polls > 0) __nanosleep(64);
+                        if (++polls > (1u << 24)) __trap();
+                    }
+                    if (take == 0) {                     // NSTAGE end items: both groups and every store warp see one
+                        item_q[s] = -1;
+                        tma::mbar_arrive(&full[s]);
+                        if (++ends == NSTAGE) break;
+                        continue;
+                    }
+                    const int g = take == 1 ? g1 : g2, np = take == 1 ? n1 : n2;
+                    const int x = g / np, j = g - x * np;
+                    const bool isz = FWD ? take == 1 : take == 2;
+                    item_q[s] = g; item_q[NSTAGE + 1 + s] = x; item_q[2 * NSTAGE + 1 + s] = isz ? 1 : 0;
+                    issue_load(isz, x, j, s);
+                    if (take == 1) {
+                        p1mask |= 1u << s; ++inflight1; last1 = 1;
+                        g1 = (int)atomicAdd(next1, 1u);
+                        if constexpr (FWD) {
+                            if (g1 < tot1) {
+                                const int nx = g1 / n1, nj = g1 - nx * n1;
+                                tma::prefetch_l2(reinterpret_cast<const unsigned char*>(a.in) + (long long)nx * plane_bytes +
+                                                 (long long)nj * ZT::TILE_BYTES, ZT::TILE_BYTES, pol_stream);
+                            }
+                        }
+                    } else {
+                        last1 = 0;
+                        g2 = (int)atomicAdd(next2, 1u);
+                    }
+                }
+                return;
+            }
             int i = 0, ready = -1;                       // planes <= ready are known to be complete in the ring
             unsigned* next = &ctl[role_z ? FZ_CTL_NEXT_Z : FZ_CTL_NEXT_Y];
             int g = (int)atomicAdd(next, 1u);            // the next tile of this role, in order
             for (;;) {
                 const int s = i % NSTAGE, n = i / NSTAGE;
-                unsigned char* dst = stages + s * FT::STAGE_BYTES;
                 if (n > 0) tma::mbar_wait(&empty[s], (unsigned)((n - 1) & 1));
                 if (g >= total) {                        // NSTAGE end items: every group and every store warp sees one
                     if (item_q[NSTAGE] < 0) item_q[NSTAGE] = i;
@@ -263,41 +375,13 @@ fft_zy_fused_kernel(const __grid_constant__ TensorMapBlob ring_map, const __grid
                     continue;
                 }
                 FItem it; it.p1 = my_p1; it.x = g / nper; it.j = g - it.x * nper;
-                item_q[s] = g; item_q[NSTAGE + 1 + s] = it.x;
+                item_q[s] = g; item_q[NSTAGE + 1 + s] = it.x; item_q[2 * NSTAGE + 1 + s] = role_z;
                 if (!it.p1 && it.x > ready) {
                     tma::wait_count(&p1_done[it.x], (unsigned)n1);
                     tma::fence_proxy_async_all();
                     ready = it.x;
                 }
-                const bool isz = FWD ? it.p1 : !it.p1;
-                if (isz) {
-                    tma::mbar_expect_tx(&full[s], ZT::TILE_BYTES);
-                    if constexpr (FWD) {                 // rows of the real input (HBM stream)
-                        const unsigned char* src = reinterpret_cast<const unsigned char*>(a.in) + (long long)it.x * plane_bytes +
-                                                   (long long)it.j * ZT::TILE_BYTES;
-                        constexpr int CHUNK = 65536;
-                        for (int o = 0; o < ZT::TILE_BYTES; o += CHUNK)
-                            tma::bulk_load_h(dst + o, src + o, ZT::TILE_BYTES - o < CHUNK ? ZT::TILE_BYTES - o : CHUNK, &full[s], pol_stream);
-                    } else {                             // RPT rows gathered from the column-tiled ring: one box
-                        tma::load4_h(dst, &ring_map, &full[s], 0, 0, it.j * RPT, it.x % a.R, pol_keep);
-                    }
-                } else {
-                    tma::mbar_expect_tx(&full[s], YT::TILE_BYTES);
-                    if constexpr (FWD) {                 // column tile j of the ring plane: one contiguous block
-                        const unsigned char* src = reinterpret_cast<const unsigned char*>(a.ring) +
-                                                   (long long)(it.x % a.R) * plane_bytes + (long long)it.j * YT::TILE_BYTES;
-                        constexpr int CHUNK = 65536;
-                        for (int o = 0; o < YT::TILE_BYTES; o += CHUNK)
-                            tma::bulk_load_h(dst + o, src + o, YT::TILE_BYTES - o < CHUNK ? YT::TILE_BYTES - o : CHUNK, &full[s], pol_keep);
-                    } else {                             // columns of plane x gathered from the slab layout
-                        const int nb = NY / a.rows_slab;
-                        for (int b = 0; b < nb; ++b) {
-                            const int r0 = b * a.rows_slab;
-                            tma::load4_h(dst + (size_t)b * a.rows_slab * YT::ROW_BYTES, &slab_map, &full[s],
-                                         it.j * TC * W, r0 % a.L, it.x, r0 / a.L, pol_stream);
-                        }
-                    }
-                }
+                issue_load(FWD ? it.p1 : !it.p1, it.x, it.j, s);
                 ++i;
                 g = (int)atomicAdd(next, 1u);            // drawn ahead: its latency hides behind the wait for the slot
                 if constexpr (FWD) {
@@ -322,7 +406,8 @@ fft_zy_fused_kernel(const __grid_constant__ TensorMapBlob ring_map, const __grid
                 tma::mbar_wait(&done[s], (unsigned)(n & 1));
                 const int g = item_q[s];
                 if (g < 0) break;
-                FItem it; it.p1 = my_p1; it.x = g / nper; it.j = g - it.x * nper;
+                const int item_z = item_q[2 * NSTAGE + 1 + s];
+                FItem it; it.p1 = FWD ? item_z : !item_z; it.x = item_q[NSTAGE + 1 + s]; it.j = g - it.x * (item_z ? n_z : n_y);
                 if (it.p1 && it.x >= a.R && it.x - a.R > freed) {          // ring slot must have been read out
                     tma::wait_count(&p2_loaded[it.x - a.R], (unsigned)n2);
                     freed = it.x - a.R;
@@ -392,13 +477,26 @@ fft_zy_fused_kernel(const __grid_constant__ TensorMapBlob ring_map, const __grid
             if constexpr (DIR > 0) wt.y = -wt.y;
         }
         const T scale = (T)a.scale;
-        for (int i = gq;; i += NG) {
+        const int mixed = NG == 2 ? a.mixed : 0;
+        int ends = 0;
+        // one role per CTA: group gq takes the CTA's items gq, gq + NG, ...; both roles in the CTA: each group looks at
+        // EVERY item in order (so it observes every phase of every full[] barrier) and takes the ones of its role
+        for (int i = mixed ? 0 : gq;; i += mixed ? 1 : NG) {
             const int s = i % NSTAGE, n = i / NSTAGE;
             C* buf = reinterpret_cast<C*>(stages + s * FT::STAGE_BYTES);
-            while (seen[s] < n) { }                      // the previous phase of this slot has been observed
+            if (!mixed) { while (seen[s] < n) { } }      // the previous phase of this slot has been observed
             tma::mbar_wait(&full[s], (unsigned)(n & 1));
             const int g = item_q[s];
-            if (g < 0) {                                 // end item: pass it on to the slot's store warp
+            if (mixed) {
+                if (g < 0) {                             // end items: the z group hands all NSTAGE of them to the store warps
+                    if (!ISZ) break;
+                    __syncwarp();
+                    if ((tid & 31) == 0) tma::mbar_arrive(&done[s]);
+                    if (++ends == NSTAGE) break;
+                    continue;
+                }
+                if (item_q[2 * NSTAGE + 1 + s] != (ISZ ? 1 : 0)) continue;
+            } else if (g < 0) {                          // end item: pass it on to the slot's store warp
                 if (gt == 0) seen[s] = n + 1;
                 __syncwarp();
                 if ((tid & 31) == 0) tma::mbar_arrive(&done[s]);
@@ -457,7 +555,7 @@ fft_zy_fused_kernel(const __grid_constant__ TensorMapBlob ring_map, const __grid
             if ((tid & 31) == 0) tma::mbar_arrive(&done[s]);
         }
     };
-    if (role_z) consume(TrueT{}); else consume(FalseT{});
+    if ((NG == 2 && a.mixed) ? gq == 0 : role_z) consume(TrueT{}); else consume(FalseT{});
 }
 
 }  // namespace fft3d

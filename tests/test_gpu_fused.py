@@ -161,7 +161,9 @@ def test_fused_options_do_not_change_the_result(fft):
     assert plan.launch_names(0)[0] == "zy_r2c_fused"
     out0 = plan.r2c(f).clone()
     back0 = plan.c2r(out0).clone()
-    for kz, ring in ((2, 8), (146, 8), (0, 8), (84, 2), (40, 3), (100, 5)):
+    for kz, ring in ((2, 8), (146, 8), (0, 8), (84, 2), (40, 3), (100, 5), (-1, 8), (-1, 2), (-1, 3)):
+        plan.set_option(B.OPT_FUSED_MIXED, 1 if kz < 0 else 0)     # kz = -1: both roles in every CTA (the default)
+        kz = max(kz, 0)
         plan.set_option(B.OPT_FUSED_Z_SMS_FWD, kz)
         plan.set_option(B.OPT_FUSED_Z_SMS_INV, kz)
         plan.set_option(B.OPT_FUSED_RING_PLANES, ring)
@@ -170,7 +172,7 @@ def test_fused_options_do_not_change_the_result(fft):
         torch.cuda.synchronize()
         assert torch.equal(torch.view_as_real(out), torch.view_as_real(out0)), (kz, ring)
         assert torch.equal(back, back0), (kz, ring)
-    for opt, val in ((B.OPT_FUSED_RING_PLANES, 1), (B.OPT_FUSED_RING_PLANES, 99), (B.OPT_FUSED_Z_SMS_FWD, 3), (99, 1)):
+    for opt, val in ((B.OPT_FUSED_RING_PLANES, 1), (B.OPT_FUSED_RING_PLANES, 99), (B.OPT_FUSED_Z_SMS_FWD, 3), (B.OPT_FUSED_MIXED, 2), (99, 1)):
         with pytest.raises(B.Fft3dError):
             plan.set_option(opt, val)
     plan.close()
