@@ -76,8 +76,10 @@ enum {
                                  (see fft3d_supported_length)                                 */
     FFT3D_ENOMEM = 3,         /* host or device allocation failed                             */
     FFT3D_ECUDA = 4,          /* no device, launch or runtime error (cudaGetLastError cleared) */
-    FFT3D_EWORKSPACE = 5      /* reserved: workspace too small cannot be detected from a bare
-                                 pointer; callers size it with fft3d_workspace_bytes          */
+    FFT3D_EWORKSPACE = 5      /* fft3d_r2c_static only: the problem needs more scratch than the
+                                 library's built-in array holds.  (With a caller-supplied
+                                 workspace a short buffer cannot be detected from a bare pointer;
+                                 callers size it with fft3d_workspace_bytes.)                 */
 };
 
 /* Create a plan for an Nx x Ny x Nz real grid split into `virtual_slabs` = p x-slabs
@@ -115,6 +117,38 @@ int fft3d_r2c(const fft3d_plan_t *plan, const void *d_real_in, void *d_cplx_out,
  * [Nx][Ny][Nz].  d_real_out may also be used as scratch while the call runs. */
 int fft3d_c2r(const fft3d_plan_t *plan, const void *d_cplx_in, void *d_real_out,
               void *d_work, void *cuda_stream);
+
+/* Forward R2C for callers that cannot allocate device memory.
+ * Everything above needs the CUDA allocator twice: fft3d_plan cudaMalloc's its twiddle tables, and fft3d_r2c wants an
+ * array-sized workspace from the caller.  That shuts out code that has no allocator to turn to -- a plug-in inside an
+ * application whose memory pool claimed the whole card at start-up (a raw cudaMalloc fails there, or is against the
+ * host's rules), the inner loop of a solver or server where cudaMalloc/cudaFree are banned because they stall the whole
+ * device and may fail when the card is full, a process held to a fixed memory budget that owns its input and output
+ * buffers and nothing more.  fft3d_r2c_static serves them: no plan, no workspace argument, and not one call to
+ * cudaMalloc, cudaFree or any other allocating routine.  Its scratch (the Nx*Ny*(Nz/2) complex intermediate array and
+ * four small twiddle tables) is a fixed array of FFT3D_STATIC_SCRATCH_BYTES = 17 MiB compiled into the library image;
+ * each GPU on which the library's code gets loaded carries that 17 MiB until the process exits, used or not.
+ *   Computes exactly what fft3d_plan(Nx,Ny,Nz,dtype,virtual_slabs) + fft3d_r2c compute (Eq. (1), steps 1-5
+ * P:69-77, output in the slab layout above), with the plain-load kernels (the ones fft3d_set_variant(plan, 1) picks):
+ * it is meant for small grids, not for speed.  d_real_in [Nx][Ny][Nz] and d_cplx_out (Nx*Ny*(Nz/2+1) complex) are the
+ * caller's DEVICE buffers on the current device, 16-byte aligned, not overlapping; d_cplx_out doubles as scratch while
+ * the call runs, d_real_in is preserved.  Work is enqueued on cuda_stream (NULL = the legacy default stream); the call
+ * does not wait for it (only the first call with a new shape may block a little: it copies the tables from pageable host
+ * memory, which the runtime orders behind earlier work on that stream).
+ *   LIMIT: Nx*Ny*(Nz/2)*sizeof(complex) plus the tables (a few KiB, at most 256 KiB) must fit the 17 MiB: every grid with
+ * Nx*Ny*Nz*sizeof(real) <= 16 MiB does (128^3 in fp64, 160^3 or 128x128x256 in fp32).  Larger problems get
+ * FFT3D_EWORKSPACE and nothing is launched.  Other errors as for fft3d_plan / fft3d_r2c (FFT3D_EINVAL,
+ * FFT3D_EUNSUPPORTED, FFT3D_ECUDA).
+ *   FIRST CALL ON A DEVICE: looks up where that device keeps the array (and may make the driver load the library's
+ * device code).  Issue it once per device during start-up, with that device current, before any stream capture begins.
+ *   SHARING: one array per device serves every call.  Calls queued on the same stream are fine, whatever their shapes.
+ * Calls whose GPU work can overlap -- two streams, or two host threads on two streams -- write the same scratch and
+ * corrupt each other: serialise them (one stream, or events).  The array is never cleared between calls and need not
+ * be: the intermediate array is written in full before it is read, and the tables are left in place on purpose, so that a
+ * run of calls with one shape uploads them once (a change of shape uploads the new ones, in stream order). */
+#define FFT3D_STATIC_SCRATCH_BYTES ((size_t)17 << 20)
+int fft3d_r2c_static(long long Nx, long long Ny, long long Nz, int dtype, int virtual_slabs,
+                     const void *d_real_in, void *d_cplx_out, void *cuda_stream);
 
 /* 3D complex-to-complex transform (in the paper's library R2C, C2C and C2R share one
  * workspace).  fft3d_plan_c2c creates a plan for an Nx x Ny x Nz COMPLEX grid over p virtual

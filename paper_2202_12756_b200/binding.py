@@ -25,6 +25,7 @@ EXPORTS = (
     "fft3d_plan_inplace", "fft3d_r2c_inplace", "fft3d_c2r_inplace", "fft3d_plan_pencil",
     "fft3d_plan_dist", "fft3d_dist_bytes", "fft3d_dist_fwd_local", "fft3d_dist_fwd_x", "fft3d_dist_fwd_col0",
     "fft3d_dist_fwd_unpack", "fft3d_dist_inv_planes", "fft3d_dist_inv_pack", "fft3d_dist_inv_x", "fft3d_dist_inv_local",
+    "fft3d_r2c_static",
     "fft3d_vmm_granularity", "fft3d_vmm_create", "fft3d_vmm_import", "fft3d_vmm_map", "fft3d_vmm_unmap", "fft3d_vmm_release",
 )
 
@@ -71,6 +72,8 @@ def load_library() -> ctypes.CDLL:
     for nm in ("fft3d_r2c_host", "fft3d_c2r_host"):
         getattr(lib, nm).argtypes = [vp, vp, vp]
         getattr(lib, nm).restype = i
+    lib.fft3d_r2c_static.argtypes = [ll, ll, ll, i, i, vp, vp, vp]
+    lib.fft3d_r2c_static.restype = i
     lib.fft3d_launches.argtypes = [vp, i]
     lib.fft3d_launches.restype = i
     lib.fft3d_launch_name.argtypes = [vp, i, i]
@@ -133,6 +136,33 @@ def supported_length(n: int) -> bool:
 
 _REAL = {F32: torch.float32, F64: torch.float64}
 _CPLX = {F32: torch.complex64, F64: torch.complex128}
+
+STATIC_SCRATCH_BYTES = 17 << 20
+
+
+def r2c_static(real_in: torch.Tensor, cplx_out: torch.Tensor, virtual_slabs: int = 1, stream=None) -> torch.Tensor:
+    """fft3d_r2c_static: forward R2C of ``real_in`` [Nx][Ny][Nz] into ``cplx_out`` (flat, Nx*Ny*(Nz/2+1) complex, slab
+    layout) for callers that cannot allocate device memory -- code living inside someone else's memory pool, or inside a
+    loop where cudaMalloc/cudaFree are off limits.  No plan and no workspace: the library's own 17 MiB built-in scratch
+    array is used, so both tensors must be supplied by the caller (this wrapper allocates nothing either) and the grid
+    must be small enough (Nx*Ny*Nz*sizeof(real) <= 16 MiB always fits; otherwise Fft3dError with status 5).  Calls on
+    one stream are ordered; calls that can overlap on the GPU share the scratch and corrupt each other."""
+    lib = load_library()
+    if not (real_in.is_cuda and real_in.is_contiguous() and real_in.dim() == 3 and real_in.dtype in (torch.float32, torch.float64)):
+        raise ValueError("real_in must be a contiguous 3-D CUDA tensor of float32 or float64")
+    Nx, Ny, Nz = (int(v) for v in real_in.shape)
+    code = F32 if real_in.dtype == torch.float32 else F64
+    if not (cplx_out.is_cuda and cplx_out.is_contiguous() and cplx_out.device == real_in.device and
+            cplx_out.dtype == _CPLX[code] and cplx_out.numel() == Nx * Ny * (Nz // 2 + 1)):
+        raise ValueError("cplx_out must be a contiguous %s CUDA tensor of %d elements on %s"
+                         % (_CPLX[code], Nx * Ny * (Nz // 2 + 1), real_in.device))
+    s = stream if stream is not None else torch.cuda.current_stream(real_in.device)
+    with torch.cuda.device(real_in.device):
+        rc = lib.fft3d_r2c_static(Nx, Ny, Nz, code, int(virtual_slabs), real_in.data_ptr(), cplx_out.data_ptr(),
+                                  ctypes.c_void_p(s.cuda_stream))
+    if rc != 0:
+        raise Fft3dError(rc, "fft3d_r2c_static(%d,%d,%d,p=%d)" % (Nx, Ny, Nz, virtual_slabs))
+    return cplx_out
 
 
 class Plan:
