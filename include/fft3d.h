@@ -320,8 +320,12 @@ int fft3d_set_variant(fft3d_plan_t *plan, int variant);
  *                            its load warp dealing the ring slots to the two streams; 0: one role per CTA
  *   FUSED_Z_SMS_FWD / _INV   with one role per CTA: SMs [0, value) run the z tiles, the others the y tiles (even;
  *                            0 = alternate CTA pairs)
- *   FUSED_RING_PLANES        yz-planes in the L2 ring (2 .. the number the workspace was sized for) */
-enum { FFT3D_OPT_FUSED_Z_SMS_FWD = 1, FFT3D_OPT_FUSED_Z_SMS_INV = 2, FFT3D_OPT_FUSED_RING_PLANES = 3, FFT3D_OPT_FUSED_MIXED = 4 };
+ *   FUSED_RING_PLANES        yz-planes in the L2 ring (2 .. the number the workspace was sized for)
+ *   FUSED_JITTER             stress testing only: every CTA's load warp pauses a pseudo-random 0..value ns (value <= 10^6)
+ *                            before each tile, which scrambles the order in which tiles are drawn and taken; the pipeline
+ *                            must neither stall nor change a bit of the result.  0 (default) = off */
+enum { FFT3D_OPT_FUSED_Z_SMS_FWD = 1, FFT3D_OPT_FUSED_Z_SMS_INV = 2, FFT3D_OPT_FUSED_RING_PLANES = 3, FFT3D_OPT_FUSED_MIXED = 4,
+       FFT3D_OPT_FUSED_JITTER = 5 };
 int fft3d_set_option(fft3d_plan_t *plan, int option, long long value);
 
 int fft3d_destroy(fft3d_plan_t *plan);          /* NULL is accepted */

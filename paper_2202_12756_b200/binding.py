@@ -12,7 +12,7 @@ import os
 import torch
 
 F32, F64 = 0, 1
-OPT_FUSED_Z_SMS_FWD, OPT_FUSED_Z_SMS_INV, OPT_FUSED_RING_PLANES, OPT_FUSED_MIXED = 1, 2, 3, 4
+OPT_FUSED_Z_SMS_FWD, OPT_FUSED_Z_SMS_INV, OPT_FUSED_RING_PLANES, OPT_FUSED_MIXED, OPT_FUSED_JITTER = 1, 2, 3, 4, 5
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libfft3d.so")
 

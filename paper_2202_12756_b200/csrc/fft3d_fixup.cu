@@ -20,6 +20,17 @@ struct PlaneArgs {
     int Nx, Ny, L, M;
 };
 
+// grid cap of the plane-sized grid-stride kernels below: 16 blocks of 256 threads per SM of the current device
+static long long grid_cap() {
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess ||
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms < 1) {
+        cudaGetLastError();
+        sms = 148;                                    // B200
+    }
+    return (long long)sms * 16;
+}
+
 __device__ __forceinline__ long long slab_row(int kx, int ky, int Nx, int L) {
     const int q = ky / L, l = ky - q * L;
     return ((long long)q * Nx + kx) * L + l;
@@ -142,7 +153,7 @@ template <typename T>
 static cudaError_t run_dist(void (*k)(const DistPlaneArgs), const DistPlaneArgs& a, cudaStream_t st) {
     const long long n = (long long)a.Nx * a.L * (a.ncols > 0 ? a.ncols : 1);
     long long blocks = (n + 255) / 256;
-    if (blocks > 148 * 16) blocks = 148 * 16;
+    if (blocks > grid_cap()) blocks = grid_cap();
     k<<<(unsigned)blocks, 256, 0, st>>>(a);
     return cudaGetLastError();
 }
@@ -161,7 +172,7 @@ template <typename T>
 static cudaError_t run(void (*k)(const PlaneArgs), const PlaneArgs& a, cudaStream_t st) {
     const long long n = (long long)a.Nx * a.Ny;
     long long blocks = (n + 255) / 256;
-    if (blocks > 148 * 16) blocks = 148 * 16;
+    if (blocks > grid_cap()) blocks = grid_cap();
     k<<<(unsigned)blocks, 256, 0, st>>>(a);
     return cudaGetLastError();
 }
@@ -212,7 +223,7 @@ __global__ void pencil_convert_kernel(const PencilArgs a) {
 }
 
 cudaError_t launch_pencil_convert(int dtype, const PencilArgs& a, cudaStream_t st) {
-    long long blocks = a.nrows < 148 * 16 ? a.nrows : 148 * 16;
+    long long blocks = a.nrows < grid_cap() ? a.nrows : grid_cap();
     if (dtype == 0) pencil_convert_kernel<float><<<(unsigned)blocks, 256, 0, st>>>(a);
     else pencil_convert_kernel<double><<<(unsigned)blocks, 256, 0, st>>>(a);
     return cudaGetLastError();

@@ -119,6 +119,7 @@ struct fft3d_plan_s {
     int fz_kz[2];              // [fwd, inv] SMs [0, kz) run the z tiles, the others the y tiles (0: split by CTA pairs)
     int fz_mixed;              // 1: every CTA runs both roles (one consumer group each); needs two consumer groups
     int fz_R_max;              // ring planes the workspace was sized for
+    int fz_jitter;             // stress option: max pause (ns) of the load warps before each item, 0 = off
     size_t slab_bytes, ring_bytes, side_bytes, flags_bytes;
     // Sub-ranges the passes work on.  A plain plan covers the whole problem; the stage entry points of a
     // distributed plan (fft3d_dist_*) run the same launch code on a copy of the plan with these narrowed.
@@ -323,6 +324,7 @@ int launch_fused(const fft3d_plan_s* pl, int d, const void* in, void* out, void*
     a.Nx = (int)pl->xpn; a.Ny = (int)pl->Ny; a.L = (int)pl->L; a.R = pl->fz_R; a.kz = pl->fz_kz[d];
     a.mixed = (pl->fz_mixed && (c2c ? ky->fc_ng : ky->fz_ng) == 2) ? 1 : 0;
     a.rows_slab = pl->y_rows_slab;
+    a.jitter = pl->fz_jitter;
     a.scale = 1.0 / ((double)pl->Nx * (double)pl->Ny * (double)pl->Nz);
     void* argv[3] = {(void*)&ring_map, (void*)&slab_map, (void*)&a};
     cudaError_t e = cudaLaunchCooperativeKernel(fn, dim3((unsigned)pl->num_sms), dim3((unsigned)f_threads), argv, f_smem, st);
@@ -805,6 +807,10 @@ int fft3d_set_option(fft3d_plan_t* pl, int option, long long value) {
             if (value != 0 && value != 1) return FFT3D_EINVAL;
             pl->fz_mixed = (int)value;
             return FFT3D_OK;
+        case FFT3D_OPT_FUSED_JITTER:
+            if (value < 0 || value > 1000000) return FFT3D_EINVAL;
+            pl->fz_jitter = (int)value;
+            return FFT3D_OK;
         case FFT3D_OPT_FUSED_RING_PLANES:
             if (!pl->fused || value < 2 || value > pl->fz_R_max || value > pl->Nx) return FFT3D_EINVAL;
             pl->fz_R = (int)value;
@@ -1165,6 +1171,12 @@ int fft3d_plan_dist(fft3d_plan_t** out, long long Nx, long long Ny, long long Nz
     fft3d_plan_t* pl = *out;
     pl->dist_G = G; pl->dist_rank = rank;
     const long long Nxl = Nx / G;
+    // plan_create judged the bulk-pipelined z kernel on the rows of the WHOLE grid; the stages run it on the local slab's
+    // (Nx/G)*Ny rows, which must be whole tiles too (otherwise: plain-load z kernel, and no fused z+y pass, which needs it)
+    if (pl->bulk_z && (Nxl * Ny) % pl->kz->zb_rpt != 0) {
+        pl->bulk_z = false;
+        pl->fused = pl->fused_default = false;
+    }
     if (pl->fused) {
         // the ring holds planes of the local x-slab only; fusion pays once the LOCAL arrays are far larger than L2
         if (Nxl < 2) pl->fused = pl->fused_default = false;
@@ -1233,6 +1245,8 @@ int fft3d_dist_fwd_x(const fft3d_plan_t* pl, const void* d_slab_part, void* d_sp
 
 static int dist_planes(const fft3d_plan_t* pl, const void* d_spec_part, void* d_plane_part, int ncols, void* stream) {
     if (pl == nullptr || pl->dist_G == 0 || d_spec_part == nullptr || d_plane_part == nullptr) return FFT3D_EINVAL;
+    if (wrong_device(pl)) return FFT3D_EINVAL;          // the current device is not the plan's
+    if (((uintptr_t)d_spec_part | (uintptr_t)d_plane_part) & 15) return FFT3D_EINVAL;
     DistPlaneArgs a{};
     a.spec = d_spec_part; a.own = d_plane_part;
     a.Nx = (int)pl->Nx; a.Ny = (int)pl->Ny; a.L = (int)pl->L; a.M = (int)pl->M; a.q = pl->dist_rank; a.ncols = ncols;
@@ -1249,8 +1263,7 @@ int fft3d_dist_inv_planes(const fft3d_plan_t* pl, const void* d_spec_part, void*
 int fft3d_dist_fwd_unpack(const fft3d_plan_t* pl, void* d_spec_part, const void* const* d_plane_parts, void* stream) {
     if (pl == nullptr || pl->dist_G == 0 || d_spec_part == nullptr || d_plane_parts == nullptr) return FFT3D_EINVAL;
     if (wrong_device(pl)) return FFT3D_EINVAL;          // the current device is not the plan's
-    if (wrong_device(pl)) return FFT3D_EINVAL;          // the current device is not the plan's
-    if (wrong_device(pl)) return FFT3D_EINVAL;          // the current device is not the plan's
+    if ((uintptr_t)d_spec_part & 15) return FFT3D_EINVAL;
     DistPlaneArgs a{};
     a.spec_out = d_spec_part;
     for (int q = 0; q < pl->dist_G; ++q) { if (d_plane_parts[q] == nullptr) return FFT3D_EINVAL; a.parts[q] = d_plane_parts[q]; }
@@ -1467,7 +1480,8 @@ static int ensure_host_buffers(fft3d_plan_t* pl) {
 }
 
 int fft3d_r2c_host(fft3d_plan_t* pl, const void* h_in, void* h_out) {
-    if (pl == nullptr || pl->kind != 0 || h_in == nullptr || h_out == nullptr) return FFT3D_EINVAL;
+    // in-place and distributed plans have no host-buffer form: refuse them before any device buffer is allocated
+    if (pl == nullptr || pl->kind != 0 || pl->inplace || pl->dist_G != 0 || h_in == nullptr || h_out == nullptr) return FFT3D_EINVAL;
     if (wrong_device(pl)) return FFT3D_EINVAL;          // the current device is not the plan's
     int rc = ensure_host_buffers(pl);
     if (rc != FFT3D_OK) return rc;
@@ -1487,7 +1501,8 @@ int fft3d_r2c_host(fft3d_plan_t* pl, const void* h_in, void* h_out) {
 }
 
 int fft3d_c2r_host(fft3d_plan_t* pl, const void* h_in, void* h_out) {
-    if (pl == nullptr || pl->kind != 0 || h_in == nullptr || h_out == nullptr) return FFT3D_EINVAL;
+    // in-place and distributed plans have no host-buffer form: refuse them before any device buffer is allocated
+    if (pl == nullptr || pl->kind != 0 || pl->inplace || pl->dist_G != 0 || h_in == nullptr || h_out == nullptr) return FFT3D_EINVAL;
     if (wrong_device(pl)) return FFT3D_EINVAL;          // the current device is not the plan's
     int rc = ensure_host_buffers(pl);
     if (rc != FFT3D_OK) return rc;

@@ -39,7 +39,15 @@
 // y tiles, and the load warp deals the ring slots to the two streams -- a phase-2 tile when its plane is complete, a
 // phase-1 tile otherwise, alternating when both are possible; phase-1 tiles never hold all the slots (their stores may
 // wait for the ring's back-pressure, which only phase-2 loads relieve) and are not taken a ring's depth ahead of the
-// phase-2 tickets.  Both groups look at every item in order and take the ones of their role.  Every SM then carries
+// phase-2 tickets.  One exception keeps the mixed pipeline live: a CTA whose phase-2 ticket waits for plane x2 takes its
+// phase-1 ticket of a plane <= x2 even into its last free slot (that very tile may be what plane x2 is waiting for, and
+// the slot count is only refreshed between items).  Liveness: take the lowest phase-2 ticket not yet loaded, plane xm.
+// Every phase-1 tile of xm is either in some CTA's slot -- its store waits for plane xm-R to be read out, i.e. for
+// phase-2 tickets below the lowest outstanding one: all loaded -- or is the un-taken phase-1 ticket of a CTA D, and then
+// xm <= D's x2, so D takes it as soon as it has a free slot; D's slots hold phase-1 tiles of planes <= xm (tickets are
+// drawn in order), whose stores likewise wait only for the read-out of planes <= xm - R (all loaded), or phase-2 tiles,
+// which wait for nothing.  So plane xm completes, its holder takes the ticket, and the minimum advances.
+// Both groups look at every item in order and take the ones of their role.  Every SM then carries
 // the same mix of compute-heavy z tiles and latency-heavy y tiles, and no SM split has to be tuned
 // (measured at 1024^3: forward 2.57 -> 2.49 ms, inverse 2.82 -> 2.76 ms on the same box).
 //
@@ -81,6 +89,9 @@ struct FusedArgs {
     double scale;            // inverse: 1/(Nx Ny Nz)
     int kz;                  // SMs [0, kz) take the z tiles (0: split by CTA pairs)
     int mixed;               // 1: every CTA runs both roles (consumer group 0 the z tiles, group 1 the y tiles)
+    int jitter;              // > 0: stress option -- every load warp sleeps a pseudo-random 0..jitter ns before each item,
+                             // which scrambles the order in which the CTAs draw and take their tiles (results and
+                             // liveness must not depend on that order); 0 in normal use
 };
 
 namespace tma {
@@ -117,6 +128,14 @@ __device__ __forceinline__ void prefetch_l2(const void* src, unsigned bytes, uns
     asm volatile("cp.async.bulk.prefetch.L2.global.L2::cache_hint [%0], %1, %2;" ::"l"(src), "r"(bytes), "l"(pol) : "memory");
 }
 __device__ __forceinline__ void fence_proxy_async_all() { asm volatile("fence.proxy.async;" ::: "memory"); }
+}  // namespace tma
+// stress option of the fused pipeline (FusedArgs::jitter): a pseudo-random pause of up to max_ns in a load warp
+__device__ __forceinline__ void jitter_sleep(int max_ns, int i) {
+    unsigned h = (unsigned)clock64() * 2654435761u ^ (blockIdx.x * 40503u + (unsigned)i * 977u);
+    h ^= h >> 15; h *= 2246822519u; h ^= h >> 13;
+    __nanosleep(h % (unsigned)max_ns);
+}
+namespace tma {
 __device__ __forceinline__ unsigned ld_acquire(const unsigned* p) {
     unsigned v;
     asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
@@ -204,15 +223,18 @@ fft_zy_fused_kernel(const __grid_constant__ TensorMapBlob ring_map, const __grid
     // seen[s] = number of phases of full[s] a consumer group has observed complete.  A slot is used by
     // the groups in turn (NSTAGE need not be a multiple of NG) and a parity wait is only meaningful
     // within one phase of the barrier's current one, so a group polls seen[s] before it waits for ITS phase.
+    // Both roles in the CTA: every group waits on every phase, and seen[g * NSTAGE + s] counts the phases group g has
+    // observed; the load warp refills slot s only when BOTH groups have observed its previous phase (a group that only
+    // skips the item does not hold the slot otherwise, and a parity wait two phases late would alias).
     volatile int* seen = reinterpret_cast<volatile int*>(empty + NSTAGE);
-    volatile int* role_s = seen + NSTAGE;                // [role_z] broadcast from thread 0
+    volatile int* role_s = seen + 2 * NSTAGE;            // [role_z] broadcast from thread 0
     volatile int* item_q = role_s + 4;                   // [s] global tile index in slot s (-1: no more tiles), [NSTAGE] first end item, [NSTAGE+1+s] its plane, [2 NSTAGE+1+s] 1 = a z tile
 
     const int tid = threadIdx.x;
     if (tid == NCONS) {
         for (int s = 0; s < NSTAGE; ++s) {
             tma::mbar_init(&full[s], 1); tma::mbar_init(&done[s], GROUP / 32); tma::mbar_init(&empty[s], 1);
-            seen[s] = 0;
+            seen[s] = 0; seen[NSTAGE + s] = 0;
         }
         item_q[NSTAGE] = -1;
         tma::fence_mbar_init();
@@ -304,6 +326,7 @@ fft_zy_fused_kernel(const __grid_constant__ TensorMapBlob ring_map, const __grid
                 unsigned p1mask = 0;                     // bit s: the item in slot s is a phase-1 tile
                 for (int i = 0;; ++i) {
                     const int s = i % NSTAGE, n = i / NSTAGE;
+                    if (a.jitter > 0) jitter_sleep(a.jitter, i);
                     // the readiness of the next phase-2 ticket's plane is read BEFORE the wait for the slot (an L2 round
                     // trip that would otherwise sit between the slot becoming free and its next load)
                     if (g2 < tot2) {
@@ -312,6 +335,7 @@ fft_zy_fused_kernel(const __grid_constant__ TensorMapBlob ring_map, const __grid
                     }
                     if (n > 0) {
                         tma::mbar_wait(&empty[s], (unsigned)((n - 1) & 1));
+                        while (seen[s] < n || seen[NSTAGE + s] < n) { }      // both groups have observed the slot's last phase
                         inflight1 -= (int)((p1mask >> s) & 1u);
                         p1mask &= ~(1u << s);
                     }
@@ -329,7 +353,13 @@ fft_zy_fused_kernel(const __grid_constant__ TensorMapBlob ring_map, const __grid
                             tma::fence_proxy_async_all(); ready = x2; can2 = true;
                         }
                         if (can2) { take = 2; break; }
-                        if (can1) { take = 1; break; }
+                        // LIVENESS: `inflight1` is only re-counted at the top of an iteration, so `can1` can stay false
+                        // for the whole poll loop -- and the plane this CTA's phase-2 ticket waits for may be incomplete
+                        // precisely because of the phase-1 ticket this CTA is holding back.  Such a ticket (plane <= x2)
+                        // is taken whatever the slot count: its store waits only for phase-2 loads of plane
+                        // (g1/n1 - R) < x2, i.e. for tickets below this CTA's g2, which other CTAs hold and which depend
+                        // on lower planes only -- the induction of the header still closes.
+                        if (can1 || (has1 && g1 / n1 <= x2)) { take = 1; break; }
                         if (polls > 0) __nanosleep(64);
                         if (++polls > (1u << 24)) __trap();
                     }
@@ -366,6 +396,7 @@ fft_zy_fused_kernel(const __grid_constant__ TensorMapBlob ring_map, const __grid
             int g = (int)atomicAdd(next, 1u);            // the next tile of this role, in order
             for (;;) {
                 const int s = i % NSTAGE, n = i / NSTAGE;
+                if (a.jitter > 0) jitter_sleep(a.jitter, i);
                 if (n > 0) tma::mbar_wait(&empty[s], (unsigned)((n - 1) & 1));
                 if (g >= total) {                        // NSTAGE end items: every group and every store warp sees one
                     if (item_q[NSTAGE] < 0) item_q[NSTAGE] = i;
@@ -487,6 +518,7 @@ fft_zy_fused_kernel(const __grid_constant__ TensorMapBlob ring_map, const __grid
             if (!mixed) { while (seen[s] < n) { } }      // the previous phase of this slot has been observed
             tma::mbar_wait(&full[s], (unsigned)(n & 1));
             const int g = item_q[s];
+            if (mixed && gt == 0) seen[gq * NSTAGE + s] = n + 1;
             if (mixed) {
                 if (g < 0) {                             // end items: the z group hands all NSTAGE of them to the store warps
                     if (!ISZ) break;
@@ -505,7 +537,7 @@ fft_zy_fused_kernel(const __grid_constant__ TensorMapBlob ring_map, const __grid
             }
             // (kept free of branches: a lane that leaves its warp here would stay apart for the whole tile body,
             //  and the body's warp shuffles then take the slow path for diverged warps)
-            if (gt == 0) seen[s] = n + 1;
+            if (!mixed && gt == 0) seen[s] = n + 1;
             if constexpr (!P1) {
                 // the ring tile has landed in shared memory (complete_tx observed): nothing of it can be read any
                 // later, so a relaxed increment is enough to let the ring slot be overwritten

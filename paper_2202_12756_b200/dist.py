@@ -15,7 +15,10 @@ from __future__ import annotations
 
 import ctypes
 import os
+import shutil
 import socket
+import stat
+import tempfile
 
 import torch
 
@@ -154,16 +157,38 @@ def all_gather_parts(dist, part, gathered, group=None):
 # ------------------------------------------------------------------------------------------------------------------
 # UNIFIED exchange array over CUDA VMM
 # ------------------------------------------------------------------------------------------------------------------
-def exchange_fds(rank, world, fd, tag, barrier):
+def private_socket_dir(dist, group=None):
+    """A directory only this user can enter (mkdtemp: mode 0700, unpredictable name), made by rank 0 and announced to the
+    group; also checks that every rank runs on rank 0's host -- descriptors travel over Unix sockets and the mapped
+    memory over NVLink peer access: both are single-node mechanisms.  Rank 0 removes the directory after use
+    (remove_socket_dir)."""
+    rank = dist.get_rank(group)
+    hosts = [None] * dist.get_world_size(group)
+    dist.all_gather_object(hosts, socket.gethostname(), group=group)
+    if len(set(hosts)) != 1:
+        raise RuntimeError("the UNIFIED exchange maps peer memory of ONE node; ranks run on %s: use exchange='chunks'"
+                           % sorted(set(hosts)))
+    box = [tempfile.mkdtemp(prefix="fft3d_xchg_") if rank == 0 else None]
+    dist.broadcast_object_list(box, src=dist.get_global_rank(group, 0) if group is not None else 0, group=group)
+    return box[0]
+
+
+def remove_socket_dir(path, rank):
+    if rank == 0:
+        shutil.rmtree(path, ignore_errors=True)
+
+
+def exchange_fds(rank, world, fd, sockdir, barrier):
     """Every rank hands its file descriptor to every other rank over Unix sockets (SCM_RIGHTS).  Returns the list of
-    descriptors in rank order (own entry = fd).  `barrier()` must synchronise the ranks; `tag` names the sockets."""
-    path = "/tmp/fft3d_%s_%d.sock"
+    descriptors in rank order (own entry = fd).  `barrier()` must synchronise the ranks.  The sockets live in `sockdir`,
+    which must belong to this user and be closed to everybody else (private_socket_dir): whoever can reach a socket
+    receives a handle to GPU memory, and whoever can replace one can inject a handle of its own."""
+    st = os.stat(sockdir)
+    if not stat.S_ISDIR(st.st_mode) or st.st_uid != os.geteuid() or (st.st_mode & 0o077) != 0:
+        raise PermissionError("%s must be a directory owned by this user with mode 0700" % sockdir)
+    path = os.path.join(sockdir, "rank_%d.sock")
     srv = socket.socket(socket.AF_UNIX, socket.SOCK_STREAM)
-    try:
-        os.unlink(path % (tag, rank))
-    except FileNotFoundError:
-        pass
-    srv.bind(path % (tag, rank))
+    srv.bind(path % rank)
     srv.listen(world)
     barrier()                                            # every server socket exists
     out = [None] * world
@@ -176,7 +201,7 @@ def exchange_fds(rank, world, fd, tag, barrier):
         peer = (rank + r) % world
         c = socket.socket(socket.AF_UNIX, socket.SOCK_STREAM)
         c.settimeout(60.0)
-        c.connect(path % (tag, peer))
+        c.connect(path % peer)
         clients.append((peer, c))
     while pending:
         conn, _ = srv.accept()
@@ -190,7 +215,7 @@ def exchange_fds(rank, world, fd, tag, barrier):
     barrier()
     srv.close()
     try:
-        os.unlink(path % (tag, rank))
+        os.unlink(path % rank)
     except FileNotFoundError:
         pass
     return out
@@ -200,7 +225,7 @@ class UnifiedExchange:
     """G device allocations mapped back to back into one virtual range: part q = rank q's memory.
 
     single-process form (tests, EmulatedRanks): UnifiedExchange.local(G, part_bytes) creates all G parts on the
-    current device; multi-process form: UnifiedExchange.across(rank, world, part_bytes, barrier) creates the own
+    current device; multi-process form: UnifiedExchange.across(rank, world, part_bytes, dist, group) creates the own
     part, passes descriptors, imports the peers' parts."""
 
     def __init__(self, handles, part_bytes, own):
@@ -231,13 +256,17 @@ class UnifiedExchange:
         return cls(hs, part_bytes, own=list(range(G)))
 
     @classmethod
-    def across(cls, rank, world, part_bytes, barrier, tag="x"):
+    def across(cls, rank, world, part_bytes, dist, group=None):
         lib = B.load_library()
+        sockdir = private_socket_dir(dist, group)        # also: all ranks on one host, or it raises
         h, fd = ctypes.c_ulonglong(), ctypes.c_int(-1)
         rc = lib.fft3d_vmm_create(part_bytes, ctypes.byref(h), ctypes.byref(fd))
         if rc != 0:
             raise B.Fft3dError(rc, "fft3d_vmm_create")
-        fds = exchange_fds(rank, world, fd.value, "%s_%d" % (tag, os.getppid()), barrier)
+        try:
+            fds = exchange_fds(rank, world, fd.value, sockdir, lambda: dist.barrier(group=group))
+        finally:
+            remove_socket_dir(sockdir, rank)
         hs = []
         for q in range(world):
             if q == rank:
@@ -297,7 +326,7 @@ class SlabFFT:
             part = p.nbytes(DIST_SLAB)
             if not UnifiedExchange.usable(part):
                 raise ValueError("part size %d is not a multiple of the VMM granularity: use exchange='chunks'" % part)
-            self.ux = UnifiedExchange.across(self.rank, self.G, part, lambda: dist.barrier(group=group))
+            self.ux = UnifiedExchange.across(self.rank, self.G, part, dist, group)
         elif exchange == "chunks":
             self.send = torch.empty((self.G,) + chunk_shape(Nx, Ny, Nz, self.G), dtype=p.complex_dtype, device=device)
             self.recv = torch.empty_like(self.send)

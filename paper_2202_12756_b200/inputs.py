@@ -192,9 +192,3 @@ def complex_grid(shape, dtype=torch.complex64, seed=0, device="cpu") -> torch.Te
     flat = _fill((Nx * Ny * Nz, 2), rdt, device,
                  lambda a, b: 2.0 * _uniform01(a, b, seed, 9, device) - 1.0, chunk=1 << 24)
     return torch.view_as_complex(flat).reshape(Nx, Ny, Nz)
-
-
-def index_tag_grid(shape, dtype=torch.float64, device="cpu") -> torch.Tensor:
-    """Each element carries its own linear index (layout tests)."""
-    n = int(np.prod(shape))
-    return torch.arange(n, dtype=torch.float64, device=device).to(dtype).reshape(shape)

@@ -131,7 +131,20 @@ def _worker(rank, world, port, shape, q):
     fft.inverse(S[:, rank * L:(rank + 1) * L, :].contiguous(), back)
     # descriptor hand-off of the UNIFIED exchange: each rank passes a pipe's read end to the other
     r_fd, w_fd = os.pipe()
-    fds = D.exchange_fds(rank, world, r_fd, "test%d" % port, lambda: dist.barrier())
+    sockdir = D.private_socket_dir(dist)
+    assert os.stat(sockdir).st_mode & 0o777 == 0o700
+    fds = D.exchange_fds(rank, world, r_fd, sockdir, lambda: dist.barrier())
+    D.remove_socket_dir(sockdir, rank)
+    if rank == 0:                                          # a directory other users could enter is refused
+        import tempfile
+        loose = tempfile.mkdtemp()
+        os.chmod(loose, 0o755)
+        try:
+            D.exchange_fds(rank, 1, r_fd, loose, lambda: None)
+            raise AssertionError("exchange_fds accepted a world-accessible socket directory")
+        except PermissionError:
+            pass
+        os.rmdir(loose)
     os.write(w_fd, (b"rank%d" % rank) * (world - 1))       # one 5-byte message for each peer that holds the read end
     got = [os.read(fd, 5).decode() if k != rank else None for k, fd in enumerate(fds)]
     dist.barrier()

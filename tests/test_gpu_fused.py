@@ -197,3 +197,36 @@ def test_fused_with_fewer_tiles_than_ctas(fft, oracle_mod):
     assert err <= bound
     assert (back.cpu() - f).abs().max().item() <= bound
     plan.close()
+
+
+@pytest.mark.parametrize("shape", [(32, 1024, 1024), (24, 512, 512)])
+def test_fused_pipeline_is_live_and_bit_identical_under_jitter(fft, shape):
+    """Liveness of the dealt pipelines must not depend on timing.  FFT3D_OPT_FUSED_JITTER makes every load warp pause a
+    pseudo-random time before each item, which scrambles the order in which the 148 CTAs draw and take their tiles (at
+    1024 x 1024 planes, 128 phase-1 and 64 phase-2 tiles per plane on a 3-slot ring: the configuration in which a CTA could
+    hold back the very phase-1 ticket its phase-2 ticket was waiting for).  A stall would end in the kernels' bounded spins
+    (__trap, a CUDA error here); the result must stay the same to the bit, in both role modes and both directions."""
+    from paper_2202_12756_b200 import inputs
+    B = fft.binding
+    f = inputs.uniform_grid(shape, torch.float32, seed=41).cuda()
+    plan = fft.Plan(*shape, dtype=torch.float32, virtual_slabs=8)
+    plan.set_variant(3)
+    assert plan.launch_impls(0)[0] == "fused_ring" and plan.launch_impls(1)[-1] == "fused_ring"
+    work = plan.empty_workspace("cuda")
+    out0 = plan.r2c(f, work=work).clone()
+    back0 = plan.c2r(out0, work=work).clone()
+    out, back = plan.empty_complex("cuda"), plan.empty_real("cuda")
+    for mixed in (1, 0):
+        plan.set_option(B.OPT_FUSED_MIXED, mixed)
+        for jitter in (300, 2000, 20000, 150000):
+            plan.set_option(B.OPT_FUSED_JITTER, jitter)
+            for _ in range(3):
+                plan.r2c(f, out, work)
+                plan.c2r(out0, back, work)
+                torch.cuda.synchronize()
+                assert torch.equal(torch.view_as_real(out), torch.view_as_real(out0)), (mixed, jitter)
+                assert torch.equal(back, back0), (mixed, jitter)
+    with pytest.raises(B.Fft3dError):
+        plan.set_option(B.OPT_FUSED_JITTER, -1)
+    plan.set_option(B.OPT_FUSED_JITTER, 0)
+    plan.close()
