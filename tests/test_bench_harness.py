@@ -87,3 +87,14 @@ def test_reference_arm_under_torchrun_prints_one_line():
     assert d["cpu_baseline"]["kind"] == "oracle" and d["cpu_baseline"]["value"] == d["value"] > 0
     assert d["e2e"] == {"value": d["value"], "unit": "GFLOP/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}
     assert d["higher_is_better"] is True and d["vs_baseline"] is None
+
+
+def test_gpus_must_match_the_launchers_world_size():
+    """`bench.py --gpus 4` started as a single process must not print an n_gpus = 1 line: it exits non-zero and says how
+    to launch it (the driver starts N > 1 under torchrun, which sets WORLD_SIZE)."""
+    env = {k: v for k, v in os.environ.items() if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK")}
+    res = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "4", "--steps", "1"],
+                         capture_output=True, text=True, timeout=300, env=env, cwd=ROOT)
+    assert res.returncode != 0
+    assert "torch.distributed.run" in res.stderr and "--nproc-per-node 4" in res.stderr
+    assert not [ln for ln in res.stdout.splitlines() if ln.startswith("{")]

@@ -39,10 +39,15 @@ CASES = [
     ((32, 32, 16), 2),           # rows shorter than 1 KiB: the plain-load row kernel
     ((16, 24, 64), 4),
     ((12, 20, 28), 2),           # radix 3, 5 and 7 lengths, Nz not a multiple of the bulk tile
-    ((6, 10, 40), 2),
+    ((6, 20, 40), 2),
     ((64, 64, 96), 8),
-    ((10, 6, 1024), 2),          # long rows, but Nx*Ny = 60 is not a whole number of 8-row tiles: plain rows
+    ((20, 6, 1024), 2),
+    ((6, 6, 128), 2),            # rows of >= 1 KiB, but Nx*Ny = 36 rows are not whole 16- or 32-row tiles: plain-load rows
+    ((6, 6, 256), 3),
 ]
+
+
+PLAIN_ROWS = {(6, 6, 128), (6, 6, 256), (32, 32, 16), (12, 20, 28)}
 
 
 @pytest.mark.parametrize("shape,p", CASES)
@@ -61,6 +66,8 @@ def test_c2c_matches_oracle(fft, oracle_mod, shape, p, dtype, variant):
         plan.close()
         pytest.skip("no fused C2C kernels for %s %s" % (shape, dtype))
     assert fused == (variant == 3)
+    if shape in PLAIN_ROWS:          # the path these cases were written for must be the one that runs
+        assert plan.launch_impls(0)[0] == "plain" and plan.launch_impls(1)[2] == "plain", plan.launch_impls(0)
     cd = plan.complex_dtype
     f = inputs.complex_grid(shape, cd, seed=11)
     d_in = f.cuda().reshape(-1)

@@ -85,7 +85,10 @@ def check_forward_pencils(oracle_mod, plan, field_host, spec, dtype, n_random=3,
     Nx, Ny, Nz = plan.shape
     rng = np.random.Generator(np.random.PCG64(seed))
     pairs = [(0, 0), (Ny // 2, Nz // 2), (1, Nz // 2 - 1), (Ny - 1, 0)]
-    if classes:
+    if classes == "few":           # 2048^3, where a pencil costs the oracle ~10 s: one row of every class l % 4, with the
+        cp = class_pencils(plan)   # thin-tile columns M-2, M-1 and the Nyquist slot M on the l % 4 == 2 row (5 kz per class)
+        pairs += [cp[0 * 5 + 1], cp[1 * 5 + 0], cp[2 * 5 + 2], cp[2 * 5 + 3], cp[2 * 5 + 4], cp[3 * 5 + 3]]
+    elif classes:
         pairs += class_pencils(plan)
     pairs += [(int(rng.integers(0, Ny)), int(rng.integers(0, Nz // 2 + 1))) for _ in range(n_random)]
     kys, kzs = zip(*pairs)
@@ -228,7 +231,9 @@ def test_config4_2048_fp32_runs_in_hbm(fft, oracle_mod):
     work = plan.empty_workspace()
     plan.r2c(field, spec, work)
     assert plan.index(2047, 2047, 1024) == 2048 * 2048 * 1025 - 1 > 2 ** 32
-    check_forward_pencils(oracle_mod, plan, field.cpu().numpy(), spec, dtype, n_random=0, classes=False)
+    host = field.cpu().numpy()
+    check_forward_pencils(oracle_mod, plan, host, spec, dtype, n_random=0, classes="few")
+    del host
     assert parseval_rel_err(plan, field, spec) <= 1e-5
     back = torch.empty_like(field)
     plan.c2r(spec, back, work)
@@ -238,6 +243,15 @@ def test_config4_2048_fp32_runs_in_hbm(fft, oracle_mod):
         err = max(err, float((bl[a:a + (1 << 30)] - fl[a:a + (1 << 30)]).abs().max()))
     assert err <= tol(shape, dtype)
     del spec, back, field, work
+    torch.cuda.empty_cache()
+    # the inverse against Eq. (2)+(3) point by point (the quarter-tile x kernel runs at this size only): the oracle
+    # reads the 34 GB spectrum from host memory
+    import psutil
+    assert plan.launch_impls(1)[1] == "tma_split4", plan.launch_impls(1)
+    if psutil.virtual_memory().available < 48 * 2 ** 30:
+        plan.close()
+        pytest.skip("forward and round trip passed; the sampled 2048^3 inverse needs a 34 GB host copy of the spectrum")
+    check_inverse_points(oracle_mod, fft, plan, dtype, n_points=16)
     plan.close()
     torch.cuda.empty_cache()
 
