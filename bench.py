@@ -7,9 +7,12 @@ on the 1024^3 fp32 grid of BASELINE.json configs[2], inputs resident in HBM.
 Prints ONE JSON line (rank 0).  `value` = GFLOP/s by BASELINE.json's convention
 (2.5 N^3 log2 N^3 per real transform, 5 per pair; the paper's convention, is 2x).
 Multi-GPU (torchrun): the ONE grid is slab-decomposed over the N ranks -- the paper's method
-(paper_2202_12756_b200/dist.py) -- so the scaling is strong; `--exchange chunks`
-(default: all-to-all over NCCL between the stages) or `unified` (the y pass stores straight into the
-peers' memory over NVLink).  `--impl reference` times the fp64 CPU oracle on a bounded sample (rank 0 only).
+(paper_2202_12756_b200/dist.py) -- so the scaling is strong; `--exchange unified`
+(the y pass stores straight into the peers' memory over NVLink; what `auto`, the default, picks wherever the
+VMM peer mapping can work) or `chunks` (all-to-all over NCCL between the stages); the line carries both
+back-ends' T_comm.  `--gpus N` must match the launcher's WORLD_SIZE (N > 1: torchrun), else the run exits non-zero.
+The default single-GPU run also times a few pairs of the other BASELINE.json configs (1536^3 and 2048^3 fp32,
+1024^3 fp64) into `config.other_configs`.  `--impl reference` times the fp64 CPU oracle on a bounded sample (rank 0 only).
 """
 from __future__ import annotations
 
@@ -303,6 +306,76 @@ def alg_bytes_per_launch(plan_real_bytes):
     return {k: b for k in ("z_r2c", "y_c2c_fwd", "x_c2c_fwd", "x_c2c_inv", "y_c2c_inv", "z_c2r", "zy_r2c_fused", "yz_c2r_fused")}
 
 
+OTHER_CONFIGS = (   # (n, dtype name, generator, virtual_slabs, label): the BASELINE.json configs beside the headline
+    (1536, "f32", "normal", 16, "configs[3]: 1536^3 fp32 i.i.d. N(0,1)"),
+    (2048, "f32", "uniform", 128, "configs[4]: 2048^3 fp32 i.i.d. uniform[-1,1)"),
+    (1024, "f64", "uniform", 128, "configs[4]: 1024^3 fp64 i.i.d. uniform[-1,1)"),
+)
+
+
+def other_config_leg(pkg, n, dname, kind, p, label, dev, local_rank, steps=3, warmup=2):
+    """A few R2C+C2R pairs of another BASELINE.json config, timed like the headline (CUDA events around `steps` pairs
+    after `warmup`, clocks sampled during them), plus the per-kernel durations and the round trip.  Device timed only."""
+    import torch
+    from paper_2202_12756_b200 import inputs
+    dtype = torch.float32 if dname == "f32" else torch.float64
+    shape = (n, n, n)
+    free, _tot = torch.cuda.mem_get_info(dev)
+    esize = 4 if dname == "f32" else 8
+    need = 4.1 * n ** 3 * esize
+    if free < need:
+        return {"workload": label, "dtype": dname, "skipped": "needs %.0f GiB of free HBM, %.0f free" % (need / 2 ** 30, free / 2 ** 30)}
+    plan = pkg.Plan(*shape, dtype=dtype, virtual_slabs=p)
+    gen = inputs.normal_grid if kind == "normal" else inputs.uniform_grid
+    field = gen(shape, dtype, seed=0, device=dev)
+    spec, back, work = plan.empty_complex(dev), plan.empty_real(dev), plan.empty_workspace(dev)
+    stream = torch.cuda.current_stream(dev)
+
+    def step():
+        plan.r2c(field, spec, work, stream)
+        plan.c2r(spec, back, work, stream)
+
+    for _ in range(warmup):
+        step()
+    torch.cuda.synchronize()
+    sampler = ClockSampler(local_rank)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(steps):
+        step()
+    e1.record(stream)
+    torch.cuda.synchronize()
+    ms_step = e0.elapsed_time(e1) / steps
+    clocks = sampler.stop()
+    plan.timing_enable(steps)
+    for _ in range(steps):
+        step()
+    torch.cuda.synchronize()
+    per_kernel = {}
+    for which in (0, 1):
+        t, calls = plan.timing_read(which)
+        for k, v in t.items():
+            per_kernel[k] = v / max(1, calls)
+    plan.timing_enable(0)
+    rt = max((back[i] - field[i]).abs().max().item() for i in range(n)) / max(field[i].abs().max().item() for i in range(n))
+    peak, _src = measured_peak()
+    alg = {k: v for k, v in alg_bytes_per_launch(plan.real_bytes).items() if k in per_kernel}
+    impls = dict(zip(plan.launch_names(0) + plan.launch_names(1), plan.launch_impls(0) + plan.launch_impls(1)))
+    out = {"workload": "%s, R2C+C2R pair, virtual_slabs=%d" % (label, p), "dtype": dname, "steps": steps, "warmup": warmup,
+           "ms_per_step": ms_step, "value_gflops": job_gflops(shape, ms_step * 1e-3),
+           "all_kernels_ms": per_kernel, "all_kernels_impl": impls,
+           "all_kernels_frac_of_hbm_peak": {k: alg[k] / (per_kernel[k] * 1e-3) / 1e9 / peak for k in alg},
+           "array_passes_per_pair": len(alg),
+           "pair_frac_of_pass_roofline": (sum(alg.values()) / peak / 1e9) / (ms_step * 1e-3),
+           "pair_frac_of_one_read_one_write": (2 * 2 * plan.real_bytes / peak / 1e9) / (ms_step * 1e-3),
+           "round_trip_rel_err": rt, "round_trip_bound": (2e-6 if dname == "f32" else 1e-13) * math.log2(n ** 3),
+           "clocks": clocks}
+    plan.close()
+    del field, spec, back, work
+    torch.cuda.empty_cache()
+    return out
+
+
 def run_cuda(args):
     import torch
     import paper_2202_12756_b200 as pkg
@@ -402,7 +475,7 @@ def run_cuda(args):
         h_back = torch.empty(shape, dtype=torch.float32).pin_memory()
         h_in.copy_(field)
         # free the device-resident bench buffers first: the host entry points own their own
-        del spec, back, work
+        spec = back = work = None
         torch.cuda.empty_cache()
         plan.r2c_host(h_in, h_spec)                     # warm-up (allocates the plan's buffers)
         plan.c2r_host(h_spec, h_back)
@@ -418,6 +491,15 @@ def run_cuda(args):
                "h2d_bytes_per_step": real_b + cplx_b, "d2h_bytes_per_step": cplx_b + real_b,
                "round_trip_rel_err": e2e_rt}
 
+    # ---- the other BASELINE.json configs, a few pairs each, after the headline has released its buffers ----
+    n_launches = args.steps * (plan.launches(0) + plan.launches(1))
+    other = None
+    if n == 1024 and not args.no_other_configs:
+        plan.close()                                    # also frees the host entry points' device buffers
+        field = spec = back = work = None
+        torch.cuda.empty_cache()
+        other = [other_config_leg(pkg, *cfg, dev, local_rank) for cfg in OTHER_CONFIGS]
+
     line = {
         "metric": METRIC, "value": value, "unit": "GFLOP/s", "n_gpus": 1,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_step,
@@ -428,9 +510,10 @@ def run_cuda(args):
                          % (real_b / 2 ** 30),
                    "parallelism": "1 GPU",
                    "gflops_paper_convention": 2 * value,
-                   "round_trip_rel_err": rt_err, "round_trip_bound": tol},
+                   "round_trip_rel_err": rt_err, "round_trip_bound": tol,
+                   "other_configs": other},
         "clocks": clocks, "e2e": e2e,
-        "gpu_launches": args.steps * (plan.launches(0) + plan.launches(1)),
+        "gpu_launches": n_launches,
         "roofline": roofline, "cpu_baseline": cpu_baseline,
     }
     print(json.dumps(line), flush=True)
@@ -438,6 +521,39 @@ def run_cuda(args):
         raise SystemExit("round trip error %.3e exceeds %.3e: the timed path is wrong" % (rt_err, tol))
     if cpu_baseline and cpu_baseline.get("gpu_vs_oracle_rel_l2", 0.0) > tol:
         raise SystemExit("the timed spectrum is off the oracle by %.3e (bound %.3e)" % (cpu_baseline["gpu_vs_oracle_rel_l2"], tol))
+
+
+def dist_launches_per_pair(plan):
+    """Kernels one rank launches per R2C+C2R pair: the stages of the plan's current variant (fft3d_launches counts the
+    z/y/x passes and the Nyquist fix-ups of both directions) plus the two plane-extraction kernels of the distributed
+    bookkeeping (fft3d_dist_fwd_col0, fft3d_dist_inv_planes)."""
+    lib = plan._lib
+    return int(lib.fft3d_launches(plan._h, 0)) + int(lib.fft3d_launches(plan._h, 1)) + 2
+
+
+def choose_exchange(asked, D, dist, dev, n, world, rank):
+    """'unified' (the y pass stores into / loads from the peers' memory over a CUDA-VMM mapping) where it
+    can work, else 'chunks' (NCCL all-to-all).  It needs: a part size that is a multiple of the VMM granularity, peer
+    access from this GPU to every other rank's GPU, and all ranks on one host.  Every rank takes the same decision (MIN
+    over the ranks).  Returns (exchange, reason)."""
+    import torch
+    if asked in ("chunks", "unified"):
+        return asked, "asked for"
+    part = 8 * n * (n // world) * (n // 2)              # [Nx][Ny/G][Nz/2] complex64
+    ok, why = True, "VMM peer mapping usable"
+    if not D.UnifiedExchange.usable(part):
+        ok, why = False, "part size %d is not a multiple of the VMM granularity" % part
+    elif world > 1:
+        me = dev.index
+        peers = [g for g in range(torch.cuda.device_count()) if g != me][:world - 1]
+        if len(peers) < world - 1 or not all(torch.cuda.can_device_access_peer(me, g) for g in peers):
+            ok, why = False, "no peer access between the ranks' GPUs"
+    if world > 1:
+        t = torch.tensor([1.0 if ok else 0.0], device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MIN)
+        if ok and t.item() < 1.0:
+            ok, why = False, "another rank cannot use the VMM peer mapping"
+    return ("unified" if ok else "chunks"), ("auto: " + why)
 
 
 def run_cuda_dist(args):
@@ -460,7 +576,8 @@ def run_cuda_dist(args):
     label, kind, _p = workload_for(n)
     shape = (n, n, n)
     Nxl = n // world
-    fft = D.SlabFFT.create(n, n, n, torch.float32, dist, dev, exchange=args.exchange)
+    exchange, why = choose_exchange(args.exchange, D, dist, dev, n, world, rank)
+    fft = D.SlabFFT.create(n, n, n, torch.float32, dist, dev, exchange=exchange)
     plan = fft.plan
     field = make_field(kind, shape, 0, dev, x_range=(rank * Nxl, (rank + 1) * Nxl))
     spec = plan.empty_spec_part(dev)
@@ -497,6 +614,18 @@ def run_cuda_dist(args):
     fft.timed = False
     t_comp = max_over_ranks(fft.times["comp"] / args.steps, dist, dev)
     t_comm = max_over_ranks(fft.times["comm"] / args.steps, dist, dev)
+    # the other exchange back-end, a few steps, for its T_comm beside the timed one's (same kernels, same buffers)
+    t_comm_other, other = None, ("chunks" if exchange == "unified" else "unified")
+    if other == "chunks" or choose_exchange("auto", D, dist, dev, n, world, rank)[0] == "unified":
+        fft2 = D.SlabFFT.create(n, n, n, torch.float32, dist, dev, exchange=other)
+        for k in range(1 + args.steps):
+            fft2.timed = k > 0
+            fft2.forward(field, spec)
+            fft2.inverse(spec, back)
+        barrier()
+        fft2.collect_times()
+        t_comm_other = max_over_ranks(fft2.times["comm"] / args.steps, dist, dev)
+        fft2.close()
     rt_num = max_over_ranks((back - field).abs().max().item(), dist, dev)
     rt_den = max_over_ranks(field.abs().max().item(), dist, dev)
     rt_err = rt_num / rt_den
@@ -536,13 +665,14 @@ def run_cuda_dist(args):
             "data": "synthetic",
             "config": {"workload": "%s, R2C+C2R pair, slab-decomposed over %d GPUs" % (label, world),
                        "l2": "per-rank arrays are %.2f GiB; inputs are not re-used between steps" % (4 * n ** 3 / world / 2 ** 30),
-                       "parallelism": "slab decomposition x%d (PAPER.md:54), exchange=%s" % (world, args.exchange),
+                       "parallelism": "slab decomposition x%d (PAPER.md:54), exchange=%s (%s)" % (world, exchange, why),
+                       "t_comm_ms_by_exchange": {exchange: t_comm, other: t_comm_other},
                        "gflops_paper_convention": 2 * value,
                        "t_comp_ms": t_comp, "t_comm_ms": t_comm, "comm_fraction_r": t_comm / max(1e-9, t_comp + t_comm),
                        "chunk_bytes": 8 * (n // world) * (n // world) * (n // 2),
                        "round_trip_rel_err": rt_err, "round_trip_bound": tol},
             "clocks": clocks, "e2e": e2e,
-            "gpu_launches": args.steps * 2 * 5,
+            "gpu_launches": args.steps * dist_launches_per_pair(plan),
             "roofline": {"bound": "hbm", "kernel": "pair", "achieved": 6 * arr / world / (ms_step * 1e-3) / 1e9,
                          "peak": peak, "unit": "GB/s", "frac": 6 * arr / world / (ms_step * 1e-3) / 1e9 / peak,
                          "traffic": None, "peak_source": peak_src,
@@ -640,15 +770,24 @@ def main():
     ap.add_argument("--size", "--n", dest="n", type=int, default=1024)
     ap.add_argument("--slabs", type=int, default=0, help="virtual_slabs (0: the value BASELINE.json gives for the size)")
     ap.add_argument("--dist", action="store_true", help="run the slab-decomposed driver even with one rank")
-    ap.add_argument("--exchange", default="chunks", choices=["chunks", "unified"],
-                    help="N > 1: all-to-all of chunks over NCCL, or stores straight into the peers' memory (VMM)")
+    ap.add_argument("--exchange", default="auto", choices=["auto", "chunks", "unified"],
+                    help="N > 1: stores straight into the peers' memory (VMM mapping; auto picks it where it can work), "
+                         "or an all-to-all of chunks over NCCL; the other one's T_comm is reported beside the timed one's")
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-other-configs", action="store_true",
+                    help="default run only: skip the few pairs of 1536^3 / 2048^3 fp32 and 1024^3 fp64 reported in config.other_configs")
     ap.add_argument("--transform", default="r2c", choices=["r2c", "c2c"],
                     help="r2c (default): the headline R2C+C2R pair; c2c: the 3D C2C pair (single GPU, no e2e leg)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "cuda" else args.warmup
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if args.impl == "cuda" and args.gpus != world:
+        # never print an n_gpus = 1 line for an N-GPU request (or the reverse): the launcher decides the world size
+        raise SystemExit("bench.py --gpus %d was started with WORLD_SIZE=%d: launch it as `python -m torch.distributed.run "
+                         "--nnodes=1 --nproc-per-node %d --master-addr 127.0.0.1 --master-port P bench.py --gpus %d ...`"
+                         % (args.gpus, world, args.gpus, args.gpus))
     if args.impl == "reference":
         run_reference(args)
     elif args.transform == "c2c":
